@@ -1,0 +1,117 @@
+/* vh.h -- C ABI of the B200-native Kurganov-Tadmor / Heun step for 3+1d relativistic viscous hydrodynamics
+ * (arXiv 1608.06577, "GPU-VH").  Citations are PAPER.md line numbers / equation numbers.
+ *
+ * The library advances, entirely on one GPU, the 15 double-precision fields per cell
+ *   q = (T^tt, T^tx, T^ty, T^tn,  pi^tt, pi^tx, pi^ty, pi^tn, pi^xx, pi^xy, pi^xn, pi^yy, pi^yn, pi^nn,  Pi)
+ * (Eqs. 56-58, :357-363; pi^{y eta} restored, reading R2) by the program flow of PAPER.md :503-529:
+ * two forward-Euler stages of the KT semi-discrete scheme (Eqs. 59-68) combined as Heun/RK2 (Eqs. 69-71), each stage
+ * followed by the per-cell inversion to (e, p, u^mu) (Eqs. 52-54, 72), the regularisation of pi^{mu nu}, Pi
+ * (Eqs. 73-74) and the ghost-cell boundary condition (Eqs. 75-76).
+ *
+ * Conventions for EVERY array argument:
+ *   - physical cells only (no ghost cells), double precision,
+ *   - index order x fastest, then y, then eta_s, then event (batch):  idx = i + nx*(j + ny*(k + nz*b)),
+ *   - multi-component arrays are component-major SoA: u4 = 4 consecutive arrays (u^tau,u^x,u^y,u^eta: contravariant, :251),
+ *     pi10 = 10 consecutive arrays in the order of q[4..13], q15 = 15 consecutive arrays,
+ *   - mem_space 0: host pointer, 1: device pointer (e.g. the storage of a torch tensor) valid on the handle's stream,
+ *   - the caller owns what it passes and may free it when the call returns; the library owns its padded internal buffers.
+ * Units: natural units, e and pressures in fm^-4, T in fm^-1, lengths in fm (reading R13).
+ *
+ * Every function returns VH_OK (0) or a negative error code and never throws or aborts; vh_last_error() gives a
+ * message for the most recent failure on that handle (or the global message when the handle is NULL).
+ * All work of vh_set_initial / vh_step / vh_get_fields is enqueued on the CUDA stream given to vh_create;
+ * vh_step is asynchronous; vh_get_fields and vh_get_status synchronise that stream before returning.
+ * There is no CPU fallback: without a CUDA device vh_create fails with VH_ERR_CUDA.
+ */
+#ifndef VH_H_
+#define VH_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VH_OK 0
+#define VH_ERR_ARG (-1)      /* NULL pointer, non-positive size, unsupported combination */
+#define VH_ERR_ALLOC (-2)    /* device allocation failed */
+#define VH_ERR_CUDA (-3)     /* CUDA runtime error (message in vh_last_error) */
+#define VH_ERR_STATE (-4)    /* call out of order (e.g. vh_step before vh_set_initial) */
+
+typedef struct vh_handle vh_handle;
+
+typedef struct {
+  int nx, ny, nz, n_batch;          /* physical cells per event; nz == 1 -> 2+1d (:474); n_batch >= 1 independent events  */
+  double dx, dy, dz;                /* fm, fm, rapidity units                                                           */
+  double tau0, dtau;                /* fm                                                                               */
+  int geometry;                     /* 0 Milne (Eqs. 27-29); 1 Cartesian, ideal only: G terms off, tau^2 -> 1 (:684)      */
+  int physics;                      /* bit0 shear pi^{mu nu}, bit1 bulk Pi; 0 = ideal (pi, Pi stay 0)                     */
+  int eos;                          /* 0: p = e/3;  1: p = (e/3)(1 - alpha exp(-e/e0));  T = (e/a)^{1/4} for both          */
+  double eos_a, eos_alpha, eos_e0;
+  double eta_over_s;                /* constant                                                                         */
+  int zeta_model;                   /* 0: zeta/s = 0; 1: amp*exp(-((T-T0)/width)^2) (BASELINE configs 3-5); 2: constant   */
+  double zeta_amp, zeta_T0, zeta_width;  /* T0, width in fm^-1                                                            */
+  double c_tau_pi;                  /* tau_pi = c_tau_pi*eta/(e+p); Eq. 13 -> 5                                          */
+  double c_tau_Pi;                  /* tau_Pi = c_tau_Pi*zeta/((e+p)(1/3-cs2)^2); configs 5, Eq. 10 -> 1/15              */
+  double delta_pipi, tau_pipi, lambda_piPi;    /* delta_pipi/tau_pi, tau_pipi/tau_pi, lambda_piPi/tau_pi: 4/3, 10/7, 6/5 (Eqs. 14-16) */
+  double delta_PiPi, lambda_Pipi_coef;         /* delta_PiPi/tau_Pi = 2/3, lambda_Pipi/tau_Pi = coef*(1/3-cs2), coef 8/5 (Eqs. 11-12) */
+  double minmod_theta;              /* flux limiter theta in [1,2], Eq. 67                                              */
+  double xi0, rho_max;              /* Eq. 74: 0.1, 1 (:445)                                                            */
+  int newton_max_iter;              /* Newton-Raphson cap for Eq. 72 (reading R6: 50)                                   */
+  double newton_rtol;               /* stop when |de| <= rtol*|e| (1e-13)                                               */
+  double tau_relax_floor_over_dtau; /* c: 1/tau_Pi, 1/tau_pi <= 1/(c*dtau) (reading R14); 0 disables                    */
+} vh_params;
+
+/* Create a solver for the grid / physics in *p on the current CUDA device.  cuda_stream: a cudaStream_t (may be NULL =
+ * default stream).  Allocates 61 padded SoA arrays (3 x 15 q, 3 x 4 u, 2 x e, 2 x p; :470-476 plus the ping-pong copy of
+ * e, p needed because inversion is fused into the stage kernel).  *out is set only on success.                         */
+int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out);
+
+/* Program-flow steps 3-5 (:489-491): build q^0 from (e, u^mu, pi^{mu nu}, Pi) by Eqs. 32-33 (:267-269), p = P0(e),
+ * u^{-1} = u^0 (footnote 4, :519), fill ghost cells, reset tau = tau0 and all counters.  pi10 / Pi may be NULL (= 0).  */
+int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double* pi10, const double* Pi, int mem_space);
+
+/* Optional, for a bit-exact restart: overwrite u^{n-1} (otherwise equal to u^n after vh_set_initial).                  */
+int vh_set_uprev(vh_handle* h, const double* u4_prev, int mem_space);
+
+/* Bit-exact restart from a state exported by vh_get_fields: installs q, e, u^n, u^{n-1} as they are (p = P0(e) is
+ * recomputed, ghost cells refilled), sets the step counter so that tau = tau0 + n_steps_done*dtau, resets the status counters.
+ * (vh_set_initial cannot do this: it rebuilds T^{tau mu} from the primitives, and pi^{mu nu} is regulated AFTER the
+ * inversion - program-flow steps 2-3 - so (e, u, pi, Pi) no longer reproduce the stored T^{tau mu} exactly.)               */
+int vh_set_state(vh_handle* h, const double* q15, const double* e, const double* u4, const double* u4_prev, long long n_steps_done,
+                 int mem_space);
+
+/* Advance n_steps full RK2 steps (program-flow steps 1-9, :503-529).  Asynchronous on the handle's stream.             */
+int vh_step(vh_handle* h, int n_steps);
+
+/* Same as vh_step, but brackets each of the four launches of a step (stage 1, ghost 1, stage 2, ghost 2) with CUDA events
+ * on the handle's stream and returns their mean durations in milliseconds in ms4[0..3] (for per-kernel roofline numbers;
+ * synchronises once per step, so use vh_step for throughput).                                                            */
+int vh_step_profile(vh_handle* h, int n_steps, double* ms4);
+
+/* Copy the state at the current tau to caller arrays; any of q15, e, p, u4, u4_prev may be NULL.  p is P0(e).          */
+int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, double* u4_prev, int mem_space);
+
+/* tau, number of steps done, number of failed Newton inversions (interface states and cells, both stages), number of
+ * cells whose inversion produced a non-finite e or u^tau, smallest regularisation factor tanh(rho)/rho applied.
+ * Any pointer may be NULL.  Synchronises the stream.                                                                   */
+int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long* n_inversion_failures,
+                  long long* n_nonfinite, double* min_reg_factor);
+
+/* Number of kernels launched on the handle since vh_create (for bench.py's gpu_launches).                             */
+long long vh_launch_count(vh_handle* h);
+
+/* Select the stage-kernel implementation: 0 = default (best available), other values select alternatives for A/B
+ * measurements.  Returns VH_ERR_ARG for an unknown variant.                                   */
+int vh_set_kernel_variant(vh_handle* h, int variant);
+
+/* Device peaks measured with this library's own microbenchmarks on the handle's device and stream:
+ * FP64 stream copy (GB/s, read+write bytes) over n_bytes (>= 1 GiB recommended) and a dependent-free FP64 FMA kernel
+ * (GFLOP/s, 2 flops per FMA) on all SMs; each the best of `repeats`.  Either output may be NULL.                       */
+int vh_measure_peaks(void* cuda_stream, long long n_bytes, int repeats, double* copy_gbs, double* fp64_gflops);
+
+const char* vh_last_error(vh_handle* h);
+void vh_destroy(vh_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VH_H_ */

@@ -23,6 +23,9 @@
 // substituted (oracle/vh_oracle_capi.cpp instantiates double and a counting type).
 // =====================================================================================
 #pragma once
+#ifndef VHO_COUNTING_SECTION
+#define VHO_COUNTING_SECTION(x) ((void)0)     // used only by vh_oracle_count.cpp (operation counting)
+#endif
 #include <cmath>
 #include <cstddef>
 #include <limits>
@@ -87,9 +90,10 @@ template <class R> inline Thermo<R> eos(const Params& P, R e) {
     t.p = (e / R(3)) * (R(1) - R(P.eos_alpha) * ex);
     t.cs2 = (R(1) / R(3)) * (R(1) - R(P.eos_alpha) * ex * (R(1) - x));   // dp/de
   }
-  t.T = pow(e / R(P.eos_a), R(0.25));
+  t.T = R(0);     // filled by temperature() where it is needed (transport coefficients only)
   return t;
 }
+template <class R> inline R temperature(const Params& P, R e) { return pow(e / R(P.eos_a), R(0.25)); }   // e = a T^4
 
 template <class R> struct Transport {
   R inv_tau_pi, eta_over_tau_pi;        // 1/tau_pi, eta/tau_pi
@@ -249,7 +253,7 @@ template <class R> class Solver {
 
   // ------------------------------------------------------------ interface state -> v_r   (:424, Alg. 3 :667-672; R5, R6)
   // qs: a reconstructed conserved state; returns the three v^i = M_i/(E+P) of that state.
-  void state_velocity(const R* qs, R t, R guess, R v[3]) {
+  void state_velocity(const R* qs, R t, R guess, bool count, R v[3]) {
     R E = qs[0] - qs[4];
     R M[3] = {qs[1] - qs[5], qs[2] - qs[6], qs[3] - qs[7]};
     R M2 = M[0] * M[0] + M[1] * M[1] + tau2(t) * M[2] * M[2];          // :339
@@ -259,7 +263,7 @@ template <class R> class Solver {
     R den = E + th.p + qs[14];
     for (int i = 0; i < 3; ++i) v[i] = M[i] / den;
     if (fail) {
-      ++n_fail;
+      if (count) ++n_fail;
       last_fail[0] = (double)E; last_fail[1] = (double)M2; last_fail[2] = (double)qs[14]; last_fail[3] = (double)guess;
       for (int i = 0; i < 3; ++i) {                                      // R6: clip |v|<1
         if (!(absr(v[i]) < R(1))) v[i] = (v[i] > R(0)) ? R(1) - R(1e-12) : ((v[i] < R(0)) ? R(-1) + R(1e-12) : R(0));
@@ -269,7 +273,7 @@ template <class R> class Solver {
 
   // Numerical flux H at the interface between stencil cells c and c+1 (Eq. 61), direction r.
   // I[n][0..4] = q_n at i-2..i+2 ; eI = e at the same cells ; c = 2 -> H_{i+1/2}, c = 1 -> H_{i-1/2}.
-  void flux(const R I[NQ][5], const R eI[5], int c, int r, R dr, R t, R H[NQ]) {
+  void flux(const R I[NQ][5], const R eI[5], int c, int r, R dr, R t, bool count, R H[NQ]) {
     R qm[NQ], qp[NQ];
     R th = R(P.minmod_theta);
     for (int n = 0; n < NQ; ++n) {
@@ -280,8 +284,8 @@ template <class R> class Solver {
       qp[n] = I[n][c + 1] - (dr / R(2)) * sn;     // q^+: Eq. 63 / 65
     }
     R vm[3], vp[3];
-    state_velocity(qm, t, eI[c], vm);             // guess: e of the cell the state was extrapolated from (R6)
-    state_velocity(qp, t, eI[c + 1], vp);
+    state_velocity(qm, t, eI[c], count, vm);      // guess: e of the cell the state was extrapolated from (R6)
+    state_velocity(qp, t, eI[c + 1], count, vp);
     R a = maxr(absr(vp[r]), absr(vm[r]));         // Eq. 62 with rho = |v_r| (:388)
     for (int n = 0; n < NQ; ++n) H[n] = (vp[r] * qp[n] + vm[r] * qm[n]) / R(2) - a * (qp[n] - qm[n]) / R(2);   // Eq. 61
   }
@@ -375,6 +379,7 @@ template <class R> class Solver {
     for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) W[m][n] = (nab[m][n] - nab[n][m]) / R(2);
 
     Thermo<R> th = eos(P, ec);
+    th.T = temperature(P, ec);
     Transport<R> tc = transport(P, ec, th);
 
     R pisig = R(0);                        // pi^{mu nu} sigma_{mu nu}
@@ -424,8 +429,14 @@ template <class R> class Solver {
           eI[d] = ei[sn];
         }
         R Hp[NQ], Hm[NQ];
-        flux(I, eI, 2, r, dr[r], t, Hp);
-        flux(I, eI, 1, r, dr[r], t, Hm);
+        // diagnostics only: each interface state is counted once in n_fail (H_{+1/2} by this cell, H_{-1/2} only by the first
+        // cell of the row) and not at all along a direction of extent 1, where H_{+1/2} - H_{-1/2} vanishes identically
+        const int ext[3] = {P.nx, P.ny, P.nz};
+        const int pos[3] = {i, j, k};
+        VHO_COUNTING_SECTION(1);
+        flux(I, eI, 2, r, dr[r], t, ext[r] > 1, Hp);
+        flux(I, eI, 1, r, dr[r], t, ext[r] > 1 && pos[r] == 2, Hm);
+        VHO_COUNTING_SECTION(0);
         for (int n = 0; n < NQ; ++n) C[n] -= (Hp[n] - Hm[n]) / dr[r];
       }
       for (int n = 0; n < NQ; ++n) qo[n][s] = qi[n][s] + R(P.dtau) * C[n];

@@ -76,6 +76,7 @@ def lib():
         L.vho_transport.argtypes = [C.POINTER(Params), C.c_double, dp]
         L.vho_invert.restype = C.c_double
         L.vho_invert.argtypes = [C.POINTER(Params), C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.vho_count_ops.argtypes = [C.POINTER(Params), dp, dp, dp, dp, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
         L.vho_time_steps.restype = C.c_double
         L.vho_time_steps.argtypes = [C.c_void_p, C.c_int]
         assert L.vho_params_size() == C.sizeof(Params), "Params layout mismatch"
@@ -199,3 +200,35 @@ def invert(params: dict, E, M2, Pi, guess):
     it, fl = C.c_int(), C.c_int()
     e = lib().vho_invert(C.byref(P), float(E), float(M2), float(Pi), float(guess), C.byref(it), C.byref(fl))
     return e, it.value, fl.value
+
+
+OP_CLASSES = ("add", "mul", "div", "cmp", "sqrt", "exp", "pow", "tanh")
+# flop weights of SURVEY.md 8(d): add/mul/compare 1, div 10, sqrt 15, exp 25, tanh 40; pow(x, 1/4) = two sqrt
+OP_WEIGHTS = dict(add=1, mul=1, div=10, cmp=1, sqrt=15, exp=25, pow=30, tanh=40)
+
+
+def count_ops(params: dict, e, u4, pi10=None, Pi=None, warm=1, n=1):
+    """Operation counts of n RK2 steps with the counting scalar (after `warm` uncounted steps).
+    Returns dict(other={class: count}, flux={class: count}) summed over all cells."""
+    P = make_params(params)
+    shape = (P.n_batch, P.nz, P.ny, P.nx)
+    e = np.ascontiguousarray(e, dtype=np.float64).reshape(shape)
+    u4 = np.ascontiguousarray(u4, dtype=np.float64).reshape((4,) + shape)
+    pi10 = None if pi10 is None else np.ascontiguousarray(pi10, dtype=np.float64).reshape((10,) + shape)
+    Pi = None if Pi is None else np.ascontiguousarray(Pi, dtype=np.float64).reshape(shape)
+    out = (C.c_longlong * 16)()
+    rc = lib().vho_count_ops(C.byref(P), _dp(e), _dp(u4), _dp(pi10), _dp(Pi), int(warm), int(n), out)
+    if rc < 0:
+        raise ValueError("vho_count_ops needs n_batch == 1")
+    vals = list(out)
+    return dict(other=dict(zip(OP_CLASSES, vals[:8])), flux=dict(zip(OP_CLASSES, vals[8:])))
+
+
+def algorithmic_flops_per_cell_update(params: dict, e, u4, pi10=None, Pi=None):
+    """Weighted flops per cell per RK2 step with every interface charged once (flux section / 2), and the raw counts."""
+    c = count_ops(params, e, u4, pi10, Pi, warm=1, n=1)
+    ncell = params["nx"] * params["ny"] * params["nz"]
+    per = {k: (c["other"][k] + 0.5 * c["flux"][k]) / ncell for k in OP_CLASSES}
+    flops = sum(OP_WEIGHTS[k] * per[k] for k in OP_CLASSES)
+    plain = per["add"] + per["mul"] + per["div"] + per["sqrt"] + per["cmp"]
+    return flops, plain, per

@@ -96,16 +96,16 @@ void vho_flux_at(vho_handle* h, int ev, int i, int j, int k, int r, int upper, d
   double I[15][5], eI[5];
   size_t c0 = s->idx(i, j, k);
   for (int d = 0; d < 5; ++d) { size_t sn = c0 + d * stride[r] - 2 * stride[r]; for (int n = 0; n < 15; ++n) I[n][d] = s->q[n][sn]; eI[d] = s->e[sn]; }
-  s->flux(I, eI, upper ? 2 : 1, r, dr[r], tau, H15);
+  s->flux(I, eI, upper ? 2 : 1, r, dr[r], tau, false, H15);
 }
 void vho_post(vho_handle* h, int ev, double tau) { Sol* s = h->ev[ev]; s->post(s->q, s->u, tau); }
 void vho_ghost(vho_handle* h, int ev) { Sol* s = h->ev[ev]; s->ghost(s->q, s->e, s->p, s->u); }
 
 // ---- scalar pieces
 double vho_minmod3(double x, double y, double z) { return vho::minmod3(x, y, z); }
-void vho_eos(const vho::Params* P, double e, double* out3) { auto t = vho::eos<double>(*P, e); out3[0] = t.p; out3[1] = t.cs2; out3[2] = t.T; }
+void vho_eos(const vho::Params* P, double e, double* out3) { auto t = vho::eos<double>(*P, e); t.T = vho::temperature<double>(*P, e); out3[0] = t.p; out3[1] = t.cs2; out3[2] = t.T; }
 void vho_transport(const vho::Params* P, double e, double* out5) {
-  auto t = vho::eos<double>(*P, e); auto c = vho::transport<double>(*P, e, t);
+  auto t = vho::eos<double>(*P, e); t.T = vho::temperature<double>(*P, e); auto c = vho::transport<double>(*P, e, t);
   out5[0] = c.inv_tau_pi; out5[1] = c.eta_over_tau_pi; out5[2] = c.inv_tau_Pi; out5[3] = c.zeta_over_tau_Pi; out5[4] = c.lambda_Pipi_over_tau_Pi;
 }
 double vho_invert(const vho::Params* P, double E, double M2, double Pi, double guess, int* iters, int* failed) {

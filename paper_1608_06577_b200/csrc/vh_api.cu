@@ -1,0 +1,452 @@
+// vh_api.cu -- C ABI (include/vh.h): handle, buffers, buffer rotation (PAPER.md program-flow steps 7, 9), kernel dispatch.
+#include "../../include/vh.h"
+#include "vh_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+
+using namespace vh;
+
+static thread_local std::string g_err;
+
+struct vh_handle {
+  vh_params prm;
+  DevParams P;
+  cudaStream_t stream = nullptr;
+  double* pool = nullptr;            // 61 padded arrays
+  double* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
+  double* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
+  double* e[2] = {nullptr, nullptr};            // e^n / e^{n+1}, e*
+  double* p[2] = {nullptr, nullptr};
+  Counters* cnt = nullptr;
+  double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
+  double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
+  long long n_steps = 0;
+  long long launches = 0;
+  bool initialised = false;
+  bool two_d = false;
+  int variant = 0;
+  std::string err;
+};
+
+static int fail(vh_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg;
+  g_err = msg;
+  return code;
+}
+#define CUDA_TRY(h, call)                                                                              \
+  do {                                                                                                 \
+    cudaError_t _e = (call);                                                                           \
+    if (_e != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e)); \
+  } while (0)
+
+static long long round_up(long long a, long long m) { return (a + m - 1) / m * m; }
+
+static int fill_dev_params(const vh_params& p, DevParams& P) {
+  std::memset(&P, 0, sizeof(P));
+  P.nx = p.nx; P.ny = p.ny; P.nz = p.nz; P.n_batch = p.n_batch;
+  const bool two_d = (p.nz == 1);
+  P.NXp = (int)round_up(p.nx + 4, 16);
+  P.NYp = p.ny + 4;
+  P.NZp = two_d ? 1 : p.nz + 4;
+  P.zoff = two_d ? 0 : 2;
+  P.plane = (long long)P.NXp * P.NYp;
+  P.bstride = P.plane * P.NZp;
+  P.fstride = P.bstride * p.n_batch;
+  P.dx = p.dx; P.dy = p.dy; P.dz = p.dz; P.dtau = p.dtau;
+  P.inv_dx = 1.0 / p.dx; P.inv_dy = 1.0 / p.dy; P.inv_dz = 1.0 / p.dz; P.inv_dtau = 1.0 / p.dtau;
+  P.shear = (p.physics & 1) ? 1 : 0;
+  P.bulk = (p.physics & 2) ? 1 : 0;
+  P.eos_a_inv = 1.0 / p.eos_a; P.eos_alpha = p.eos_alpha; P.eos_e0_inv = (p.eos == 1) ? 1.0 / p.eos_e0 : 0.0;
+  P.inv_ctaupi_etas = 1.0 / (p.c_tau_pi * p.eta_over_s);
+  P.inv_ctaupi = 1.0 / p.c_tau_pi;
+  P.zeta_model = p.zeta_model; P.zeta_amp = p.zeta_amp; P.zeta_T0 = p.zeta_T0;
+  P.zeta_inv_width = (p.zeta_model == 1) ? 1.0 / p.zeta_width : 0.0;
+  P.inv_ctauPi = 1.0 / p.c_tau_Pi;
+  P.delta_pipi = p.delta_pipi; P.tau_pipi = p.tau_pipi; P.lambda_piPi = p.lambda_piPi;
+  P.delta_PiPi = p.delta_PiPi; P.lambda_Pipi_coef = p.lambda_Pipi_coef;
+  P.theta = p.minmod_theta;
+  P.inv_rho_max = 1.0 / p.rho_max; P.xi0_rho_max = p.xi0 * p.rho_max;
+  P.newton_max_iter = p.newton_max_iter; P.newton_rtol = p.newton_rtol;
+  P.debug = getenv("VH_DEBUG_FLAGS") ? atoi(getenv("VH_DEBUG_FLAGS")) : 0;
+  P.relax_clamp = (p.tau_relax_floor_over_dtau > 0.0) ? 1.0 / (p.tau_relax_floor_over_dtau * p.dtau) : std::numeric_limits<double>::infinity();
+  return 0;
+}
+
+static int check_params(const vh_params* p, std::string& why) {
+  if (!p) { why = "params is NULL"; return -1; }
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->n_batch < 1) { why = "grid extents and n_batch must be >= 1"; return -1; }
+  if (!(p->dx > 0 && p->dy > 0 && p->dz > 0 && p->dtau > 0)) { why = "spacings and dtau must be > 0"; return -1; }
+  if (p->geometry != 0 && p->geometry != 1) { why = "geometry must be 0 (Milne) or 1 (Cartesian)"; return -1; }
+  if (p->geometry == 1 && p->physics != 0) { why = "Cartesian geometry supports ideal physics only (PAPER.md:684)"; return -1; }
+  if (p->geometry == 0 && !(p->tau0 > 0)) { why = "Milne geometry needs tau0 > 0"; return -1; }
+  if (p->physics < 0 || p->physics > 3) { why = "physics must be a combination of bit0 (shear) and bit1 (bulk)"; return -1; }
+  if (p->eos != 0 && p->eos != 1) { why = "eos must be 0 or 1"; return -1; }
+  if (!(p->eos_a > 0)) { why = "eos_a must be > 0"; return -1; }
+  if (p->eos == 1 && !(p->eos_e0 > 0)) { why = "eos_e0 must be > 0"; return -1; }
+  if (p->physics != 0 && !(p->eta_over_s > 0 && p->c_tau_pi > 0 && p->c_tau_Pi > 0)) { why = "eta_over_s, c_tau_pi, c_tau_Pi must be > 0"; return -1; }
+  if (p->zeta_model < 0 || p->zeta_model > 2) { why = "zeta_model must be 0, 1 or 2"; return -1; }
+  if (p->zeta_model == 1 && !(p->zeta_width > 0)) { why = "zeta_width must be > 0"; return -1; }
+  if (!(p->minmod_theta >= 1.0 && p->minmod_theta <= 2.0)) { why = "minmod_theta must lie in [1,2] (Eq. 67)"; return -1; }
+  if (!(p->rho_max > 0 && p->xi0 > 0)) { why = "xi0, rho_max must be > 0"; return -1; }
+  if (p->newton_max_iter < 1 || !(p->newton_rtol > 0)) { why = "newton_max_iter >= 1 and newton_rtol > 0 required"; return -1; }
+  if ((long long)p->nz * p->n_batch > 65535) { why = "nz*n_batch exceeds the grid z limit (65535)"; return -1; }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------------ dispatch
+// VH_DEBUG_SYNC=1 in the environment: synchronise after every launch and name the kernel that faulted.
+static cudaError_t debug_sync(vh_handle* h, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  static const bool on = getenv("VH_DEBUG_SYNC") != nullptr;
+  if (e == cudaSuccess && on) {
+    e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) fprintf(stderr, "[vh] %s faulted at step %lld: %s\n", what, h->n_steps, cudaGetErrorString(e));
+  }
+  return e;
+}
+template <int EOS, bool VISC, bool MILNE, bool TWO_D>
+static cudaError_t launch_stage_t(vh_handle* h, int stage, const StageArgs& A) {
+  const DevParams& P = h->P;
+  dim3 block(32, 8);
+  dim3 grid((P.nx + 31) / 32, (P.ny + 7) / 8, P.nz * P.n_batch);
+  if (stage == 1) stage_cell_kernel<EOS, VISC, MILNE, TWO_D, 1><<<grid, block, 0, h->stream>>>(P, A);
+  else stage_cell_kernel<EOS, VISC, MILNE, TWO_D, 2><<<grid, block, 0, h->stream>>>(P, A);
+  h->launches++;
+  return debug_sync(h, stage == 1 ? "stage 1 kernel" : "stage 2 kernel");
+}
+template <int EOS, bool VISC, bool MILNE>
+static cudaError_t launch_stage_d(vh_handle* h, int stage, const StageArgs& A) {
+  return h->two_d ? launch_stage_t<EOS, VISC, MILNE, true>(h, stage, A) : launch_stage_t<EOS, VISC, MILNE, false>(h, stage, A);
+}
+static cudaError_t launch_stage(vh_handle* h, int stage, const StageArgs& A) {
+  const bool visc = h->prm.physics != 0, milne = h->prm.geometry == 0;
+  const int eos = h->prm.eos;
+  if (visc) return eos ? launch_stage_d<1, true, true>(h, stage, A) : launch_stage_d<0, true, true>(h, stage, A);
+  if (milne) return eos ? launch_stage_d<1, false, true>(h, stage, A) : launch_stage_d<0, false, true>(h, stage, A);
+  return eos ? launch_stage_d<1, false, false>(h, stage, A) : launch_stage_d<0, false, false>(h, stage, A);
+}
+static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, double* u) {
+  const DevParams& P = h->P;
+  long long W = h->two_d ? (long long)P.ny + P.nx : (long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny;
+  dim3 grid((unsigned)((W + 255) / 256), 21, P.n_batch);
+  GhostArgs G{q, e, p, u};
+  if (h->two_d) ghost_kernel<true><<<grid, 256, 0, h->stream>>>(P, G);
+  else ghost_kernel<false><<<grid, 256, 0, h->stream>>>(P, G);
+  h->launches++;
+  return debug_sync(h, "ghost kernel");
+}
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
+  std::string why;
+  if (!out) return fail(nullptr, VH_ERR_ARG, "out is NULL");
+  if (check_params(p, why)) return fail(nullptr, VH_ERR_ARG, why);
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev < 1) return fail(nullptr, VH_ERR_CUDA, std::string("no CUDA device: ") + cudaGetErrorString(ce));
+  vh_handle* h = new (std::nothrow) vh_handle;
+  if (!h) return fail(nullptr, VH_ERR_ALLOC, "host allocation failed");
+  h->prm = *p;
+  fill_dev_params(*p, h->P);
+  h->two_d = (p->nz == 1);
+  h->stream = (cudaStream_t)cuda_stream;
+  const long long fs = h->P.fstride;
+  const size_t bytes = (size_t)61 * fs * sizeof(double);
+  ce = cudaMalloc((void**)&h->pool, bytes);
+  if (ce != cudaSuccess) { delete h; return fail(nullptr, VH_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes: " + cudaGetErrorString(ce)); }
+  ce = cudaMalloc((void**)&h->cnt, sizeof(Counters));
+  if (ce != cudaSuccess) { cudaFree(h->pool); delete h; return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc(counters) failed"); }
+  double* w = h->pool;
+  for (int i = 0; i < 3; ++i) { h->q[i] = w; w += 15 * fs; }
+  for (int i = 0; i < 3; ++i) { h->u[i] = w; w += 4 * fs; }
+  for (int i = 0; i < 2; ++i) { h->e[i] = w; w += fs; }
+  for (int i = 0; i < 2; ++i) { h->p[i] = w; w += fs; }
+  ce = cudaMemsetAsync(h->pool, 0, bytes, h->stream);
+  if (ce != cudaSuccess) { cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_CUDA, "cudaMemsetAsync failed"); }
+  *out = h;
+  return VH_OK;
+}
+
+void vh_destroy(vh_handle* h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->stream);
+  cudaFree(h->pool);
+  cudaFree(h->cnt);
+  cudaFree(h->stage_in);
+  cudaFree(h->stage_out);
+  delete h;
+}
+
+const char* vh_last_error(vh_handle* h) { return h ? h->err.c_str() : g_err.c_str(); }
+long long vh_launch_count(vh_handle* h) { return h ? h->launches : 0; }
+
+int vh_set_kernel_variant(vh_handle* h, int variant) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (variant != 0 && variant != 1) return fail(h, VH_ERR_ARG, "unknown kernel variant");
+  h->variant = variant;
+  return VH_OK;
+}
+
+static int ensure_stage(vh_handle* h, double** buf, size_t* have, size_t need) {
+  if (*have >= need) return VH_OK;
+  cudaFree(*buf);
+  *buf = nullptr; *have = 0;
+  if (cudaMalloc((void**)buf, need) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(staging) failed");
+  *have = need;
+  return VH_OK;
+}
+
+static int reset_counters(vh_handle* h) {
+  Counters c;
+  c.n_fail = 0; c.n_nonfinite = 0;
+  double one = 1.0;
+  std::memcpy(&c.min_reg_bits, &one, sizeof(double));
+  CUDA_TRY(h, cudaMemcpyAsync(h->cnt, &c, sizeof(c), cudaMemcpyHostToDevice, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));    // c lives on this stack frame
+  return VH_OK;
+}
+
+int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double* pi10, const double* Pi, int mem_space) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!e || !u4) return fail(h, VH_ERR_ARG, "e and u4 are required");
+  if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
+  const DevParams& P = h->P;
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  const double *de = e, *du = u4, *dpi = pi10, *dPi = Pi;
+  if (mem_space == 0) {
+    int rc = ensure_stage(h, &h->stage_in, &h->stage_in_bytes, (size_t)16 * np * sizeof(double));
+    if (rc) return rc;
+    double* s = h->stage_in;
+    CUDA_TRY(h, cudaMemcpyAsync(s, e, np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(s + np, u4, 4 * np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    if (pi10) CUDA_TRY(h, cudaMemcpyAsync(s + 5 * np, pi10, 10 * np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    if (Pi) CUDA_TRY(h, cudaMemcpyAsync(s + 15 * np, Pi, np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    de = s; du = s + np; dpi = pi10 ? s + 5 * np : nullptr; dPi = Pi ? s + 15 * np : nullptr;
+  }
+  unsigned nb = (unsigned)((np + 255) / 256);
+  if (h->prm.eos) init_kernel<1><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
+  else init_kernel<0><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
+  h->launches++;
+  CUDA_TRY(h, cudaGetLastError());
+  CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
+  h->n_steps = 0;
+  int rc = reset_counters(h);
+  if (rc) return rc;
+  h->initialised = true;
+  return VH_OK;
+}
+
+int vh_set_state(vh_handle* h, const double* q15, const double* e, const double* u4, const double* u4_prev, long long n_steps_done,
+                 int mem_space) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!q15 || !e || !u4 || !u4_prev || n_steps_done < 0) return fail(h, VH_ERR_ARG, "q15, e, u4, u4_prev are required; n_steps_done >= 0");
+  if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
+  const DevParams& P = h->P;
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  const unsigned nb = (unsigned)((np + 255) / 256);
+  struct Item { const double* src; double* dst; int nc; };
+  Item items[4] = {{q15, h->q[0], 15}, {e, h->e[0], 1}, {u4, h->u[0], 4}, {u4_prev, h->u[1], 4}};
+  if (mem_space == 0) {
+    int rc = ensure_stage(h, &h->stage_in, &h->stage_in_bytes, (size_t)16 * np * sizeof(double));
+    if (rc) return rc;
+  }
+  for (const Item& it : items) {
+    const double* src = it.src;
+    if (mem_space == 0) {
+      CUDA_TRY(h, cudaMemcpyAsync(h->stage_in, it.src, (size_t)it.nc * np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+      src = h->stage_in;
+    }
+    pack_kernel<false><<<nb, 256, 0, h->stream>>>(P, it.dst, const_cast<double*>(src), it.nc);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+  }
+  if (h->prm.eos) pressure_kernel<1><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
+  else pressure_kernel<0><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
+  h->launches++;
+  CUDA_TRY(h, cudaGetLastError());
+  CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
+  h->n_steps = n_steps_done;
+  int rc = reset_counters(h);
+  if (rc) return rc;
+  h->initialised = true;
+  return VH_OK;
+}
+
+int vh_set_uprev(vh_handle* h, const double* u4_prev, int mem_space) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_set_uprev before vh_set_initial");
+  if (!u4_prev || (mem_space != 0 && mem_space != 1)) return fail(h, VH_ERR_ARG, "bad argument");
+  const DevParams& P = h->P;
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  const double* src = u4_prev;
+  if (mem_space == 0) {
+    int rc = ensure_stage(h, &h->stage_in, &h->stage_in_bytes, (size_t)16 * np * sizeof(double));
+    if (rc) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(h->stage_in, u4_prev, 4 * np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    src = h->stage_in;
+  }
+  pack_kernel<false><<<(unsigned)((np + 255) / 256), 256, 0, h->stream>>>(P, h->u[1], const_cast<double*>(src), 4);
+  h->launches++;
+  CUDA_TRY(h, cudaGetLastError());
+  if (mem_space == 0) CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return VH_OK;
+}
+
+static int one_step(vh_handle* h, cudaEvent_t* ev) {
+  const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;     // :493
+  const double t1 = t + h->prm.dtau;
+  StageArgs A;
+  // steps 1-4: q* = E[q^n; e,p,u^n,u^{n-1}] at tau^n, then (e*,p*,u*) at tau^n + dtau, regulate, ghosts
+  A.q_in = h->q[0]; A.e_in = h->e[0]; A.p_in = h->p[0]; A.u_in = h->u[0]; A.u_prev = h->u[1]; A.q_n = nullptr;
+  A.q_out = h->q[1]; A.e_out = h->e[1]; A.p_out = h->p[1]; A.u_out = h->u[2]; A.cnt = h->cnt; A.t = t; A.t_post = t1;
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[0], h->stream));
+  CUDA_TRY(h, launch_stage(h, 1, A));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[1], h->stream));
+  CUDA_TRY(h, launch_ghost(h, h->q[1], h->e[1], h->p[1], h->u[2]));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[2], h->stream));
+  // steps 5-8: q** = E[q*; e*,p*,u*,u^n] at tau^n + dtau; q^{n+1} = (q^n + q**)/2; invert, regulate, ghosts.
+  // u^{n+1} overwrites the buffer of u^{n-1}, e^{n+1}/p^{n+1} the buffers of e^n/p^n (neither is read by stage 2).
+  A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
+  A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1]; A.t = t1; A.t_post = t1;
+  CUDA_TRY(h, launch_stage(h, 2, A));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[3], h->stream));
+  CUDA_TRY(h, launch_ghost(h, h->q[2], h->e[0], h->p[0], h->u[1]));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[4], h->stream));
+  // steps 7, 9: rotate.  u: (u^n, u^{n-1}, u*) <- (u^{n+1}, u^n, scratch); q: q^n <-> q^{n+1}
+  double* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;
+  double* qn = h->q[2]; h->q[2] = h->q[0]; h->q[0] = qn;
+  h->n_steps++;
+  return VH_OK;
+}
+
+int vh_step(vh_handle* h, int n_steps) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_step before vh_set_initial");
+  if (n_steps < 0) return fail(h, VH_ERR_ARG, "n_steps must be >= 0");
+  for (int it = 0; it < n_steps; ++it) {
+    int rc = one_step(h, nullptr);
+    if (rc) return rc;
+  }
+  return VH_OK;
+}
+
+int vh_step_profile(vh_handle* h, int n_steps, double* ms4) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_step_profile before vh_set_initial");
+  if (n_steps < 1 || !ms4) return fail(h, VH_ERR_ARG, "n_steps >= 1 and ms4 != NULL required");
+  cudaEvent_t ev[5];
+  for (int i = 0; i < 5; ++i) CUDA_TRY(h, cudaEventCreate(&ev[i]));
+  double acc[4] = {0, 0, 0, 0};
+  for (int it = 0; it < n_steps; ++it) {
+    int rc = one_step(h, ev);
+    if (rc) return rc;
+    CUDA_TRY(h, cudaEventSynchronize(ev[4]));
+    for (int i = 0; i < 4; ++i) { float ms = 0; CUDA_TRY(h, cudaEventElapsedTime(&ms, ev[i], ev[i + 1])); acc[i] += ms; }
+  }
+  for (int i = 0; i < 5; ++i) cudaEventDestroy(ev[i]);
+  for (int i = 0; i < 4; ++i) ms4[i] = acc[i] / n_steps;
+  return VH_OK;
+}
+
+int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, double* u4_prev, int mem_space) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_fields before vh_set_initial");
+  if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
+  const DevParams& P = h->P;
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  const unsigned nb = (unsigned)((np + 255) / 256);
+  struct Item { double* dst; double* src; int nc; };
+  Item items[5] = {{q15, h->q[0], 15}, {e, h->e[0], 1}, {p, h->p[0], 1}, {u4, h->u[0], 4}, {u4_prev, h->u[1], 4}};
+  if (mem_space == 0) {
+    int rc = ensure_stage(h, &h->stage_out, &h->stage_out_bytes, (size_t)15 * np * sizeof(double));
+    if (rc) return rc;
+  }
+  for (const Item& it : items) {
+    if (!it.dst) continue;
+    double* target = (mem_space == 1) ? it.dst : h->stage_out;
+    pack_kernel<true><<<nb, 256, 0, h->stream>>>(P, it.src, target, it.nc);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    if (mem_space == 0) CUDA_TRY(h, cudaMemcpyAsync(it.dst, h->stage_out, (size_t)it.nc * np * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  }
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  return VH_OK;
+}
+
+int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long* n_inversion_failures, long long* n_nonfinite,
+                  double* min_reg_factor) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  Counters c;
+  CUDA_TRY(h, cudaMemcpyAsync(&c, h->cnt, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+  if (tau) *tau = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
+  if (n_steps_done) *n_steps_done = h->n_steps;
+  if (n_inversion_failures) *n_inversion_failures = (long long)c.n_fail;
+  if (n_nonfinite) *n_nonfinite = (long long)c.n_nonfinite;
+  if (min_reg_factor) std::memcpy(min_reg_factor, &c.min_reg_bits, sizeof(double));
+  return VH_OK;
+}
+
+int vh_measure_peaks(void* cuda_stream, long long n_bytes, int repeats, double* copy_gbs, double* fp64_gflops) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n_bytes < (1 << 20) || repeats < 1) return fail(nullptr, VH_ERR_ARG, "n_bytes >= 1 MiB and repeats >= 1 required");
+  int dev = 0, nsm = 0;
+  CUDA_TRY(nullptr, cudaGetDevice(&dev));
+  CUDA_TRY(nullptr, cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(nullptr, cudaEventCreate(&e0));
+  CUDA_TRY(nullptr, cudaEventCreate(&e1));
+  if (copy_gbs) {
+    double *a = nullptr, *b = nullptr;
+    long long n2 = n_bytes / 16;
+    if (cudaMalloc((void**)&a, n2 * 16) != cudaSuccess || cudaMalloc((void**)&b, n2 * 16) != cudaSuccess) {
+      cudaFree(a); cudaFree(b);
+      return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc(copy buffers) failed");
+    }
+    cudaMemsetAsync(a, 0, n2 * 16, st);
+    double best = 0;
+    for (int r = 0; r < repeats + 1; ++r) {
+      cudaEventRecord(e0, st);
+      copy_kernel<<<nsm * 16, 256, 0, st>>>((const double2*)a, (double2*)b, n2);
+      cudaEventRecord(e1, st);
+      cudaEventSynchronize(e1);
+      float ms = 0;
+      cudaEventElapsedTime(&ms, e0, e1);
+      double gbs = 2.0 * n2 * 16 / (ms * 1e-3) / 1e9;
+      if (r > 0 && gbs > best) best = gbs;
+    }
+    cudaFree(a); cudaFree(b);
+    *copy_gbs = best;
+  }
+  if (fp64_gflops) {
+    double* o = nullptr;
+    CUDA_TRY(nullptr, cudaMalloc((void**)&o, 8));
+    const int iters = 4096, blocks = nsm * 8;
+    double best = 0;
+    for (int r = 0; r < repeats + 1; ++r) {
+      cudaEventRecord(e0, st);
+      fma_kernel<<<blocks, 256, 0, st>>>(o, iters, 0.999999, 1e-6);
+      cudaEventRecord(e1, st);
+      cudaEventSynchronize(e1);
+      float ms = 0;
+      cudaEventElapsedTime(&ms, e0, e1);
+      double gf = 2.0 * 64.0 * iters * 256.0 * blocks / (ms * 1e-3) / 1e9;
+      if (r > 0 && gf > best) best = gf;
+    }
+    cudaFree(o);
+    *fp64_gflops = best;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  CUDA_TRY(nullptr, cudaGetLastError());
+  return VH_OK;
+}
+
+}  // extern "C"

@@ -63,17 +63,18 @@ def centred_axis(n, d):
     return (np.arange(n) - 0.5 * (n - 1)) * d
 
 
-def hotspots_energy(nx, ny, nz, dx, dy, dz, n_hot, width, seed, three_d, pedestal_gev=0.05):
-    """e(x,y,eta) [fm^-4] = pedestal + sum_h A_h exp(-|x-x_h|^2/(2 w^2)); draw order per hotspot: A, r, phi, (eta)."""
+def hotspots_energy(nx, ny, nz, dx, dy, dz, n_hot, width, seed, three_d, pedestal_gev=0.05, radius=5.0, eta_half=2.0):
+    """e(x,y,eta) [fm^-4] = pedestal + sum_h A_h exp(-|x-x_h|^2/(2 w^2)); draw order per hotspot: A, r, phi, (eta).
+    Centres uniform in a disc of `radius` fm (5 fm in BASELINE.json) and in |eta| < eta_half (2); small test grids shrink both."""
     rng = SplitMix64(seed)
     A = np.empty(n_hot); xh = np.empty(n_hot); yh = np.empty(n_hot); zh = np.zeros(n_hot)
     for h in range(n_hot):
         A[h] = 5.0 + 25.0 * rng.uniform()
-        r = 5.0 * math.sqrt(rng.uniform())
+        r = radius * math.sqrt(rng.uniform())
         ph = 2.0 * math.pi * rng.uniform()
         xh[h] = r * math.cos(ph); yh[h] = r * math.sin(ph)
         if three_d:
-            zh[h] = -2.0 + 4.0 * rng.uniform()
+            zh[h] = eta_half * (-1.0 + 2.0 * rng.uniform())
     x = centred_axis(nx, dx); y = centred_axis(ny, dy); z = centred_axis(nz, dz)
     gx = np.exp(-((x[None, :] - xh[:, None]) ** 2) / (2 * width * width))          # [h, nx]
     gy = np.exp(-((y[None, :] - yh[:, None]) ** 2) / (2 * width * width))          # [h, ny]
@@ -193,20 +194,21 @@ def config_gubser(n=201, d=0.05, eta_over_s=0.2, n_steps=400, theta=1.8):
 
 
 # ------------------------------------------------------------------ configs 3-5: seeded hotspots
-def config_3d(nx=128, ny=128, nz=128, dx=0.1, dy=0.1, dz=0.1, n_hot=40, width=0.5, seed=BASE_SEED, n_steps=100, **over):
+def config_3d(nx=128, ny=128, nz=128, dx=0.1, dy=0.1, dz=0.1, n_hot=40, width=0.5, seed=BASE_SEED, n_steps=100, radius=5.0, eta_half=2.0,
+              **over):
     """BASELINE.json configs[2] (defaults) and configs[4] (512,512,128, dx=dy=0.05, n_hot=200, n_steps=50)."""
     prm = base_params(nx=nx, ny=ny, nz=nz, dx=dx, dy=dy, dz=dz, tau0=0.5, dtau=0.025, **over)
-    e = hotspots_energy(nx, ny, nz, dx, dy, dz, n_hot, width, seed, three_d=True)
+    e = hotspots_energy(nx, ny, nz, dx, dy, dz, n_hot, width, seed, three_d=True, radius=radius, eta_half=eta_half)
     shp = (1, nz, ny, nx)
     return prm, dict(e=e.reshape(shp), u=rest_velocity(shp), pi=None, Pi=None), n_steps
 
 
-def config_batched2d(n_batch=256, n=201, d=0.1, n_hot=20, width=0.4, seed=BASE_SEED, n_steps=200, **over):
+def config_batched2d(n_batch=256, n=201, d=0.1, n_hot=20, width=0.4, seed=BASE_SEED, n_steps=200, radius=5.0, **over):
     """BASELINE.json configs[3]: n_batch independent 2+1d events, event b seeded with seed+b."""
     prm = base_params(nx=n, ny=n, nz=1, n_batch=n_batch, dx=d, dy=d, dz=1.0, tau0=0.5, dtau=0.025, **over)
     e = np.empty((n_batch, 1, n, n))
     for b in range(n_batch):
-        e[b] = hotspots_energy(n, n, 1, d, d, 1.0, n_hot, width, seed + b, three_d=False)
+        e[b] = hotspots_energy(n, n, 1, d, d, 1.0, n_hot, width, seed + b, three_d=False, radius=radius)
     shp = (n_batch, 1, n, n)
     return prm, dict(e=e, u=rest_velocity(shp), pi=None, Pi=None), n_steps
 

@@ -1,0 +1,223 @@
+"""Thin Python binding of the C ABI in include/vh.h (argument marshalling only; every step runs in the CUDA kernels).
+
+torch is used for device memory (the arrays handed to / returned from the library) and for the CUDA stream.
+There is no CPU fallback: if libvh.so is missing or no CUDA device is present, construction raises."""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SO = os.path.join(HERE, "libvh.so")
+
+VH_OK = 0
+
+
+class vh_params(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("n_batch", C.c_int),
+        ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+        ("tau0", C.c_double), ("dtau", C.c_double),
+        ("geometry", C.c_int), ("physics", C.c_int), ("eos", C.c_int),
+        ("eos_a", C.c_double), ("eos_alpha", C.c_double), ("eos_e0", C.c_double),
+        ("eta_over_s", C.c_double),
+        ("zeta_model", C.c_int), ("zeta_amp", C.c_double), ("zeta_T0", C.c_double), ("zeta_width", C.c_double),
+        ("c_tau_pi", C.c_double), ("c_tau_Pi", C.c_double),
+        ("delta_pipi", C.c_double), ("tau_pipi", C.c_double), ("lambda_piPi", C.c_double),
+        ("delta_PiPi", C.c_double), ("lambda_Pipi_coef", C.c_double),
+        ("minmod_theta", C.c_double), ("xi0", C.c_double), ("rho_max", C.c_double),
+        ("newton_max_iter", C.c_int), ("newton_rtol", C.c_double),
+        ("tau_relax_floor_over_dtau", C.c_double),
+    ]
+
+
+# every symbol include/vh.h declares
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_launch_count",
+           "vh_set_kernel_variant", "vh_measure_peaks", "vh_last_error", "vh_destroy"]
+
+_lib = None
+
+
+def load_library():
+    """dlopen libvh.so and declare the prototypes.  Works without a GPU (no CUDA call is made)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(SO):
+        raise RuntimeError("CUDA extension %s is missing: run `python -m paper_1608_06577_b200.build` (there is no CPU fallback)" % SO)
+    L = C.CDLL(SO)
+    vp = C.c_void_p
+    for name in EXPORTS:
+        getattr(L, name).restype = C.c_int
+    L.vh_create.argtypes = [C.POINTER(vh_params), vp, C.POINTER(vp)]
+    L.vh_set_initial.argtypes = [vp, vp, vp, vp, vp, C.c_int]
+    L.vh_set_uprev.argtypes = [vp, vp, C.c_int]
+    L.vh_set_state.argtypes = [vp, vp, vp, vp, vp, C.c_longlong, C.c_int]
+    L.vh_step.argtypes = [vp, C.c_int]
+    L.vh_step_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
+    L.vh_get_fields.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
+    L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
+    L.vh_launch_count.argtypes = [vp]
+    L.vh_launch_count.restype = C.c_longlong
+    L.vh_set_kernel_variant.argtypes = [vp, C.c_int]
+    L.vh_measure_peaks.argtypes = [vp, C.c_longlong, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.vh_last_error.argtypes = [vp]
+    L.vh_last_error.restype = C.c_char_p
+    L.vh_destroy.argtypes = [vp]
+    L.vh_destroy.restype = None
+    _lib = L
+    return L
+
+
+def make_params(d: dict) -> vh_params:
+    p = vh_params()
+    for name, _ in vh_params._fields_:
+        if name not in d:
+            raise KeyError("missing parameter %r" % name)
+        setattr(p, name, d[name])
+    return p
+
+
+class VHError(RuntimeError):
+    pass
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    return C.c_void_p(t.data_ptr())
+
+
+class Solver:
+    """vh_create / vh_set_initial / vh_step / vh_get_fields on one GPU.
+
+    Arrays are torch tensors (float64) of shape [..., n_batch, nz, ny, nx]: CUDA tensors are passed as device pointers
+    (mem_space 1), CPU tensors as host pointers (mem_space 0; the library does the copies on its stream)."""
+
+    def __init__(self, params: dict, device="cuda:0", stream=None):
+        import torch
+
+        self.torch = torch
+        self.L = load_library()
+        if not torch.cuda.is_available():
+            raise VHError("no CUDA device available (there is no CPU fallback)")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.d = dict(params)
+        self.P = make_params(params)
+        self.h = C.c_void_p()
+        rc = self.L.vh_create(C.byref(self.P), C.c_void_p(self.stream.cuda_stream), C.byref(self.h))
+        if rc != VH_OK:
+            msg = self.L.vh_last_error(None)
+            self.h = None
+            raise VHError("vh_create failed (%d): %s" % (rc, msg.decode() if msg else "?"))
+        self.shape = (self.P.n_batch, self.P.nz, self.P.ny, self.P.nx)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.vh_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc != VH_OK:
+            msg = self.L.vh_last_error(self.h)
+            raise VHError("%s failed (%d): %s" % (what, rc, msg.decode() if msg else "?"))
+
+    def _prep(self, a, lead):
+        torch = self.torch
+        if a is None:
+            return None
+        if not isinstance(a, torch.Tensor):
+            a = torch.as_tensor(a, dtype=torch.float64)
+        a = a.to(torch.float64).contiguous()
+        want = 1
+        for s in lead + self.shape:
+            want *= s
+        if a.numel() != want:
+            raise ValueError("array has %d elements, expected %d" % (a.numel(), want))
+        return a
+
+    def _space(self, tensors):
+        spaces = {t.is_cuda for t in tensors if t is not None}
+        if len(spaces) != 1:
+            raise ValueError("all arrays of one call must live in the same memory space")
+        return 1 if spaces.pop() else 0
+
+    def set_initial(self, e, u4, pi10=None, Pi=None):
+        e = self._prep(e, ()); u4 = self._prep(u4, (4,)); pi10 = self._prep(pi10, (10,)); Pi = self._prep(Pi, ())
+        ms = self._space([e, u4, pi10, Pi])
+        self._check(self.L.vh_set_initial(self.h, _ptr(e), _ptr(u4), _ptr(pi10), _ptr(Pi), ms), "vh_set_initial")
+        if ms == 1:
+            self.stream.synchronize()      # the caller may free its tensors on return
+
+    def set_state(self, q15, e, u4, u4_prev, n_steps_done=0):
+        q15 = self._prep(q15, (15,)); e = self._prep(e, ()); u4 = self._prep(u4, (4,)); u4_prev = self._prep(u4_prev, (4,))
+        ms = self._space([q15, e, u4, u4_prev])
+        self._check(self.L.vh_set_state(self.h, _ptr(q15), _ptr(e), _ptr(u4), _ptr(u4_prev), int(n_steps_done), ms), "vh_set_state")
+        self.stream.synchronize()
+
+    def set_uprev(self, u4_prev):
+        a = self._prep(u4_prev, (4,))
+        ms = self._space([a])
+        self._check(self.L.vh_set_uprev(self.h, _ptr(a), ms), "vh_set_uprev")
+        if ms == 1:
+            self.stream.synchronize()
+
+    def step(self, n=1):
+        self._check(self.L.vh_step(self.h, int(n)), "vh_step")
+
+    def step_profile(self, n=1):
+        """n steps with CUDA events around each launch; mean ms of (stage 1, ghost 1, stage 2, ghost 2)."""
+        ms = (C.c_double * 4)()
+        self._check(self.L.vh_step_profile(self.h, int(n), ms), "vh_step_profile")
+        return dict(zip(("stage1", "ghost1", "stage2", "ghost2"), list(ms)))
+
+    def get_fields(self, device=None, with_uprev=False, out=None):
+        """Returns dict(q [15,...], e, p, u [4,...]) as tensors on `device` ('cpu' -> host buffers, mem_space 0)."""
+        torch = self.torch
+        dev = self.device if device is None else torch.device(device)
+        if out is None:
+            kw = dict(dtype=torch.float64, device=dev)
+            if dev.type == "cpu":
+                kw["pin_memory"] = True
+            out = dict(q=torch.empty((15,) + self.shape, **kw), e=torch.empty(self.shape, **kw), p=torch.empty(self.shape, **kw),
+                       u=torch.empty((4,) + self.shape, **kw))
+            if with_uprev:
+                out["up"] = torch.empty((4,) + self.shape, **kw)
+        ms = self._space([v for v in out.values()])
+        self._check(self.L.vh_get_fields(self.h, _ptr(out.get("q")), _ptr(out.get("e")), _ptr(out.get("p")), _ptr(out.get("u")),
+                                         _ptr(out.get("up")), ms), "vh_get_fields")
+        return out
+
+    def status(self):
+        tau, mr = C.c_double(), C.c_double()
+        a, b, c = C.c_longlong(), C.c_longlong(), C.c_longlong()
+        self._check(self.L.vh_get_status(self.h, C.byref(tau), C.byref(a), C.byref(b), C.byref(c), C.byref(mr)), "vh_get_status")
+        return {"tau": tau.value, "n_steps": a.value, "n_inversion_failures": b.value, "n_nonfinite": c.value, "min_reg_factor": mr.value}
+
+    def launch_count(self):
+        return int(self.L.vh_launch_count(self.h))
+
+    def set_kernel_variant(self, v):
+        self._check(self.L.vh_set_kernel_variant(self.h, int(v)), "vh_set_kernel_variant")
+
+
+def measure_peaks(n_bytes=1 << 30, repeats=10, stream=None):
+    """(copy GB/s, FP64 FMA GFLOP/s) measured by the library's own microbenchmarks on the current device."""
+    import torch
+
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise VHError("no CUDA device available")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    a, b = C.c_double(), C.c_double()
+    rc = L.vh_measure_peaks(C.c_void_p(st.cuda_stream), int(n_bytes), int(repeats), C.byref(a), C.byref(b))
+    if rc != VH_OK:
+        msg = L.vh_last_error(None)
+        raise VHError("vh_measure_peaks failed (%d): %s" % (rc, msg.decode() if msg else "?"))
+    return a.value, b.value

@@ -1,0 +1,100 @@
+"""CPU-side checks of the boundary: libvh.so loads without a GPU and exports every symbol include/vh.h declares;
+the product path fails loudly (no CPU fallback) when no CUDA device is present; package hygiene."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1608_06577_b200 import build, vh
+
+    build.build()
+    return vh.load_library()
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "vh.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(vh_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_1608_06577_b200 import vh
+
+    names = declared_functions()
+    assert len(names) >= 11
+    for n in names:
+        assert hasattr(lib, n), "libvh.so does not export %s" % n
+    assert sorted(vh.EXPORTS) == names, "the Python binding and include/vh.h disagree on the entry points"
+
+
+def test_params_struct_layout_matches_header():
+    from paper_1608_06577_b200 import vh
+
+    src = open(os.path.join(ROOT, "include", "vh.h")).read()
+    body = src[src.index("typedef struct {") + len("typedef struct {") : src.index("} vh_params;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split(";"):
+        m = re.match(r"\s*(int|double)\s+(.*)", decl.strip(), flags=re.S)
+        if m:
+            for name in m.group(2).split(","):
+                fields.append((name.strip(), m.group(1)))
+    got = [(n, "int" if t is C.c_int else "double") for n, t in vh.vh_params._fields_]
+    assert got == fields
+
+
+def test_no_gpu_means_loud_failure(lib):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("this box has a GPU")
+    from paper_1608_06577_b200 import inputs, vh
+
+    with pytest.raises(vh.VHError):
+        vh.Solver(inputs.base_params(nx=4, ny=4, nz=4))
+    p = vh.make_params(inputs.base_params(nx=4, ny=4, nz=4))
+    h = C.c_void_p()
+    assert lib.vh_create(C.byref(p), None, C.byref(h)) == -3      # VH_ERR_CUDA
+    assert h.value is None
+    assert lib.vh_create(None, None, C.byref(h)) == -1            # VH_ERR_ARG before any CUDA call
+    assert b"NULL" in lib.vh_last_error(None)
+
+
+def test_product_path_does_not_touch_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1608_06577_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "vh_oracle" not in txt and "oracle/" not in txt.replace("shares nothing with oracle/", ""), os.path.join(dirpath, f)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".hpp")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "libvh.so" not in txt and "import vh\n" not in txt and "vh_device" not in txt
+
+
+def test_inputs_are_seeded_and_reproducible():
+    import numpy as np
+
+    from paper_1608_06577_b200 import inputs
+
+    r = inputs.SplitMix64(inputs.BASE_SEED)
+    first = [r.next_u64() for _ in range(3)]
+    r2 = inputs.SplitMix64(inputs.BASE_SEED)
+    assert first == [r2.next_u64() for _ in range(3)]
+    # SplitMix64 reference value for seed 0 (first output of the published algorithm)
+    assert inputs.SplitMix64(0).next_u64() == 0xE220A8397B1DCDAF
+    _, a, _ = inputs.config_3d(16, 16, 8, n_hot=4)
+    _, b, _ = inputs.config_3d(16, 16, 8, n_hot=4)
+    np.testing.assert_array_equal(a["e"], b["e"])
+    assert a["e"].min() >= 0.05 / inputs.HBARC * (1 - 1e-12)       # pedestal (reading R14)
+    _, c, _ = inputs.config_batched2d(n_batch=2, n=12, n_hot=3)
+    assert not np.array_equal(c["e"][0], c["e"][1])                 # event b uses seed + b

@@ -1,0 +1,276 @@
+"""GPU <-> oracle parity through the C ABI (include/vh.h), element by element on the same seeded inputs.
+
+Bar (BASELINE.json north_star; norm of DESIGN.md reading R18): per field f,
+    max_cells |gpu - oracle| / max_cells |oracle|  <= 1e-9 after 10 steps, FP64;
+fields that are identically zero in the oracle must stay below 1e-9 * max|T^{tau tau}| absolutely.
+Inversion-failure counters must agree exactly."""
+import numpy as np
+import pytest
+
+from paper_1608_06577_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def vh():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_1608_06577_b200 import vh as _vh
+
+    _vh.load_library()
+    return _vh
+
+
+def run_both(vh, vo, prm, init, n_steps, uprev=None, host_io=False):
+    import torch
+
+    o = vo.Oracle(prm)
+    o.set_initial(init["e"], init["u"], init.get("pi"), init.get("Pi"))
+    if uprev is not None:
+        o.set_uprev(uprev)
+    o.step(n_steps)
+    fo = o.get_fields(with_uprev=True)
+    so = o.status()
+
+    s = vh.Solver(prm)
+    dev = "cpu" if host_io else "cuda:0"
+    t = lambda a: None if a is None else torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
+    s.set_initial(t(init["e"]), t(init["u"]), t(init.get("pi")), t(init.get("Pi")))
+    if uprev is not None:
+        s.set_uprev(t(uprev))
+    s.step(n_steps)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields(device=dev, with_uprev=True).items()}
+    sg = s.status()
+    s.close()
+    return fo, so, fg, sg
+
+
+NOISE = 1e-6      # fields below NOISE x (natural scale) are rounding noise: compared absolutely against that floor (R18)
+
+
+def field_errors(fo, fg):
+    """max|gpu - oracle| / max(max|oracle|, NOISE * S): S = max|T^{tau tau}| for the conserved fields, e, p; 1 for u^mu."""
+    scale_T = np.max(np.abs(fo["q"][0]))
+    errs = {}
+    def one(name, a, b, S):
+        errs[name] = np.max(np.abs(a - b)) / max(np.max(np.abs(a)), NOISE * S)
+    for n in range(15):
+        one("q%d" % n, fo["q"][n], fg["q"][n], scale_T)
+    one("e", fo["e"], fg["e"], scale_T); one("p", fo["p"], fg["p"], scale_T)
+    for m in range(4):
+        one("u%d" % m, fo["u"][m], fg["u"][m], 1.0)
+        one("up%d" % m, fo["up"][m], fg["up"][m], 1.0)
+    return errs
+
+
+def assert_parity(fo, so, fg, sg, tol=TOL):
+    errs = field_errors(fo, fg)
+    bad = {k: v for k, v in errs.items() if not (v <= tol)}
+    assert not bad, "fields beyond %g: %s" % (tol, bad)
+    assert sg["tau"] == pytest.approx(so["tau"], rel=1e-15)
+    assert sg["n_steps"] == so["n_steps"]
+    assert sg["n_inversion_failures"] == so["n_inversion_failures"]
+    assert sg["n_nonfinite"] == so["n_nonfinite"]
+    assert sg["min_reg_factor"] == pytest.approx(so["min_reg_factor"], rel=1e-9)
+    return errs
+
+
+def test_config3_physics_hotspots_3d_ragged_tiles(vh, vo):
+    # BASELINE configs[2] physics on a grid spanning 2 x 3 x 12 thread tiles with a ragged tail in x (40 = 32 + 8)
+    prm, init, _ = inputs.config_3d(40, 24, 12, n_hot=6, width=0.5, seed=inputs.BASE_SEED, radius=1.5, eta_half=0.5)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, 10)
+    assert so["n_inversion_failures"] == 0
+    assert np.max(np.abs(fo["u"][1:])) > 0.05 and np.max(np.abs(fo["q"][4:14])) > 1e-3      # real dynamics, not noise
+    assert_parity(fo, so, fg, sg)
+
+
+def test_generic_state_all_terms_3d(vh, vo):
+    # flow in all directions (vorticity, u^eta != 0), all ten pi components and Pi non-zero, u^{n-1} != u^n
+    prm = inputs.base_params(nx=36, ny=20, nz=10, dx=0.12, dy=0.1, dz=0.15, tau0=0.8, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=21)
+    up = st["u"] * 1.0
+    up[1:] *= 0.97
+    up[0] = np.sqrt(1 + up[1] ** 2 + up[2] ** 2 + prm["tau0"] ** 2 * up[3] ** 2)
+    fo, so, fg, sg = run_both(vh, vo, prm, st, 10, uprev=up)
+    assert np.max(np.abs(fo["q"][12])) > 0 and np.max(np.abs(fo["q"][14])) > 0 and np.max(np.abs(fo["u"][3])) > 0
+    assert_parity(fo, so, fg, sg)
+
+
+@pytest.mark.parametrize("physics", [1, 2])
+def test_shear_only_and_bulk_only(vh, vo, physics):
+    prm = inputs.base_params(nx=20, ny=12, nz=6, tau0=0.6, dtau=0.02, physics=physics)
+    st = inputs.smooth_random_state(prm, seed=5 + physics)
+    fo, so, fg, sg = run_both(vh, vo, prm, st, 6)
+    if physics == 1:
+        assert np.max(np.abs(fg["q"][14])) == 0.0
+    else:
+        assert np.max(np.abs(fg["q"][4:14])) == 0.0
+    assert_parity(fo, so, fg, sg)
+
+
+def test_batched_2plus1d_events(vh, vo):
+    # BASELINE configs[3] physics: independent 2+1d events in one launch; ragged in x and y
+    prm, init, _ = inputs.config_batched2d(n_batch=3, n=45, n_hot=5, seed=inputs.BASE_SEED, radius=1.8)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, 10)
+    assert so["n_inversion_failures"] == 0
+    assert_parity(fo, so, fg, sg)
+    # events are independent: event 1 alone gives the same bits as event 1 inside the batch
+    import torch
+    prm1 = dict(prm, n_batch=1)
+    s = vh.Solver(prm1)
+    s.set_initial(torch.as_tensor(init["e"][1:2], device="cuda:0"), torch.as_tensor(init["u"][:, 1:2].copy(), device="cuda:0"))
+    s.step(10)
+    f1 = s.get_fields()
+    np.testing.assert_array_equal(f1["q"].cpu().numpy()[:, 0], fg["q"][:, 1])
+    s.close()
+
+
+def test_2plus1d_generic_state(vh, vo):
+    prm = inputs.base_params(nx=33, ny=17, nz=1, n_batch=2, dz=1.0, tau0=0.7, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=9)
+    st["pi"][[3, 6, 8]] = 0.0      # boost-invariant: components with one eta index vanish and stay zero
+    fo, so, fg, sg = run_both(vh, vo, prm, st, 10)
+    assert_parity(fo, so, fg, sg)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_config1_shock_tube(vh, vo, axis):
+    # BASELINE configs[0]: full run (100 steps), ideal Cartesian; includes the step-0 inversion failures of the
+    # cell next to the membrane, whose handling (R6) must be identical
+    prm, init, n_steps, _ = inputs.config_shocktube(n=200, axis=axis)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, n_steps)
+    assert_parity(fo, so, fg, sg, tol=1e-6)      # full-run bar of north_star
+    prm, init, _, _ = inputs.config_shocktube(n=200, axis=axis)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, 10)
+    assert_parity(fo, so, fg, sg)
+
+
+def test_config2_gubser_viscous(vh, vo):
+    # BASELINE configs[1] at reduced size (81 x 81, 10 steps): conformal EOS, shear only, theta = 1.8, tau_pipi = 0
+    prm, init, _, _ = inputs.config_gubser(n=81, d=0.05, eta_over_s=0.2)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, 10)
+    assert so["n_inversion_failures"] == 0
+    assert_parity(fo, so, fg, sg)
+
+
+def test_ideal_milne_3d_and_conformal(vh, vo):
+    for eos in (0, 1):
+        prm, init, _ = inputs.config_3d(18, 14, 9, n_hot=3, width=0.4, seed=3, physics=0, eos=eos, radius=0.6, eta_half=0.3)
+        fo, so, fg, sg = run_both(vh, vo, prm, init, 8)
+        assert np.max(np.abs(fg["q"][4:])) == 0.0 and np.max(np.abs(fo["u"][1:])) > 0.05
+        assert_parity(fo, so, fg, sg)
+
+
+def test_near_uniform_ideal_flow_at_rounding_noise_level(vh, vo):
+    # regression: a box far from every hotspot (pedestal + Gaussian tails, velocities ~1e-12) once faulted in the ideal kernels
+    for geometry in (0, 1):
+        prm, init, _ = inputs.config_3d(18, 14, 9, n_hot=3, width=0.4, seed=3, physics=0, eos=0, geometry=geometry)
+        fo, so, fg, sg = run_both(vh, vo, prm, init, 8)
+        assert_parity(fo, so, fg, sg)
+
+
+@pytest.mark.parametrize("dims", [(1, 1, 1), (3, 2, 1), (2, 1, 3), (1, 5, 2), (64, 8, 2), (32, 1, 1)])
+def test_degenerate_and_tiny_grids(vh, vo, dims):
+    prm = inputs.base_params(nx=dims[0], ny=dims[1], nz=dims[2], tau0=0.6)
+    st = inputs.smooth_random_state(prm, seed=sum(dims))
+    if dims[2] == 1:
+        st["pi"][[3, 6, 8]] = 0.0
+    fo, so, fg, sg = run_both(vh, vo, prm, st, 5)
+    assert_parity(fo, so, fg, sg)
+
+
+def test_host_buffers_and_restart(vh, vo):
+    # mem_space 0 (host pointers) gives the same bits as mem_space 1; get_fields + set_initial + set_uprev restarts bit-exactly
+    import torch
+    prm, init, _ = inputs.config_3d(20, 12, 6, n_hot=3, width=0.4, seed=2, radius=0.8, eta_half=0.2)
+    fo, so, fh, sh = run_both(vh, vo, prm, init, 4, host_io=True)
+    _, _, fd, sd = run_both(vh, vo, prm, init, 4, host_io=False)
+    for k in fh:
+        np.testing.assert_array_equal(fh[k], fd[k])
+    assert_parity(fo, so, fh, sh)
+    # bit-exact restart from the exported state (vh_set_state), in both memory spaces
+    s2 = vh.Solver(prm)
+    s2.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+    s2.step(7)
+    f7 = {k: v.cpu().numpy() for k, v in s2.get_fields().items()}
+    s2.close()
+    for dev in ("cuda:0", "cpu"):
+        s = vh.Solver(prm)
+        t = lambda a: torch.as_tensor(np.ascontiguousarray(a), device=dev)
+        s.set_state(t(fd["q"]), t(fd["e"]), t(fd["u"]), t(fd["up"]), n_steps_done=4)
+        s.step(3)
+        fr = {k: v.cpu().numpy() for k, v in s.get_fields().items()}
+        assert s.status()["tau"] == pytest.approx(prm["tau0"] + 7 * prm["dtau"], rel=1e-15)
+        s.close()
+        for k in ("q", "e", "p", "u"):
+            np.testing.assert_array_equal(fr[k], f7[k])
+
+
+def test_error_codes_and_status(vh):
+    import ctypes as C
+    import torch
+    L = vh.load_library()
+    bad = inputs.base_params(nx=0, ny=4, nz=4)
+    with pytest.raises(vh.VHError):
+        vh.Solver(bad)
+    with pytest.raises(vh.VHError):
+        vh.Solver(inputs.base_params(nx=4, ny=4, nz=4, geometry=1, physics=3))
+    with pytest.raises(vh.VHError):
+        vh.Solver(inputs.base_params(nx=4, ny=4, nz=4, minmod_theta=2.5))
+    s = vh.Solver(inputs.base_params(nx=4, ny=4, nz=4))
+    assert L.vh_step(s.h, 1) == -4                       # VH_ERR_STATE: before vh_set_initial
+    assert b"vh_set_initial" in L.vh_last_error(s.h)
+    assert L.vh_set_initial(s.h, None, None, None, None, 1) == -1
+    assert L.vh_set_kernel_variant(s.h, 99) == -1
+    shp = (1, 4, 4, 4)
+    s.set_initial(torch.full(shp, 10.0, dtype=torch.float64, device="cuda:0"), torch.as_tensor(inputs.rest_velocity(shp), device="cuda:0"))
+    assert L.vh_step(s.h, -1) == -1
+    n0 = s.launch_count()
+    s.step(2)
+    assert s.launch_count() - n0 == 8                    # 2 stage + 2 ghost kernels per step
+    st = s.status()
+    assert st["n_steps"] == 2 and st["tau"] == pytest.approx(0.5 + 2 * 0.025) and st["n_inversion_failures"] == 0
+    s.close()
+
+
+def test_full_size_config3_sampled_subboxes(vh, vo):
+    """BASELINE configs[2] at its full size (128^3, the launch configuration bench.py times): 2 steps on the GPU; the oracle
+    recomputes sampled sub-boxes.  One RK2 step has a domain of dependence of +-4 cells (two stages of the +-2 stencil), so
+    the inner cells of a sub-box cut out of the same initial data, 8 cells away from every cut face, are exact after 2 steps."""
+    import torch
+    prm, init, _ = inputs.config_3d()
+    s = vh.Solver(prm)
+    s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+    s.step(2)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields().items()}
+    sg = s.status()
+    s.close()
+    assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
+    assert np.all(np.isfinite(fg["q"])) and np.all(fg["e"] > 0)
+    B, H = 24, 8
+    worst = 0.0
+    for (x0, y0, z0) in [(0, 0, 0), (104, 104, 104), (52, 52, 52), (60, 40, 70), (104, 0, 50), (30, 104, 0), (96, 20, 96)]:
+        sub = dict(prm, nx=B, ny=B, nz=B)
+        cut = lambda a: np.ascontiguousarray(a[..., z0:z0 + B, y0:y0 + B, x0:x0 + B])
+        o = vo.Oracle(sub)
+        o.set_initial(cut(init["e"]), cut(init["u"]))
+        o.step(2)
+        fo = o.get_fields()
+        # inner region: H cells from a cut face, 0 from a face that coincides with the domain boundary
+        lo = lambda c0: 0 if c0 == 0 else H
+        hi = lambda c0: B if c0 + B == 128 else B - H
+        sl = (slice(lo(z0), hi(z0)), slice(lo(y0), hi(y0)), slice(lo(x0), hi(x0)))
+        gl = (slice(z0 + sl[0].start, z0 + sl[0].stop), slice(y0 + sl[1].start, y0 + sl[1].stop), slice(x0 + sl[2].start, x0 + sl[2].stop))
+        S = np.max(np.abs(fo["q"][0]))
+        for n in range(15):
+            a, b = fo["q"][n][0][sl], fg["q"][n][0][gl]
+            worst = max(worst, np.max(np.abs(a - b)) / max(np.max(np.abs(fo["q"][n])), NOISE * S))
+        worst = max(worst, np.max(np.abs(fo["e"][0][sl] - fg["e"][0][gl])) / np.max(np.abs(fo["e"])))
+        for m in range(4):
+            worst = max(worst, np.max(np.abs(fo["u"][m][0][sl] - fg["u"][m][0][gl])) / max(np.max(np.abs(fo["u"][m])), NOISE))
+    assert worst <= TOL, worst
