@@ -1,6 +1,6 @@
 // vh_api.cu -- C ABI (include/vh.h): handle, buffers, buffer rotation (PAPER.md program-flow steps 7, 9), kernel dispatch.
 #include "../../include/vh.h"
-#include "vh_kernels.cuh"
+#include "vh_kernels2.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -18,11 +18,13 @@ struct vh_handle {
   vh_params prm;
   DevParams P;
   cudaStream_t stream = nullptr;
-  double* pool = nullptr;            // 61 padded arrays
+  double* pool = nullptr;            // 67 padded arrays
   double* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
   double* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
   double* e[2] = {nullptr, nullptr};            // e^n / e^{n+1}, e*
   double* p[2] = {nullptr, nullptr};
+  double* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
+  double* vR = nullptr;              // [3] ... high face
   Counters* cnt = nullptr;
   double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
   double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
@@ -30,7 +32,7 @@ struct vh_handle {
   long long launches = 0;
   bool initialised = false;
   bool two_d = false;
-  int variant = 0;
+  int variant = 0;                   // 0: split pipeline (velocity + stage kernels); 1: one-thread-per-cell kernel + ghost kernel
   std::string err;
 };
 
@@ -131,6 +133,39 @@ static cudaError_t launch_stage(vh_handle* h, int stage, const StageArgs& A) {
   if (milne) return eos ? launch_stage_d<1, false, true>(h, stage, A) : launch_stage_d<0, false, true>(h, stage, A);
   return eos ? launch_stage_d<1, false, false>(h, stage, A) : launch_stage_d<0, false, false>(h, stage, A);
 }
+
+// ---- split pipeline (variant 0): velocity kernel + stage kernel (vh_kernels2.cuh)
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
+static cudaError_t launch_split_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid) {
+  const DevParams& P = h->P;
+  constexpr int BX = 32, BY = TWO_D ? 8 : 4, BZ = TWO_D ? 1 : 2;
+  dim3 block(BX, BY, BZ);
+  dim3 grid((P.nx + BX - 1) / BX, (P.ny + BY - 1) / BY, ((P.nz + BZ - 1) / BZ) * P.n_batch);
+  VelArgs V{S.q_in, S.e_in, h->vL, h->vR, S.cnt, S.t};
+  velocity_kernel<EOS, VISC, MILNE, TWO_D, THETA1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, V);
+  h->launches++;
+  cudaError_t e = debug_sync(h, "velocity kernel");
+  if (e != cudaSuccess) return e;
+  if (mid) cudaEventRecord(mid, h->stream);
+  Stage2Args A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post};
+  if (stage == 1) stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, A);
+  else stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, A);
+  h->launches++;
+  return debug_sync(h, stage == 1 ? "stage 1 kernel" : "stage 2 kernel");
+}
+template <int EOS, bool VISC, bool MILNE>
+static cudaError_t launch_split_d(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+  const bool th1 = h->prm.minmod_theta == 1.0;
+  if (h->two_d) return th1 ? launch_split_t<EOS, VISC, MILNE, true, true>(h, stage, A, mid) : launch_split_t<EOS, VISC, MILNE, true, false>(h, stage, A, mid);
+  return th1 ? launch_split_t<EOS, VISC, MILNE, false, true>(h, stage, A, mid) : launch_split_t<EOS, VISC, MILNE, false, false>(h, stage, A, mid);
+}
+static cudaError_t launch_split(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+  const bool visc = h->prm.physics != 0, milne = h->prm.geometry == 0;
+  const int eos = h->prm.eos;
+  if (visc) return eos ? launch_split_d<1, true, true>(h, stage, A, mid) : launch_split_d<0, true, true>(h, stage, A, mid);
+  if (milne) return eos ? launch_split_d<1, false, true>(h, stage, A, mid) : launch_split_d<0, false, true>(h, stage, A, mid);
+  return eos ? launch_split_d<1, false, false>(h, stage, A, mid) : launch_split_d<0, false, false>(h, stage, A, mid);
+}
 static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, double* u) {
   const DevParams& P = h->P;
   long long W = h->two_d ? (long long)P.ny + P.nx : (long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny;
@@ -159,7 +194,7 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   h->two_d = (p->nz == 1);
   h->stream = (cudaStream_t)cuda_stream;
   const long long fs = h->P.fstride;
-  const size_t bytes = (size_t)61 * fs * sizeof(double);
+  const size_t bytes = (size_t)67 * fs * sizeof(double);
   ce = cudaMalloc((void**)&h->pool, bytes);
   if (ce != cudaSuccess) { delete h; return fail(nullptr, VH_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes: " + cudaGetErrorString(ce)); }
   ce = cudaMalloc((void**)&h->cnt, sizeof(Counters));
@@ -169,6 +204,8 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   for (int i = 0; i < 3; ++i) { h->u[i] = w; w += 4 * fs; }
   for (int i = 0; i < 2; ++i) { h->e[i] = w; w += fs; }
   for (int i = 0; i < 2; ++i) { h->p[i] = w; w += fs; }
+  h->vL = w; w += 3 * fs;
+  h->vR = w; w += 3 * fs;
   ce = cudaMemsetAsync(h->pool, 0, bytes, h->stream);
   if (ce != cudaSuccess) { cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_CUDA, "cudaMemsetAsync failed"); }
   *out = h;
@@ -307,18 +344,29 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   // steps 1-4: q* = E[q^n; e,p,u^n,u^{n-1}] at tau^n, then (e*,p*,u*) at tau^n + dtau, regulate, ghosts
   A.q_in = h->q[0]; A.e_in = h->e[0]; A.p_in = h->p[0]; A.u_in = h->u[0]; A.u_prev = h->u[1]; A.q_n = nullptr;
   A.q_out = h->q[1]; A.e_out = h->e[1]; A.p_out = h->p[1]; A.u_out = h->u[2]; A.cnt = h->cnt; A.t = t; A.t_post = t1;
+  // variant 0: (velocity kernel, stage kernel) per stage, ghost replicas written by the stage kernel;
+  // variant 1: (cell kernel, ghost kernel) per stage.  ev[0..4] bracket the four launches of the step.
+  const bool split = (h->variant == 0);
   if (ev) CUDA_TRY(h, cudaEventRecord(ev[0], h->stream));
-  CUDA_TRY(h, launch_stage(h, 1, A));
-  if (ev) CUDA_TRY(h, cudaEventRecord(ev[1], h->stream));
-  CUDA_TRY(h, launch_ghost(h, h->q[1], h->e[1], h->p[1], h->u[2]));
+  if (split) {
+    CUDA_TRY(h, launch_split(h, 1, A, ev ? ev[1] : nullptr));
+  } else {
+    CUDA_TRY(h, launch_stage(h, 1, A));
+    if (ev) CUDA_TRY(h, cudaEventRecord(ev[1], h->stream));
+    CUDA_TRY(h, launch_ghost(h, h->q[1], h->e[1], h->p[1], h->u[2]));
+  }
   if (ev) CUDA_TRY(h, cudaEventRecord(ev[2], h->stream));
   // steps 5-8: q** = E[q*; e*,p*,u*,u^n] at tau^n + dtau; q^{n+1} = (q^n + q**)/2; invert, regulate, ghosts.
   // u^{n+1} overwrites the buffer of u^{n-1}, e^{n+1}/p^{n+1} the buffers of e^n/p^n (neither is read by stage 2).
   A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
   A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1]; A.t = t1; A.t_post = t1;
-  CUDA_TRY(h, launch_stage(h, 2, A));
-  if (ev) CUDA_TRY(h, cudaEventRecord(ev[3], h->stream));
-  CUDA_TRY(h, launch_ghost(h, h->q[2], h->e[0], h->p[0], h->u[1]));
+  if (split) {
+    CUDA_TRY(h, launch_split(h, 2, A, ev ? ev[3] : nullptr));
+  } else {
+    CUDA_TRY(h, launch_stage(h, 2, A));
+    if (ev) CUDA_TRY(h, cudaEventRecord(ev[3], h->stream));
+    CUDA_TRY(h, launch_ghost(h, h->q[2], h->e[0], h->p[0], h->u[1]));
+  }
   if (ev) CUDA_TRY(h, cudaEventRecord(ev[4], h->stream));
   // steps 7, 9: rotate.  u: (u^n, u^{n-1}, u*) <- (u^{n+1}, u^n, scratch); q: q^n <-> q^{n+1}
   double* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;

@@ -1,0 +1,145 @@
+// vh_math.cuh -- FP64 building blocks of the product kernels: branch-free reciprocal / square roots built on the MUFU
+// seeds (a few DFMA instead of the IEEE slow-path calls), the minmod-limited half slope (Eqs. 67-68) with the sign
+// logic on the integer pipe, and the paired Newton-Raphson inversion of Eq. 72.  Shares nothing with oracle/.
+#pragma once
+#include "vh_device.cuh"
+
+namespace vh {
+
+// 1/x to ~1 ulp: MUFU.RCP64H seed (~20 bits) + two Newton steps.  No denormal / overflow slow path: callers pass
+// well-scaled positive quantities; inf/NaN/0 propagate as NaN/inf and are caught by the callers' finiteness checks.
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = fma(-x, y, 1.0);
+  y = fma(y, t, y);
+  t = fma(-x, y, 1.0);
+  return fma(y, t, y);
+}
+// one Newton step only (~40 bits): enough wherever the quotient only steers an iteration
+__device__ __forceinline__ double rcp_half(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = fma(-x, y, 1.0);
+  return fma(y, t, y);
+}
+// 1/sqrt(x) to ~1 ulp: MUFU.RSQ64H seed + two Newton steps
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double hx = 0.5 * x;
+  double t = fma(-hx * y, y, 0.5);
+  y = fma(y, t, y);
+  t = fma(-hx * y, y, 0.5);
+  return fma(y, t, y);
+}
+// sqrt(x) for x > 0 (x = 0 gives 0): x * rsqrt(x) with one correction step
+__device__ __forceinline__ double sqrt_fast(double x) {
+  double r = rsqrt_fast(x);
+  double s = x * r;
+  double d = fma(-s, s, x);
+  s = fma(0.5 * r, d, s);
+  return (x > 0.0) ? s : 0.0;
+}
+
+// (dr/2) * minmod(theta d1/dr, (d1+d2)/(2 dr), theta d2/dr) with d1 = q0 - qm, d2 = qp - q0   (Eqs. 67-68, R10).
+// When d1, d2 have the same sign the centred difference has it too and |d1+d2|/2 = (|d1|+|d2|)/2; for theta = 1 it lies
+// between the one-sided ones and drops out.  A zero one-sided difference gives min = 0, so only the sign bits are compared.
+template <bool THETA1>
+__device__ __forceinline__ double half_slope2(double d1, double d2, double half_theta) {
+  const double a1 = fabs(d1), a2 = fabs(d2);
+  double m = (a1 < a2) ? a1 : a2;
+  if (THETA1) {
+    m *= 0.5;
+  } else {
+    m *= half_theta;
+    const double b = 0.25 * (a1 + a2);
+    m = (b < m) ? b : m;
+  }
+  const int h1 = __double2hiint(d1), h2 = __double2hiint(d2);
+  const bool opposite = (h1 ^ h2) < 0;
+  int mh = __double2hiint(m) | (h1 & 0x80000000);
+  double r = __hiloint2double(mh, __double2loint(m));
+  return opposite ? 0.0 : r;
+}
+
+// ---------------------------------------------------------------- paired Newton-Raphson on Eq. 72 (R6)
+// Two independent states are iterated together so that their dependent FP64 chains interleave.  Same stopping rule, cap and
+// failure semantics as invert_energy(); a converged state stops updating while its partner (or another lane) iterates.
+struct NewtonState {
+  double E, M2, Pi;     // inputs
+  double e;             // iterate
+  double p, rden;       // P0 and 1/(E + P0 + Pi) extrapolated to the returned e (valid when !fail)
+  bool fail;
+};
+
+template <int EOS>
+__device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, NewtonState& B, double guess) {
+  const bool gok = (guess > 0.0) && isfinite(guess);
+  bool badA = !(A.E > 0.0) || !isfinite(A.E) || !isfinite(A.M2) || !isfinite(A.Pi);
+  bool badB = !(B.E > 0.0) || !isfinite(B.E) || !isfinite(B.M2) || !isfinite(B.Pi);
+  A.e = gok ? guess : A.E;
+  B.e = gok ? guess : B.E;
+  bool doneA = badA, doneB = badB, convA = false, convB = false;
+  A.p = 0.0; B.p = 0.0; A.rden = 0.0; B.rden = 0.0;
+  for (int it = 0; it < P.newton_max_iter; ++it) {
+    if (__all_sync(0xffffffffu, doneA && doneB)) break;
+    double pA, cA, pB, cB;
+    eos_p_cs2<EOS>(P, A.e, pA, cA);
+    eos_p_cs2<EOS>(P, B.e, pB, cB);
+    const double rA = rcp_fast(A.E + pA + A.Pi), rB = rcp_fast(B.E + pB + B.Pi);
+    const double fA = A.e - A.E + A.M2 * rA, fB = B.e - B.E + B.M2 * rB;
+    const double gA = fma(-A.M2 * cA, rA * rA, 1.0), gB = fma(-B.M2 * cB, rB * rB, 1.0);
+    const double dA = fA * rcp_fast(gA), dB = fB * rcp_fast(gB);
+    const double eA = A.e - dA, eB = B.e - dB;
+    if (!doneA) {
+      A.e = eA;
+      A.p = fma(-cA, dA, pA);                    // P0(e - de) = P0(e) - cs2 de + O(de^2), de <= rtol e at convergence
+      A.rden = fma(rA * rA, cA * dA, rA);        // 1/(den - cs2 de) to the same order
+      if (fabs(dA) <= P.newton_rtol * fabs(eA)) { convA = true; doneA = true; }
+    }
+    if (!doneB) {
+      B.e = eB;
+      B.p = fma(-cB, dB, pB);
+      B.rden = fma(rB * rB, cB * dB, rB);
+      if (fabs(dB) <= P.newton_rtol * fabs(eB)) { convB = true; doneB = true; }
+    }
+  }
+  A.fail = badA || !convA || !(A.e > 0.0) || !isfinite(A.e);
+  B.fail = badB || !convB || !(B.e > 0.0) || !isfinite(B.e);
+  if (A.fail) { A.e = fmax(A.E, 1e-300); A.p = eos_p<EOS>(P, A.e); A.rden = 1.0 / (A.E + A.p + A.Pi); }
+  if (B.fail) { B.e = fmax(B.E, 1e-300); B.p = eos_p<EOS>(P, B.e); B.rden = 1.0 / (B.E + B.p + B.Pi); }
+}
+
+// single state (cell inversion in the stage epilogue)
+template <int EOS>
+__device__ __forceinline__ double newton_single(const DevParams& P, double E, double M2, double Pi, double guess, bool& fail) {
+  const bool bad = !(E > 0.0) || !isfinite(E) || !isfinite(M2) || !isfinite(Pi);
+  double e = ((guess > 0.0) && isfinite(guess)) ? guess : E;
+  bool done = bad, conv = false;
+  for (int it = 0; it < P.newton_max_iter; ++it) {
+    if (__all_sync(0xffffffffu, done)) break;
+    double p, c;
+    eos_p_cs2<EOS>(P, e, p, c);
+    const double r = rcp_fast(E + p + Pi);
+    const double f = e - E + M2 * r;
+    const double g = fma(-M2 * c, r * r, 1.0);
+    const double d = f * rcp_fast(g);
+    const double en = e - d;
+    if (!done) {
+      e = en;
+      if (fabs(d) <= P.newton_rtol * fabs(en)) { conv = true; done = true; }
+    }
+  }
+  fail = bad || !conv || !(e > 0.0) || !isfinite(e);
+  if (fail) e = fmax(E, 1e-300);
+  return e;
+}
+
+// clip of a failed state's velocity (R6)
+__device__ __forceinline__ double clip_velocity(double v) {
+  if (!(fabs(v) < 1.0)) v = (v > 0.0) ? 1.0 - 1e-12 : ((v < 0.0) ? -1.0 + 1e-12 : 0.0);
+  return v;
+}
+
+}  // namespace vh
