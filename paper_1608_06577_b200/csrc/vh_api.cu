@@ -12,6 +12,10 @@
 
 using namespace vh;
 
+#ifndef VH_STAGE_MINB
+#define VH_STAGE_MINB 2      // resident blocks per SM the stage kernel is compiled for (register cap 65536/(256*MINB))
+#endif
+
 static thread_local std::string g_err;
 
 struct vh_handle {
@@ -148,8 +152,8 @@ static cudaError_t launch_split_t(vh_handle* h, int stage, const StageArgs& S, c
   if (e != cudaSuccess) return e;
   if (mid) cudaEventRecord(mid, h->stream);
   Stage2Args A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post};
-  if (stage == 1) stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, A);
-  else stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, A);
+  if (stage == 1) stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1, BX, BY, BZ, VH_STAGE_MINB><<<grid, block, 0, h->stream>>>(P, A);
+  else stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2, BX, BY, BZ, VH_STAGE_MINB><<<grid, block, 0, h->stream>>>(P, A);
   h->launches++;
   return debug_sync(h, stage == 1 ? "stage 1 kernel" : "stage 2 kernel");
 }

@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(BX* BY* BZ) velocity_kernel(const __grid_const
 
 // ------------------------------------------------------------------------------------------------ flux divergence
 // acc[n] -= dtau/dr (H_{+1/2} - H_{-1/2}) for direction of stride s, with H = cp q^+ + cm q^- where
-// cp = (v^+ - a)/2, cm = (v^- + a)/2, a = max(|v^+|,|v^-|)   (Eqs. 61-62 regrouped).
+// cp = (v^+ - a)/2, cm = (v^- + a)/2, a = max(|v^+|,|v^-|)   (Eqs. 61-62 regrouped; dtau/dr folded into cp, cm).
 template <bool VISC, bool THETA1>
 __device__ __forceinline__ void flux_dir2(const DevParams& P, const double* __restrict__ q, const double* __restrict__ vL,
                                           const double* __restrict__ vR, long long s, double w, double* acc) {
@@ -125,8 +125,8 @@ __device__ __forceinline__ void flux_dir2(const DevParams& P, const double* __re
     const double vm_lo = vR[-s], vp_lo = vL[0], vm_hi = vR[0], vp_hi = vL[s];
     const double a_lo = fmax(fabs(vm_lo), fabs(vp_lo)), a_hi = fmax(fabs(vm_hi), fabs(vp_hi));
     const double hw = 0.5 * w;
-    cph = hw * (vp_hi - a_hi); cmh = hw * (vm_hi + a_hi);
-    cpl = hw * (vp_lo - a_lo); cml = hw * (vm_lo + a_lo);
+    cph = hw * (a_hi - vp_hi); cmh = -hw * (vm_hi + a_hi);      // -dtau/dr * (cp, cm) of the high face
+    cpl = hw * (vp_lo - a_lo); cml = hw * (vm_lo + a_lo);       // +dtau/dr * (cp, cm) of the low face
   }
 #pragma unroll
   for (int n = 0; n < NF; ++n) {
@@ -134,29 +134,31 @@ __device__ __forceinline__ void flux_dir2(const DevParams& P, const double* __re
     const double a0 = f[-2 * s], a1 = f[-s], a2 = f[0], a3 = f[s], a4 = f[2 * s];
     const double d0 = a1 - a0, d1 = a2 - a1, d2 = a3 - a2, d3 = a4 - a3;
     const double hm = half_slope2<THETA1>(d0, d1, ht), h0 = half_slope2<THETA1>(d1, d2, ht), hp = half_slope2<THETA1>(d2, d3, ht);
-    const double Hhi = fma(cph, a3 - hp, cmh * (a2 + h0));      // q^+_{+1/2} (Eq. 63), q^-_{+1/2} (Eq. 64)
-    const double Hlo = fma(cpl, a2 - h0, cml * (a1 + hm));      // q^+_{-1/2} (Eq. 65), q^-_{-1/2} (Eq. 66)
-    acc[n] -= Hhi - Hlo;
+    double r = acc[n];
+    r = fma(cph, a3 - hp, r);      // q^+_{+1/2} (Eq. 63)
+    r = fma(cmh, a2 + h0, r);      // q^-_{+1/2} (Eq. 64)
+    r = fma(cpl, a2 - h0, r);      // q^+_{-1/2} (Eq. 65)
+    r = fma(cml, a1 + hm, r);      // q^-_{-1/2} (Eq. 66)
+    acc[n] = r;
   }
 }
 
-// ------------------------------------------------------------------------------------------------ sources (App. B)
-// Adds dtau * J to acc.
-template <int EOS, bool VISC, bool MILNE, bool TWO_D>
-__device__ __forceinline__ void sources2(const DevParams& P, const Stage2Args& A, long long c, double t, const double* qc, double ec, double pc,
-                                         const double* uc, double* acc) {
+// ------------------------------------------------------------------------------------------------ conservation sources
+// acc[0..3] += dtau (S_c + G_c) (B.2-B.5, :1013) and the velocity gradients du[a][n] = partial_a u^n, div v (:424).
+template <bool VISC, bool MILNE, bool TWO_D>
+__device__ __forceinline__ void conservation_sources2(const DevParams& P, const Stage2Args& A, long long c, double t, const double* uc,
+                                                      double* acc, double du[4][4], double& divv) {
   const double* __restrict__ q = A.q_in;
   const double* __restrict__ pp = A.p_in;
   const double* __restrict__ uu = A.u_in;
   const long long fs = P.fstride;
   const double t2 = MILNE ? t * t : 1.0;
-  const double it = MILNE ? 1.0 / t : 1.0;
+  const double it = MILNE ? rcp_fast(t) : 1.0;
   const double it2 = it * it;
   const double dt = P.dtau;
   const long long strides[3] = {1, (long long)P.NXp, P.plane};
   const double hinv[3] = {0.5 * P.inv_dx, 0.5 * P.inv_dy, 0.5 * P.inv_dz};
-  double du[4][4];     // du[a][n] = partial_a u^n ; a = 0 is time (backward difference, :424)
-  double divv = 0.0;
+  divv = 0.0;
 #pragma unroll
   for (int n = 0; n < 4; ++n) du[0][n] = VISC ? (uc[n] - A.u_prev[n * fs + c]) * P.inv_dtau : 0.0;
 #pragma unroll
@@ -182,20 +184,20 @@ __device__ __forceinline__ void sources2(const DevParams& P, const Stage2Args& A
         const double ptt = q[PTT * fs + cn], ptx = q[PTX * fs + cn], pty = q[PTY * fs + cn], ptn = q[PTN * fs + cn];
         // A^{i nu} = P (v^i delta^nu_tau - g^{i nu}) - v^i pi^{tau nu} + pi^{i nu}   (B.2-B.5)
         if (d == 0) {
-          Ax[0] = vi * (Pt - ptt) + ptx;
-          Ax[1] = Pt - vi * ptx + q[PXX * fs + cn];
-          Ax[2] = -vi * pty + q[PXY * fs + cn];
-          Ax[3] = -vi * ptn + q[PXN * fs + cn];
+          Ax[0] = fma(vi, Pt - ptt, ptx);
+          Ax[1] = fma(-vi, ptx, Pt + q[PXX * fs + cn]);
+          Ax[2] = fma(-vi, pty, q[PXY * fs + cn]);
+          Ax[3] = fma(-vi, ptn, q[PXN * fs + cn]);
         } else if (d == 1) {
-          Ax[0] = vi * (Pt - ptt) + pty;
-          Ax[1] = -vi * ptx + q[PXY * fs + cn];
-          Ax[2] = Pt - vi * pty + q[PYY * fs + cn];
-          Ax[3] = -vi * ptn + q[PYN * fs + cn];
+          Ax[0] = fma(vi, Pt - ptt, pty);
+          Ax[1] = fma(-vi, ptx, q[PXY * fs + cn]);
+          Ax[2] = fma(-vi, pty, Pt + q[PYY * fs + cn]);
+          Ax[3] = fma(-vi, ptn, q[PYN * fs + cn]);
         } else {
-          Ax[0] = vi * (Pt - ptt) + ptn;
-          Ax[1] = -vi * ptx + q[PXN * fs + cn];
-          Ax[2] = -vi * pty + q[PYN * fs + cn];
-          Ax[3] = Pt * it2 - vi * ptn + q[PNN * fs + cn];
+          Ax[0] = fma(vi, Pt - ptt, ptn);
+          Ax[1] = fma(-vi, ptx, q[PXN * fs + cn]);
+          Ax[2] = fma(-vi, pty, q[PYN * fs + cn]);
+          Ax[3] = fma(-vi, ptn, fma(Pt, it2, q[PNN * fs + cn]));
         }
       } else {
         Ax[0] = vi * Pt;
@@ -203,87 +205,177 @@ __device__ __forceinline__ void sources2(const DevParams& P, const Stage2Args& A
         Ax[2] = (d == 1) ? Pt : 0.0;
         Ax[3] = (d == 2) ? Pt * it2 : 0.0;
       }
-      divv += (side ? vi : -vi) * hinv[d];
+      divv = fma(side ? vi : -vi, hinv[d], divv);
     }
     const double wd = dt * hinv[d];
 #pragma unroll
     for (int n = 0; n < 4; ++n) {
-      acc[n] -= (Ap[n] - Am[n]) * wd;
+      acc[n] = fma(Am[n] - Ap[n], wd, acc[n]);
       du[d + 1][n] = (up[n] - um[n]) * hinv[d];
     }
   }
   if (MILNE) {     // G_c (:1013), T^{eta eta} from Eq. 34
-    const double Ptc = pc + (VISC ? qc[BPI] : 0.0);
-    const double Tnn = (ec + Ptc) * uc[3] * uc[3] + Ptc * it2 + (VISC ? qc[PNN] : 0.0);
+    const double ec = A.e_in[c], pc = pp[c];
+    const double Ptc = pc + (VISC ? q[BPI * fs + c] : 0.0);
+    const double Tnn = fma((ec + Ptc) * uc[3], uc[3], fma(Ptc, it2, VISC ? q[PNN * fs + c] : 0.0));
     const double wt = dt * it;
-    acc[0] -= (qc[TTT] + t2 * Tnn) * wt;
-    acc[1] -= qc[TTX] * wt;
-    acc[2] -= qc[TTY] * wt;
-    acc[3] -= 3.0 * qc[TTN] * wt;
-  }
-  if (VISC) {
-    Kin K;
-    kinematics(uc, du[0], du[1], du[2], du[3], t, K);
-    double p0, cs2;
-    eos_p_cs2<EOS>(P, ec, p0, cs2);
-    double Jpi[10], JPi;
-    dissipative_sources<EOS>(P, t, uc, K, qc + PTT, qc[BPI], ec, p0, cs2, divv, Jpi, JPi);
-    if (P.shear) {
-#pragma unroll
-      for (int n = 0; n < 10; ++n) acc[PTT + n] = fma(dt, Jpi[n], acc[PTT + n]);
-    }
-    if (P.bulk) acc[BPI] = fma(dt, JPi, acc[BPI]);
+    acc[0] = fma(-wt, fma(t2, Tnn, q[TTT * fs + c]), acc[0]);
+    acc[1] = fma(-wt, q[TTX * fs + c], acc[1]);
+    acc[2] = fma(-wt, q[TTY * fs + c], acc[2]);
+    acc[3] = fma(-3.0 * wt, q[TTN * fs + c], acc[3]);
   }
 }
 
+// ------------------------------------------------------------------------------------------------ dissipative sources
+// J = S + G for pi^{mu nu} (10) and Pi (B.10-B.12, Eqs. 39-46), one component at a time: emit(slot, J).
+template <int EOS, class Emit>
+__device__ __forceinline__ void dissipative_sources2(const DevParams& P, double t, const double u[4], const Kin& K, const double pi[10], double Pi,
+                                                     double e, double divv, Emit emit) {
+  const double t2 = t * t, it = rcp_fast(t);
+  // transport coefficients (Eqs. 10-16; R14)
+  double p, cs2;
+  eos_p_cs2<EOS>(P, e, p, cs2);
+  const double T = sqrt_fast(sqrt_fast(e * P.eos_a_inv));
+  const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
+  const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
+  double zs = 0.0;
+  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp(-d * d); }
+  else if (P.zeta_model == 2) zs = P.zeta_amp;
+  const double b = (1.0 / 3.0) - cs2;
+  double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi / zs : CUDART_INF;
+  itP = fmin(itP, P.relax_clamp);
+  const double zotP = (zs > 0.0) ? zs * ((e + p) / T) * itP : 0.0;
+  const double lPp = P.lambda_Pipi_coef * b;
+  const double iut = rcp_fast(u[0]);
+  const double ut = u[0], un = u[3];
+
+  // pi^{mu nu} sigma_{mu nu}: symmetric double contraction with the metric weights of g = diag(1,-1,-1,-t2)
+  const double* S = K.sig;
+  const double pisig = pi[0] * S[0] - 2.0 * (pi[1] * S[1] + pi[2] * S[2]) + pi[4] * S[4] + 2.0 * pi[5] * S[5] + pi[7] * S[7] +
+                       t2 * (2.0 * (pi[6] * S[6] + pi[8] * S[8] - pi[3] * S[3]) + t2 * pi[9] * S[9]);
+  // A^mu = pi^{lambda mu} Du_lambda (Eq. 43)
+  double Av[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+    Av[m] = pi[sym(0, m)] * K.Du[0] + pi[sym(1, m)] * K.Du[1] + pi[sym(2, m)] * K.Du[2] + pi[sym(3, m)] * K.Du[3];
+  // g_l W^{l n} and g_l sigma^{l n} (rows scaled by the metric)
+  double gW[4][4], gS[4][4];
+  {
+    const double W01 = K.W[0], W02 = K.W[1], W03 = K.W[2], W12 = K.W[3], W13 = K.W[4], W23 = K.W[5];
+    gW[0][0] = 0.0;      gW[0][1] = W01;       gW[0][2] = W02;       gW[0][3] = W03;
+    gW[1][0] = W01;      gW[1][1] = 0.0;       gW[1][2] = -W12;      gW[1][3] = -W13;
+    gW[2][0] = W02;      gW[2][1] = W12;       gW[2][2] = 0.0;       gW[2][3] = -W23;
+    gW[3][0] = t2 * W03; gW[3][1] = t2 * W13;  gW[3][2] = t2 * W23;  gW[3][3] = 0.0;
+#pragma unroll
+    for (int n = 0; n < 4; ++n) {
+      gS[0][n] = S[sym(0, n)]; gS[1][n] = -S[sym(1, n)]; gS[2][n] = -S[sym(2, n)]; gS[3][n] = -t2 * S[sym(3, n)];
+    }
+  }
+  const double it2 = it * it;
+  const double gi[4] = {1.0, -1.0, -1.0, -it2};
+  const double third_pisig = (1.0 / 3.0) * pisig;
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = m; n < 4; ++n) {
+      const int s = sym(m, n);
+      double B = 0.0, C = 0.0;     // B = pi^{m l} g_l W^{l n} + (m<->n) ; C = pi^{m l} g_l sigma^{l n} + (m<->n)
+#pragma unroll
+      for (int l = 0; l < 4; ++l) {
+        if (l != n) B = fma(pi[sym(m, l)], gW[l][n], B);
+        if (l != m) B = fma(pi[sym(n, l)], gW[l][m], B);
+        C = fma(pi[sym(m, l)], gS[l][n], C);
+        C = fma(pi[sym(n, l)], gS[l][m], C);
+      }
+      const double Dmn = ((m == n) ? gi[m] : 0.0) - u[m] * u[n];
+      const double I1 = u[n] * Av[m] + u[m] * Av[n];                          // Eq. 43
+      const double I4 = 0.5 * C - Dmn * third_pisig;                          // Eq. 46
+      // Eq. 42: I1 + delta_pipi theta pi - I3 + tau_pipi I4 - lambda_piPi Pi sigma ; I3 = kVorticitySign * B (Eq. 45, R4)
+      double Ipi = I1 + P.delta_pipi * K.theta * pi[s] - kVorticitySign * B + P.tau_pipi * I4 - P.lambda_piPi * Pi * S[s];
+      // G_pi = u^a Gamma^mu_{ab} pi^{b nu} + (mu<->nu)  (:300; R1, R2)
+      double G = 0.0;
+      if (s == 0) G = 2.0 * t * un * pi[3];
+      if (s == 1) G = t * un * pi[6];
+      if (s == 2) G = t * un * pi[8];
+      if (s == 3) G = t * un * pi[9] + (ut * pi[3] + un * pi[0]) * it;
+      if (s == 6) G = (ut * pi[6] + un * pi[1]) * it;
+      if (s == 8) G = (ut * pi[8] + un * pi[2]) * it;
+      if (s == 9) G = 2.0 * (ut * pi[9] + un * pi[3]) * it;
+      emit(PTT + s, fma(fma(eotp2, S[s], -fma(pi[s], itp, Ipi + G)), iut, pi[s] * divv));      // B.11, B.9
+    }
+  const double IPi = P.delta_PiPi * Pi * K.theta - lPp * pisig;                                // Eq. 41
+  emit(BPI, fma(-fma(zotP, K.theta, fma(Pi, itP, IPi)), iut, Pi * divv));                       // B.10
+}
+
 // ------------------------------------------------------------------------------------------------ stage kernel
-template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE, int BX, int BY, int BZ>
-__global__ void __launch_bounds__(BX* BY* BZ) stage_kernel(const __grid_constant__ DevParams P, const __grid_constant__ Stage2Args A) {
+// Per-thread phases: (1) flux divergence, (2) conservation sources + velocity gradients, (3) kinematics + dissipative
+// sources, (4) cell inversion + regularisation, (5) stores with ghost replicas.  The 15 running values q + dtau C[q] are
+// parked in shared memory (one conflict-free slot per thread and field) between phases so that the register file holds
+// two blocks per SM.
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE, int BX, int BY, int BZ, int MINB>
+__global__ void __launch_bounds__(BX* BY* BZ, MINB) stage_kernel(const __grid_constant__ DevParams P, const __grid_constant__ Stage2Args A) {
+  constexpr int NT = BX * BY * BZ;
+  constexpr int NF = VISC ? NQ : 4;
+  __shared__ double park[NF][NT];
+  const int tid = threadIdx.x + BX * (threadIdx.y + BY * threadIdx.z);
   int i, j, k;
   long long c;
   const bool valid = cell_index<BX, BY, BZ>(P, i, j, k, c);
   const long long fs = P.fstride;
-  constexpr int NF = VISC ? NQ : 4;
   const double t = A.t;
   unsigned long long nfail = 0, nnonf = 0;
   double minfac = 1.0;
 
-  double qc[NQ], acc[NQ];
-#pragma unroll
-  for (int n = 0; n < NQ; ++n) { qc[n] = (n < NF) ? A.q_in[n * fs + c] : 0.0; acc[n] = qc[n]; }
-  const double ec = A.e_in[c], pc = A.p_in[c];
   double uc[4];
 #pragma unroll
   for (int n = 0; n < 4; ++n) uc[n] = A.u_in[n * fs + c];
-
-  // E[w] = w + dtau C[w]  (:413): flux divergence of every direction of extent > 1, then the sources
-  if (P.nx > 1) flux_dir2<VISC, THETA1>(P, A.q_in + c, A.vL + c, A.vR + c, 1, P.dtau * P.inv_dx, acc);
-  if (P.ny > 1) flux_dir2<VISC, THETA1>(P, A.q_in + c, A.vL + fs + c, A.vR + fs + c, P.NXp, P.dtau * P.inv_dy, acc);
-  if (!TWO_D) flux_dir2<VISC, THETA1>(P, A.q_in + c, A.vL + 2 * fs + c, A.vR + 2 * fs + c, P.plane, P.dtau * P.inv_dz, acc);
-  sources2<EOS, VISC, MILNE, TWO_D>(P, A, c, t, qc, ec, pc, uc, acc);
-
-  double qo[NQ];
+  {
+    double acc[NF];
 #pragma unroll
-  for (int n = 0; n < NQ; ++n) {
-    double v = 0.0;
-    if (n < NF) {
-      v = acc[n];
-      if (STAGE == 2) v = 0.5 * (A.q_n[n * fs + c] + v);           // Eq. 70, beta = 1/2
+    for (int n = 0; n < NF; ++n) acc[n] = A.q_in[n * fs + c];
+    // E[w] = w + dtau C[w]  (:413): flux divergence of every direction of extent > 1
+    if (P.nx > 1) flux_dir2<VISC, THETA1>(P, A.q_in + c, A.vL + c, A.vR + c, 1, P.dtau * P.inv_dx, acc);
+    if (P.ny > 1) flux_dir2<VISC, THETA1>(P, A.q_in + c, A.vL + fs + c, A.vR + fs + c, P.NXp, P.dtau * P.inv_dy, acc);
+    if (!TWO_D) flux_dir2<VISC, THETA1>(P, A.q_in + c, A.vL + 2 * fs + c, A.vR + 2 * fs + c, P.plane, P.dtau * P.inv_dz, acc);
+    if (VISC) {
+#pragma unroll
+      for (int n = 4; n < NF; ++n) park[n][tid] = acc[n];
     }
-    if (VISC && n >= PTT && n < BPI && !P.shear) v = 0.0;
-    if (VISC && n == BPI && !P.bulk) v = 0.0;
-    qo[n] = v;
+    double du[4][4], divv;
+    conservation_sources2<VISC, MILNE, TWO_D>(P, A, c, t, uc, acc, du, divv);
+#pragma unroll
+    for (int n = 0; n < 4; ++n) {
+      double v = acc[n];
+      if (STAGE == 2) v = 0.5 * (A.q_n[n * fs + c] + v);           // Eq. 70, beta = 1/2
+      park[n][tid] = v;
+    }
+    if (VISC) {
+      Kin K;
+      kinematics(uc, du[0], du[1], du[2], du[3], t, K);
+      double pi[10];
+#pragma unroll
+      for (int n = 0; n < 10; ++n) pi[n] = A.q_in[(PTT + n) * fs + c];
+      const double Pi = A.q_in[BPI * fs + c];
+      const double ec = A.e_in[c];
+      dissipative_sources2<EOS>(P, t, uc, K, pi, Pi, ec, divv, [&](int slot, double J) {
+        const bool on = (slot == BPI) ? (P.bulk != 0) : (P.shear != 0);
+        double v = fma(P.dtau, J, park[slot][tid]);
+        if (STAGE == 2) v = 0.5 * (A.q_n[slot * fs + c] + v);      // Eq. 70
+        park[slot][tid] = on ? v : 0.0;
+      });
+    }
   }
 
   // Post: Eqs. 52-54, 72 then 73-74 (R8: regulate after the inversion)
   const double tp = A.t_post;
   const double tp2 = MILNE ? tp * tp : 1.0;
-  const double E = qo[TTT] - (VISC ? qo[PTT] : 0.0);
-  const double Mx = qo[TTX] - (VISC ? qo[PTX] : 0.0), My = qo[TTY] - (VISC ? qo[PTY] : 0.0), Mn = qo[TTN] - (VISC ? qo[PTN] : 0.0);
-  const double Pi = VISC ? qo[BPI] : 0.0;
+  const double E = park[TTT][tid] - (VISC ? park[PTT][tid] : 0.0);
+  const double Mx = park[TTX][tid] - (VISC ? park[PTX][tid] : 0.0), My = park[TTY][tid] - (VISC ? park[PTY][tid] : 0.0),
+               Mn = park[TTN][tid] - (VISC ? park[PTN][tid] : 0.0);
+  const double Pi = VISC ? park[BPI][tid] : 0.0;
   const double M2 = Mx * Mx + My * My + tp2 * Mn * Mn;
   bool fail;
-  const double e = newton_single<EOS>(P, E, M2, Pi, ec, fail);
+  const double e = newton_single<EOS>(P, E, M2, Pi, A.e_in[c], fail);
   if (fail) ++nfail;
   const double p0 = eos_p<EOS>(P, e);
   const double Pt = p0 + Pi;
@@ -291,11 +383,13 @@ __global__ void __launch_bounds__(BX* BY* BZ) stage_kernel(const __grid_constant
   const double inv = rcp_fast((e + Pt) * ut);                    // Eq. 54
   const double u[4] = {ut, Mx * inv, My * inv, Mn * inv};
   if (!(isfinite(e) && isfinite(ut))) ++nnonf;
+  double fac = 1.0;
   if (VISC) {
-    const double fac = regulation_factor<MILNE>(P, qo, e, p0, u, tp);
-    minfac = fmin(minfac, fac);
+    double qo[NQ];
 #pragma unroll
-    for (int n = PTT; n < NQ; ++n) qo[n] *= fac;
+    for (int n = PTT; n < NQ; ++n) qo[n] = park[n][tid];
+    fac = regulation_factor<MILNE>(P, qo, e, p0, u, tp);
+    minfac = fmin(minfac, fac);
   }
 
   if (valid) {
@@ -316,7 +410,7 @@ __global__ void __launch_bounds__(BX* BY* BZ) stage_kernel(const __grid_constant
       }
     };
 #pragma unroll
-    for (int n = 0; n < NQ; ++n) put(A.q_out + n * fs, qo[n]);
+    for (int n = 0; n < NQ; ++n) put(A.q_out + n * fs, (n < NF) ? ((n >= PTT) ? park[n][tid] * fac : park[n][tid]) : 0.0);
     put(A.e_out, e);
     put(A.p_out, p0);
 #pragma unroll
