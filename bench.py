@@ -208,7 +208,7 @@ def main():
     st = s.status()
 
     # ---------------- per-kernel durations (CUDA events around each launch on the launching stream)
-    prof = s.step_profile(min(K, 10))
+    prof = s.step_profile(min(K, 10))       # launch order: velocity 1, stage 1, velocity 2, stage 2 (variants 0, 2)
 
     # ---------------- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()

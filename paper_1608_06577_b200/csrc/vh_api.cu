@@ -1,6 +1,6 @@
 // vh_api.cu -- C ABI (include/vh.h): handle, buffers, buffer rotation (PAPER.md program-flow steps 7, 9), kernel dispatch.
 #include "../../include/vh.h"
-#include "vh_kernels2.cuh"
+#include "vh_kernels3.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -36,7 +36,8 @@ struct vh_handle {
   long long launches = 0;
   bool initialised = false;
   bool two_d = false;
-  int variant = 0;                   // 0: split pipeline (velocity + stage kernels); 1: one-thread-per-cell kernel + ghost kernel
+  int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
+  CUtensorMap mapA, mapZ;            // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes)
   std::string err;
 };
 
@@ -170,6 +171,83 @@ static cudaError_t launch_split(vh_handle* h, int stage, const StageArgs& A, cud
   if (milne) return eos ? launch_split_d<1, false, true>(h, stage, A, mid) : launch_split_d<0, false, true>(h, stage, A, mid);
   return eos ? launch_split_d<1, false, false>(h, stage, A, mid) : launch_split_d<0, false, false>(h, stage, A, mid);
 }
+
+// ---- tile pipeline (variant 0): velocity kernel + TMA tile kernel (vh_kernels3.cuh)
+// One 5-d tensor map (x, y, eta, event, array) over the whole pool of padded arrays per box shape.  cuTensorMapEncodeTiled is a
+// driver-API entry point; it is looked up through the runtime so that the library needs no link-time dependency on libcuda.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static int make_tensor_maps(vh_handle* h, int n_arrays) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess || !fn)
+    return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  EncodeTiledFn encode = (EncodeTiledFn)fn;
+  const DevParams& P = h->P;
+  const cuuint64_t dims[5] = {(cuuint64_t)P.NXp, (cuuint64_t)P.NYp, (cuuint64_t)P.NZp, (cuuint64_t)P.n_batch, (cuuint64_t)n_arrays};
+  const cuuint64_t strides[4] = {(cuuint64_t)P.NXp * 8, (cuuint64_t)P.plane * 8, (cuuint64_t)P.bstride * 8, (cuuint64_t)P.fstride * 8};
+  const cuuint32_t ones[5] = {1, 1, 1, 1, 1};
+  const bool td = h->two_d;
+  const cuuint32_t boxA[5] = {(cuuint32_t)(td ? Tile<true>::AX : Tile<false>::AX), (cuuint32_t)(td ? Tile<true>::AY : Tile<false>::AY),
+                              (cuuint32_t)(td ? Tile<true>::TZ : Tile<false>::TZ), 1, 1};
+  const cuuint32_t boxZ[5] = {(cuuint32_t)Tile<false>::TX, (cuuint32_t)Tile<false>::TY, 2, 1, 1};
+  CUresult r = encode(&h->mapA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box A) failed with CUresult " + std::to_string((int)r));
+  r = encode(&h->mapZ, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box Z) failed with CUresult " + std::to_string((int)r));
+  return VH_OK;
+}
+
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
+static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
+  using T = Tile<TWO_D>;
+  constexpr int NF = VISC ? NQ : 4;
+  constexpr size_t smem = (size_t)(T::NSTAGE * T::SLOT + NF * T::NT) * sizeof(double) + T::NSTAGE * sizeof(uint64_t);
+  auto kern = stage_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE>;
+  static bool configured = false;      // one attribute call per instantiation (single device per process)
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const DevParams& P = h->P;
+  dim3 grid((P.nx + T::TX - 1) / T::TX, (P.ny + T::TY - 1) / T::TY, ((P.nz + T::TZ - 1) / T::TZ) * P.n_batch);
+  kern<<<grid, T::NT, smem, h->stream>>>(P, A, h->mapA, h->mapZ);
+  h->launches++;
+  return debug_sync(h, STAGE == 1 ? "stage 1 tile kernel" : "stage 2 tile kernel");
+}
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
+static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid) {
+  const DevParams& P = h->P;
+  constexpr int BX = 32, BY = TWO_D ? 8 : 4, BZ = TWO_D ? 1 : 2;
+  dim3 block(BX, BY, BZ);
+  dim3 grid((P.nx + BX - 1) / BX, (P.ny + BY - 1) / BY, ((P.nz + BZ - 1) / BZ) * P.n_batch);
+  VelArgs V{S.q_in, S.e_in, h->vL, h->vR, S.cnt, S.t};
+  velocity_kernel<EOS, VISC, MILNE, TWO_D, THETA1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, V);
+  h->launches++;
+  cudaError_t e = debug_sync(h, "velocity kernel");
+  if (e != cudaSuccess) return e;
+  if (mid) cudaEventRecord(mid, h->stream);
+  const long long fs = P.fstride;
+  TileArgs A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post,
+             (int)((S.q_in - h->pool) / fs), (int)((S.u_in - h->pool) / fs), (int)((S.p_in - h->pool) / fs)};
+  return (stage == 1) ? launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1>(h, A) : launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2>(h, A);
+}
+template <int EOS, bool VISC, bool MILNE>
+static cudaError_t launch_tile_d(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+  const bool th1 = h->prm.minmod_theta == 1.0;
+  if (h->two_d) return th1 ? launch_tile_t<EOS, VISC, MILNE, true, true>(h, stage, A, mid) : launch_tile_t<EOS, VISC, MILNE, true, false>(h, stage, A, mid);
+  return th1 ? launch_tile_t<EOS, VISC, MILNE, false, true>(h, stage, A, mid) : launch_tile_t<EOS, VISC, MILNE, false, false>(h, stage, A, mid);
+}
+static cudaError_t launch_tile(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+  const bool visc = h->prm.physics != 0, milne = h->prm.geometry == 0;
+  const int eos = h->prm.eos;
+  if (visc) return eos ? launch_tile_d<1, true, true>(h, stage, A, mid) : launch_tile_d<0, true, true>(h, stage, A, mid);
+  if (milne) return eos ? launch_tile_d<1, false, true>(h, stage, A, mid) : launch_tile_d<0, false, true>(h, stage, A, mid);
+  return eos ? launch_tile_d<1, false, false>(h, stage, A, mid) : launch_tile_d<0, false, false>(h, stage, A, mid);
+}
 static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, double* u) {
   const DevParams& P = h->P;
   long long W = h->two_d ? (long long)P.ny + P.nx : (long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny;
@@ -212,6 +290,11 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   h->vR = w; w += 3 * fs;
   ce = cudaMemsetAsync(h->pool, 0, bytes, h->stream);
   if (ce != cudaSuccess) { cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_CUDA, "cudaMemsetAsync failed"); }
+  if (make_tensor_maps(h, 67) != VH_OK) {
+    std::string msg = h->err;
+    cudaFree(h->pool); cudaFree(h->cnt); delete h;
+    return fail(nullptr, VH_ERR_CUDA, msg);
+  }
   *out = h;
   return VH_OK;
 }
@@ -231,7 +314,7 @@ long long vh_launch_count(vh_handle* h) { return h ? h->launches : 0; }
 
 int vh_set_kernel_variant(vh_handle* h, int variant) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
-  if (variant != 0 && variant != 1) return fail(h, VH_ERR_ARG, "unknown kernel variant");
+  if (variant < 0 || variant > 2) return fail(h, VH_ERR_ARG, "unknown kernel variant");
   h->variant = variant;
   return VH_OK;
 }
@@ -348,12 +431,13 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   // steps 1-4: q* = E[q^n; e,p,u^n,u^{n-1}] at tau^n, then (e*,p*,u*) at tau^n + dtau, regulate, ghosts
   A.q_in = h->q[0]; A.e_in = h->e[0]; A.p_in = h->p[0]; A.u_in = h->u[0]; A.u_prev = h->u[1]; A.q_n = nullptr;
   A.q_out = h->q[1]; A.e_out = h->e[1]; A.p_out = h->p[1]; A.u_out = h->u[2]; A.cnt = h->cnt; A.t = t; A.t_post = t1;
-  // variant 0: (velocity kernel, stage kernel) per stage, ghost replicas written by the stage kernel;
+  // variants 0, 2: (velocity kernel, stage kernel) per stage, ghost replicas written by the stage kernel;
   // variant 1: (cell kernel, ghost kernel) per stage.  ev[0..4] bracket the four launches of the step.
-  const bool split = (h->variant == 0);
+  const bool split = (h->variant != 1);
+  const bool tile = (h->variant == 0);
   if (ev) CUDA_TRY(h, cudaEventRecord(ev[0], h->stream));
   if (split) {
-    CUDA_TRY(h, launch_split(h, 1, A, ev ? ev[1] : nullptr));
+    CUDA_TRY(h, tile ? launch_tile(h, 1, A, ev ? ev[1] : nullptr) : launch_split(h, 1, A, ev ? ev[1] : nullptr));
   } else {
     CUDA_TRY(h, launch_stage(h, 1, A));
     if (ev) CUDA_TRY(h, cudaEventRecord(ev[1], h->stream));
@@ -365,7 +449,7 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
   A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1]; A.t = t1; A.t_post = t1;
   if (split) {
-    CUDA_TRY(h, launch_split(h, 2, A, ev ? ev[3] : nullptr));
+    CUDA_TRY(h, tile ? launch_tile(h, 2, A, ev ? ev[3] : nullptr) : launch_split(h, 2, A, ev ? ev[3] : nullptr));
   } else {
     CUDA_TRY(h, launch_stage(h, 2, A));
     if (ev) CUDA_TRY(h, cudaEventRecord(ev[3], h->stream));

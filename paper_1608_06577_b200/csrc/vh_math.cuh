@@ -1,6 +1,6 @@
 // vh_math.cuh -- FP64 building blocks of the product kernels: branch-free reciprocal / square roots built on the MUFU
 // seeds (a few DFMA instead of the IEEE slow-path calls), the minmod-limited half slope (Eqs. 67-68) with the sign
-// logic on the integer pipe, and the paired Newton-Raphson inversion of Eq. 72.  Shares nothing with oracle/.
+// logic on the integer pipe, and the paired Newton-Raphson inversion of Eq. 72.  Independent of the CPU test code.
 #pragma once
 #include "vh_device.cuh"
 
