@@ -37,7 +37,7 @@ struct vh_handle {
   bool initialised = false;
   bool two_d = false;
   int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
-  CUtensorMap mapA, mapZ;            // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes)
+  CUtensorMap mapA, mapZ, mapC;      // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes, box C: the tile)
   std::string err;
 };
 
@@ -197,14 +197,18 @@ static int make_tensor_maps(vh_handle* h, int n_arrays) {
   r = encode(&h->mapZ, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box Z) failed with CUresult " + std::to_string((int)r));
+  const cuuint32_t boxC[5] = {(cuuint32_t)Tile<false>::TX, (cuuint32_t)(td ? Tile<true>::TY : Tile<false>::TY),
+                              (cuuint32_t)(td ? Tile<true>::TZ : Tile<false>::TZ), 1, 1};
+  r = encode(&h->mapC, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxC, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box C) failed with CUresult " + std::to_string((int)r));
   return VH_OK;
 }
 
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
 static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
   using T = Tile<TWO_D>;
-  constexpr int NF = VISC ? NQ : 4;
-  constexpr size_t smem = (size_t)(T::NSTAGE * T::SLOT + NF * T::NT) * sizeof(double) + T::NSTAGE * sizeof(uint64_t);
+  constexpr size_t smem = tile_smem_bytes<TWO_D, VISC>();
   auto kern = stage_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE>;
   static bool configured = false;      // one attribute call per instantiation (single device per process)
   if (!configured) {
@@ -214,7 +218,7 @@ static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
   }
   const DevParams& P = h->P;
   dim3 grid((P.nx + T::TX - 1) / T::TX, (P.ny + T::TY - 1) / T::TY, ((P.nz + T::TZ - 1) / T::TZ) * P.n_batch);
-  kern<<<grid, T::NT, smem, h->stream>>>(P, A, h->mapA, h->mapZ);
+  kern<<<grid, T::NT, smem, h->stream>>>(P, A, h->mapA, h->mapZ, h->mapC);
   h->launches++;
   return debug_sync(h, STAGE == 1 ? "stage 1 tile kernel" : "stage 2 tile kernel");
 }

@@ -5,13 +5,16 @@
 // mbarrier ("full") that the loads complete with their byte count.  A slot holds the star-shaped neighbourhood of the
 // tile for one array: box A = (TX+4) x (TY+4) x TZ (the tile with its +-2 halo in x and y) plus, in 3+1d, two boxes of
 // TX x TY x 2 planes below and above the tile (the +-2 halo in eta); ghost edges / corners are never loaded (:453).
-// While array s is consumed the loads of arrays s+1 .. s+NSTAGE-1 are in flight, so no thread ever waits on a global load
-// in the stencil part.  Per array the thread reads its 13-point star from the slot and accumulates
+// While array s is consumed the loads of arrays s+1 .. s+NSTAGE-1 are in flight.  A slot is handed back by a counter:
+// lane 0 of every warp adds 1 (release) after the warp's reads, and the warp that completes the count re-arms the
+// barrier and issues the next loads into that slot - no block-wide barrier inside the stream.
+// Per array the thread reads its 13-point star from the slot and accumulates
 //   * the KT flux divergence of that field in x, y, eta (Eqs. 59-68) and
-//   * that field's contribution to the central-difference sources of the four conservation laws (B.2-B.5),
-// so each neighbour value is read once.  The running values q + dtau C[q] are parked in shared memory (one slot per
-// thread and field) until the epilogue: cell inversion (Eqs. 52-54, 72), regularisation (Eqs. 73-74), the stores and
-// the ghost-cell replicas (Eqs. 75-76).  See DESIGN.md "Kernels".
+//   * that field's contribution to the sources of the four conservation laws (B.2-B.5 and G_c, :1013),
+// so each neighbour value is read once.  The cell's own pi^{mu nu}, Pi (needed all at once by the relaxation sources,
+// Eqs. 39-46) arrive by eleven more TMA boxes, in thread order.  The running values q + dtau C[q] are parked in shared
+// memory (one slot per thread and field) until the epilogue: cell inversion (Eqs. 52-54, 72), regularisation
+// (Eqs. 73-74), the stores and the ghost-cell replicas (Eqs. 75-76).  See DESIGN.md "Kernels".
 #pragma once
 #include <cuda.h>
 #include <stdint.h>
@@ -25,12 +28,19 @@ template <bool TWO_D> struct Tile {
   static constexpr int TY = TWO_D ? 16 : 4;
   static constexpr int TZ = TWO_D ? 1 : 4;
   static constexpr int NT = TX * TY * TZ;                       // 512 threads
+  static constexpr int NW = NT / 32;                            // warps
   static constexpr int AX = TX + 4, AY = TY + 4;
   static constexpr int A_SIZE = AX * AY * TZ;                   // doubles in box A
   static constexpr int Z_SIZE = TWO_D ? 0 : TX * TY * 2;        // doubles in one eta-halo box
   static constexpr int SLOT = A_SIZE + 2 * Z_SIZE;              // doubles per ring slot (13312 B / 5760 B: multiples of 128)
   static constexpr int NSTAGE = 4;
+  static constexpr int NCEN = 11;                               // centre rows: pi^{mu nu} (10), Pi
 };
+template <bool TWO_D, bool VISC> constexpr size_t tile_smem_bytes() {
+  using T = Tile<TWO_D>;
+  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(double) + (T::NSTAGE + 1) * sizeof(uint64_t) +
+         T::NSTAGE * sizeof(unsigned);
+}
 
 struct TileArgs {
   const double* q_in; const double* e_in; const double* p_in; const double* u_in; const double* u_prev;
@@ -70,22 +80,30 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, u
       "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
       : "memory");
 }
+// counter of warps that are done with a ring slot: +1 with release/acquire ordering at CTA scope, returns the old value
+__device__ __forceinline__ unsigned slot_counter_add(unsigned* p) {
+  unsigned old;
+  asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(p)) : "memory");
+  return old;
+}
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ------------------------------------------------------------------------------------------------ flux of one field, one direction
-// r -= dtau/dr (H_{+1/2} - H_{-1/2}) from the five values a0..a4 along the direction (Eqs. 61-68; same grouping as flux_dir2)
+// r -= dtau/dr (H_{+1/2} - H_{-1/2}) from the five values a0..a4 along the direction (Eqs. 61-68): H = cp q^+ + cm q^- with
+// cp = (v^+ - a)/2, cm = (v^- + a)/2 (Eq. 61 regrouped), dtau/dr and the sign of the face folded into the coefficients.
 template <bool THETA1>
 __device__ __forceinline__ double flux_line(double a0, double a1, double a2, double a3, double a4, double cph, double cmh, double cpl,
-                                            double cml, double ht, double r) {
+                                            double cml, double theta, double r) {
   const double d0 = a1 - a0, d1 = a2 - a1, d2 = a3 - a2, d3 = a4 - a3;
-  const double hm = half_slope2<THETA1>(d0, d1, ht), h0 = half_slope2<THETA1>(d1, d2, ht), hp = half_slope2<THETA1>(d2, d3, ht);
-  r = fma(cph, a3 - hp, r);      // q^+_{+1/2} (Eq. 63)
-  r = fma(cmh, a2 + h0, r);      // q^-_{+1/2} (Eq. 64)
-  r = fma(cpl, a2 - h0, r);      // q^+_{-1/2} (Eq. 65)
-  r = fma(cml, a1 + hm, r);      // q^-_{-1/2} (Eq. 66)
+  const double sm = minmod_slope<THETA1>(d0, d1, theta), s0 = minmod_slope<THETA1>(d1, d2, theta), sp = minmod_slope<THETA1>(d2, d3, theta);
+  r = fma(cph, fma(-0.5, sp, a3), r);      // q^+_{+1/2} (Eq. 63)
+  r = fma(cmh, fma(0.5, s0, a2), r);       // q^-_{+1/2} (Eq. 64)
+  r = fma(cpl, fma(-0.5, s0, a2), r);      // q^+_{-1/2} (Eq. 65)
+  r = fma(cml, fma(0.5, sm, a1), r);       // q^-_{-1/2} (Eq. 66)
   return r;
 }
 
-// face coefficients of one direction from the four state velocities (Eq. 62; dtau/dr folded in, see flux_dir2)
+// face coefficients of one direction from the four state velocities (Eq. 62; w = dtau/dr)
 __device__ __forceinline__ void face_coefficients(double vm_lo, double vp_lo, double vm_hi, double vp_hi, double w, double& cph, double& cmh,
                                                   double& cpl, double& cml) {
   const double a_lo = fmax(fabs(vm_lo), fabs(vp_lo)), a_hi = fmax(fabs(vm_hi), fabs(vp_hi));
@@ -94,11 +112,96 @@ __device__ __forceinline__ void face_coefficients(double vm_lo, double vp_lo, do
   cpl = hw * (vp_lo - a_lo); cml = hw * (vm_lo + a_lo);
 }
 
+// ------------------------------------------------------------------------------------------------ relaxation sources
+// dtau * (S + G) for pi^{mu nu} (10) and Pi (B.10-B.12, Eqs. 39-46), one component at a time: emit(slot, dtau*J).
+// pi(s) returns the cell's pi component s (kept in shared memory, not in registers).  The terms of Eq. 42 are regrouped:
+//   dtau J^{mn} = c_pi pi^{mn} + c_S sigma^{mn} - (u'^n A'^m + u'^m A'^n) - sum_l (pi^{ml} Y^{ln} + pi^{nl} Y^{lm}) + k3 g^{mn} - w G^{mn}
+// with w = dtau/u^tau, u' = w u, A'^m = pi^{lm} Du_l + (tau_pipi pi:sigma / 6) u^m  (I_1 and the u u part of I_4's projector),
+// Y^{ln} = w g_ll (0.5 tau_pipi sigma^{ln} - s_omega W^{ln})  (I_4 and -I_3 share the contraction with pi), k3 = w tau_pipi pi:sigma / 3,
+// c_pi = dtau (div v - (1/tau_pi + delta_pipi theta)/u^tau), c_S = w (2 eta/tau_pi + lambda_piPi Pi).
+template <int EOS, class PiGet, class Emit>
+__device__ __forceinline__ void dissipative_sources3(const DevParams& P, double t, const double u[4], const Kin& K, PiGet pi, double Pi, double e,
+                                                     double divv, double dt, Emit emit) {
+  const double t2 = t * t, it = rcp_fast(t), it2 = it * it;
+  // transport coefficients (Eqs. 10-16; R14)
+  double p, cs2;
+  eos_p_cs2<EOS>(P, e, p, cs2);
+  const double T = sqrt_fast(sqrt_fast(e * P.eos_a_inv));
+  const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
+  const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
+  double zs = 0.0;
+  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp(-d * d); }
+  else if (P.zeta_model == 2) zs = P.zeta_amp;
+  const double b = (1.0 / 3.0) - cs2;
+  double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi * rcp_fast(zs) : CUDART_INF;
+  itP = fmin(itP, P.relax_clamp);
+  const double zotP = (zs > 0.0) ? zs * ((e + p) * rcp_fast(T)) * itP : 0.0;
+  const double lPp = P.lambda_Pipi_coef * b;
+  const double iut = rcp_fast(u[0]);
+  const double w = dt * iut;
+  const double* S = K.sig;
+
+  // pi^{mu nu} sigma_{mu nu}: symmetric double contraction with the metric weights of g = diag(1,-1,-1,-t2)
+  const double pisig = pi(0) * S[0] - 2.0 * (pi(1) * S[1] + pi(2) * S[2]) + pi(4) * S[4] + 2.0 * pi(5) * S[5] + pi(7) * S[7] +
+                       t2 * (2.0 * (pi(6) * S[6] + pi(8) * S[8] - pi(3) * S[3]) + t2 * pi(9) * S[9]);
+  const double beta = P.tau_pipi * pisig * (1.0 / 6.0);
+  const double k3 = 2.0 * w * beta;
+  double Ap[4], up[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    Ap[m] = fma(beta, u[m], pi(sym(0, m)) * K.Du[0] + pi(sym(1, m)) * K.Du[1] + pi(sym(2, m)) * K.Du[2] + pi(sym(3, m)) * K.Du[3]);
+    up[m] = w * u[m];
+  }
+  // Y^{ln} = w g_ll (0.5 tau_pipi sigma^{ln} - s_omega W^{ln})
+  double Y[4][4];
+  {
+    const double gl[4] = {w, -w, -w, -w * t2};
+    const double Wm[4][4] = {{0.0, K.W[0], K.W[1], K.W[2]}, {-K.W[0], 0.0, K.W[3], K.W[4]}, {-K.W[1], -K.W[3], 0.0, K.W[5]}, {-K.W[2], -K.W[4], -K.W[5], 0.0}};
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      const double a = -kVorticitySign * gl[l], bb = 0.5 * P.tau_pipi * gl[l];
+#pragma unroll
+      for (int n = 0; n < 4; ++n) Y[l][n] = (l == n) ? bb * S[sym(l, n)] : fma(a, Wm[l][n], bb * S[sym(l, n)]);
+    }
+  }
+  const double cpi = dt * fma(-iut, fma(P.delta_pipi, K.theta, itp), divv);
+  const double cS = w * fma(P.lambda_piPi, Pi, eotp2);
+  const double gi[4] = {1.0, -1.0, -1.0, -it2};
+  const double g1 = w * t * u[3], g2 = w * u[0] * it, g3 = w * u[3] * it;      // Christoffel weights of G_pi (:300; R1, R2)
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = m; n < 4; ++n) {
+      const int s = sym(m, n);
+      double J = cpi * pi(s);
+      J = fma(cS, S[s], J);
+      J = fma(-up[n], Ap[m], J);
+      J = fma(-up[m], Ap[n], J);
+#pragma unroll
+      for (int l = 0; l < 4; ++l) {
+        J = fma(-pi(sym(m, l)), Y[l][n], J);
+        J = fma(-pi(sym(n, l)), Y[l][m], J);
+      }
+      if (m == n) J = fma(k3, gi[m], J);
+      // G_pi = u^a Gamma^mu_{ab} pi^{b nu} + (mu<->nu)
+      if (s == 0) J = fma(-2.0 * g1, pi(3), J);
+      if (s == 1) J = fma(-g1, pi(6), J);
+      if (s == 2) J = fma(-g1, pi(8), J);
+      if (s == 3) J = fma(-g1, pi(9), fma(-g2, pi(3), fma(-g3, pi(0), J)));
+      if (s == 6) J = fma(-g2, pi(6), fma(-g3, pi(1), J));
+      if (s == 8) J = fma(-g2, pi(8), fma(-g3, pi(2), J));
+      if (s == 9) J = fma(-2.0 * g2, pi(9), fma(-2.0 * g3, pi(3), J));
+      emit(PTT + s, J);
+    }
+  const double IPi = P.delta_PiPi * Pi * K.theta - lPp * pisig;                                // Eq. 41
+  emit(BPI, dt * fma(-fma(zotP, K.theta, fma(Pi, itP, IPi)), iut, Pi * divv));                  // B.10
+}
+
 // ------------------------------------------------------------------------------------------------ the kernel
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
 __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     stage_tile_kernel(const __grid_constant__ DevParams P, const __grid_constant__ TileArgs A, const __grid_constant__ CUtensorMap mapA,
-                      const __grid_constant__ CUtensorMap mapZ) {
+                      const __grid_constant__ CUtensorMap mapZ, const __grid_constant__ CUtensorMap mapC) {
   using T = Tile<TWO_D>;
   constexpr int TX = T::TX, TY = T::TY, TZ = T::TZ, NT = T::NT, AX = T::AX, AY = T::AY, NSTAGE = T::NSTAGE;
   constexpr int NF = VISC ? NQ : 4;
@@ -107,8 +210,10 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double* ring = reinterpret_cast<double*>(smem_raw);                       // [NSTAGE][SLOT]
-  double* park = ring + NSTAGE * T::SLOT;                                   // [NF][NT]
-  uint64_t* full = reinterpret_cast<uint64_t*>(park + NF * NT);             // [NSTAGE]
+  double* park = ring + NSTAGE * T::SLOT;                                   // [NF][NT]   running values
+  double* cen = park + NF * NT;                                             // [NCEN][NT] the cell's own pi^{mu nu}, Pi (VISC)
+  uint64_t* full = reinterpret_cast<uint64_t*>(cen + (VISC ? T::NCEN * NT : 0));   // [NSTAGE] ring slots, [NSTAGE] = centre rows
+  unsigned* used = reinterpret_cast<unsigned*>(full + NSTAGE + 1);          // [NSTAGE] warps done with the slot (monotonic)
 
   const int tid = threadIdx.x;
   const int tx = tid % TX, ty = (tid / TX) % TY, tz = tid / (TX * TY);
@@ -121,7 +226,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   const long long c = (long long)b * P.bstride + (long long)(k + P.zoff) * P.plane + (long long)(j + 2) * P.NXp + (i + 2);
   const long long fs = P.fstride;
 
-  // ---- producer: thread 0 issues the loads of stream position s into slot s % NSTAGE
+  // ---- producer side: the loads of stream position s go into slot s % NSTAGE
   auto issue = [&](int s) {
     const int arr = (s < 4) ? A.a_u + s : ((s == 4) ? A.a_p : A.a_q + (s - 5));
     uint64_t* bar = &full[s % NSTAGE];
@@ -130,28 +235,39 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     // padded coordinates: physical cell (i0, j0, k0) sits at (i0+2, j0+2, k0+zoff); box A starts two cells before it in x, y
     tma_load_5d(dst, &mapA, bar, i0, j0, TWO_D ? 0 : k0 + 2, b, arr);
     if (!TWO_D) {
-      tma_load_5d(dst + T::A_SIZE, &mapZ, bar, i0 + 2, j0 + 2, k0, b, arr);                     // planes k0-2, k0-1
+      tma_load_5d(dst + T::A_SIZE, &mapZ, bar, i0 + 2, j0 + 2, k0, b, arr);                       // planes k0-2, k0-1
       tma_load_5d(dst + T::A_SIZE + T::Z_SIZE, &mapZ, bar, i0 + 2, j0 + 2, k0 + 2 + TZ, b, arr);  // planes k0+TZ, k0+TZ+1
     }
   };
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < NSTAGE; ++s) mbar_init(&full[s], 1);
+    for (int s = 0; s <= NSTAGE; ++s) mbar_init(&full[s], 1);
+#pragma unroll
+    for (int s = 0; s < NSTAGE; ++s) used[s] = 0u;
     fence_mbar_init();
   }
   __syncthreads();
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < NSTAGE; ++s) issue(s);
+    if (VISC) {      // the tile's own pi^{mu nu}, Pi: boxes of TX x TY x TZ land in thread order
+      mbar_arrive_expect_tx(&full[NSTAGE], (unsigned)(T::NCEN * NT * sizeof(double)));
+#pragma unroll 1
+      for (int n = 0; n < T::NCEN; ++n) tma_load_5d(cen + n * NT, &mapC, &full[NSTAGE], i0 + 2, j0 + 2, TWO_D ? 0 : k0 + 2, b, A.a_q + PTT + n);
+    }
   }
-  // consumer side of the ring: wait for stream position s; after the reads, release() lets thread 0 refill the slot
+  // ---- consumer side: wait for stream position s; after the warp's reads, release(s) counts the warp out of the slot and the
+  // warp that completes the count refills it (nobody waits for anybody here)
   auto acquire = [&](int s) -> const double* {
     mbar_wait(&full[s % NSTAGE], (unsigned)((s / NSTAGE) & 1));
     return ring + (s % NSTAGE) * T::SLOT;
   };
   auto release = [&](int s) {
-    __syncthreads();
-    if (tid == 0 && s + NSTAGE < NSTREAM) issue(s + NSTAGE);
+    __syncwarp();
+    if ((tid & 31) == 0) {
+      const unsigned old = slot_counter_add(&used[s % NSTAGE]);
+      if ((old + 1u) % (unsigned)T::NW == 0u && s + NSTAGE < NSTREAM) issue(s + NSTAGE);
+    }
   };
 
   // ---- per-thread offsets into a slot: centre in box A, and the four eta neighbours (box A, or the halo boxes at the tile faces)
@@ -172,14 +288,35 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   const double it = MILNE ? rcp_fast(t) : 1.0;
   const double it2 = it * it;
   const double dt = P.dtau;
+  const double wt = MILNE ? dt * it : 0.0;               // dtau/tau: weight of the geometric sources G_c (:1013)
   const double hinv[3] = {0.5 * P.inv_dx, 0.5 * P.inv_dy, 0.5 * P.inv_dz};
   const double wd[3] = {dt * hinv[0], dt * hinv[1], dt * hinv[2]};
   constexpr int ND = TWO_D ? 2 : 3;
   unsigned long long nfail = 0, nnonf = 0;
   double minfac = 1.0;
 
+  // centre-only operands: plain coalesced loads issued before the stream is consumed
+  const double ec = A.e_in[c];
+  double upv[4] = {0.0, 0.0, 0.0, 0.0};
+  if (VISC) {
+#pragma unroll
+    for (int n = 0; n < 4; ++n) upv[n] = A.u_prev[n * fs + c];
+  }
+  {      // pull what phases 3 and 4 read directly (state velocities, q^n) towards L2 while the stream runs
+    const long long sd[3] = {1, (long long)P.NXp, P.plane};
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+      prefetch_l2(A.vL + d * fs + c); prefetch_l2(A.vR + d * fs + c);
+      if (d > 0) { prefetch_l2(A.vL + d * fs + c + sd[d]); prefetch_l2(A.vR + d * fs + c - sd[d]); }
+    }
+    if (STAGE == 2) {
+#pragma unroll
+      for (int n = 0; n < NF; ++n) prefetch_l2(A.q_n + n * fs + c);
+    }
+  }
+
   // ================================================================= phase 1: u^mu and p (velocity gradients, v^i, p terms)
-  double uc[4], du[4][4], vm[3], vp[3], acc[4] = {0.0, 0.0, 0.0, 0.0}, divv = 0.0, pc;
+  double uc[4], du[4][4], vm[3], vp[3], acc[4] = {0.0, 0.0, 0.0, 0.0}, divv = 0.0, gPi = 0.0;
   {
     double rm[3], rp[3];      // 1/u^tau at the six neighbours
 #pragma unroll
@@ -204,7 +341,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       }
     }
     const double* s = acquire(4) + oc;
-    pc = s[0];
+    const double pc = s[0];
     const double xm = s[-1], xp = s[1], ym = s[-AX], yp = s[AX];
     double zm = 0.0, zp = 0.0;
     if (!TWO_D) { const double* sb = s - oc; zm = sb[ozm1]; zp = sb[ozp1]; }
@@ -218,31 +355,25 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       acc[0] = fma(wd[2], fma(vm[2], zm, -vp[2] * zp), acc[0]);
       acc[3] = wd[2] * it2 * (zm - zp);
     }
+    if (MILNE) {
+      // G_c^tau = -(T^{tau tau} + tau^2 T^{eta eta})/tau with T^{eta eta} = (e + P)(u^eta)^2 + P/tau^2 + pi^{eta eta}, P = p + Pi (Eq. 34):
+      // the e, p part here; the Pi, pi^{eta eta} and T^{tau mu} parts are added when those fields stream through
+      const double g = t2 * uc[3] * uc[3];
+      acc[0] = fma(-wt, fma(ec + pc, g, pc), acc[0]);
+      gPi = wt * (g + 1.0);
+    }
   }
 
-  // ================================================================= phase 2: per-cell sources (G_c, S_pi + G_pi, S_Pi)
-  {
-    const double ec = A.e_in[c];
-    if (MILNE) {     // G_c (:1013), T^{eta eta} from Eq. 34
-      const double Ptc = pc + (VISC ? A.q_in[BPI * fs + c] : 0.0);
-      const double Tnn = fma((ec + Ptc) * uc[3], uc[3], fma(Ptc, it2, VISC ? A.q_in[PNN * fs + c] : 0.0));
-      const double wt = dt * it;
-      acc[0] = fma(-wt, fma(t2, Tnn, A.q_in[TTT * fs + c]), acc[0]);
-      acc[1] = fma(-wt, A.q_in[TTX * fs + c], acc[1]);
-      acc[2] = fma(-wt, A.q_in[TTY * fs + c], acc[2]);
-      acc[3] = fma(-3.0 * wt, A.q_in[TTN * fs + c], acc[3]);
-    }
-    if (VISC) {
+  // ================================================================= phase 2: relaxation sources (S_pi + G_pi, S_Pi) -> park
+  if (VISC) {
 #pragma unroll
-      for (int n = 0; n < 4; ++n) du[0][n] = (uc[n] - A.u_prev[n * fs + c]) * P.inv_dtau;      // backward difference in time (:424)
-      Kin K;
-      kinematics(uc, du[0], du[1], du[2], du[3], t, K);
-      double pi[10];
-#pragma unroll
-      for (int n = 0; n < 10; ++n) pi[n] = A.q_in[(PTT + n) * fs + c];
-      const double Pi = A.q_in[BPI * fs + c];
-      dissipative_sources2<EOS>(P, t, uc, K, pi, Pi, ec, divv, [&](int slot, double J) { park[slot * NT + tid] = dt * J; });
-    }
+    for (int n = 0; n < 4; ++n) du[0][n] = (uc[n] - upv[n]) * P.inv_dtau;      // backward difference in time (:424)
+    Kin K;
+    kinematics(uc, du[0], du[1], du[2], du[3], t, K);
+    mbar_wait(&full[NSTAGE], 0u);
+    const double* mine = cen + tid;
+    dissipative_sources3<EOS>(P, t, uc, K, [&](int s) { return mine[s * NT]; }, mine[10 * NT], ec, divv, dt,
+                              [&](int slot, double J) { park[slot * NT + tid] = J; });
   }
 
   // ================================================================= phase 3: the q fields (flux divergence + conservation sources)
@@ -262,8 +393,9 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
         }
       }
     }
-    const double ht = 0.5 * P.theta;
+    const double theta = P.theta;
     const bool fx = P.nx > 1, fy = P.ny > 1, fz = !TWO_D;
+    const double wt2 = wt * t2;
 #pragma unroll 1
     for (int n = 0; n < NF; ++n) {
       const double* sb = acquire(5 + n);
@@ -276,9 +408,10 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       release(5 + n);
       double r = a2;
       if (VISC && n >= PTT) r += park[n * NT + tid];
-      if (fx) r = flux_line<THETA1>(x0, x1, a2, x3, x4, cf[0][0], cf[0][1], cf[0][2], cf[0][3], ht, r);
-      if (fy) r = flux_line<THETA1>(y0, y1, a2, y3, y4, cf[1][0], cf[1][1], cf[1][2], cf[1][3], ht, r);
-      if (fz) r = flux_line<THETA1>(z0, z1, a2, z3, z4, cf[2][0], cf[2][1], cf[2][2], cf[2][3], ht, r);
+      if (MILNE && n < 4) r = fma((n == 3) ? -3.0 * wt : -wt, a2, r);      // G_c (:1013): -T^{tau mu}/tau, -3 T^{tau eta}/tau
+      if (fx) r = flux_line<THETA1>(x0, x1, a2, x3, x4, cf[0][0], cf[0][1], cf[0][2], cf[0][3], theta, r);
+      if (fy) r = flux_line<THETA1>(y0, y1, a2, y3, y4, cf[1][0], cf[1][1], cf[1][2], cf[1][3], theta, r);
+      if (fz) r = flux_line<THETA1>(z0, z1, a2, z3, z4, cf[2][0], cf[2][1], cf[2][2], cf[2][3], theta, r);
       park[n * NT + tid] = r;
       if (VISC && n >= PTT) {
         // this field's part of A^{i nu} = P (v^i delta^nu_tau - g^{i nu}) - v^i pi^{tau nu} + pi^{i nu}, differenced (B.2-B.5)
@@ -287,7 +420,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
           double vt = wd[0] * fma(vp[0], x3, -vm[0] * x1);
           vt = fma(wd[1], fma(vp[1], y3, -vm[1] * y1), vt);
           if (!TWO_D) vt = fma(wd[2], fma(vp[2], z3, -vm[2] * z1), vt);
-          if (n == BPI) { acc[0] -= vt; acc[1] += gx; acc[2] += gy; acc[3] = fma(gz, it2, acc[3]); }
+          if (n == BPI) { acc[0] = fma(-gPi, a2, acc[0] - vt); acc[1] += gx; acc[2] += gy; acc[3] = fma(gz, it2, acc[3]); }
           else if (n == PTT) acc[0] += vt;
           else if (n == PTX) { acc[1] += vt; acc[0] += gx; }
           else if (n == PTY) { acc[2] += vt; acc[0] += gy; }
@@ -297,7 +430,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
         else if (n == PXN) { acc[3] += gx; acc[1] += gz; }
         else if (n == PYY) acc[2] += gy;
         else if (n == PYN) { acc[3] += gy; acc[2] += gz; }
-        else acc[3] += gz;       // PNN
+        else { acc[3] += gz; acc[0] = fma(-wt2, a2, acc[0]); }       // PNN (with its part of tau^2 T^{eta eta} in G_c^tau)
       }
     }
   }
@@ -315,16 +448,16 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     }
     qv[n] = v;
   }
-  // Post: Eqs. 52-54, 72 then 73-74 (R8: regulate after the inversion)
+  // Post: Eqs. 52-54, 72 then 73-74 (R8: regulate after the inversion).  Threads outside the grid (ragged tiles) carry a
+  // benign state so that the warp-voted Newton loop is not held up by them.
   const double tp = A.t_post;
   const double tp2 = MILNE ? tp * tp : 1.0;
-  // threads outside the grid (ragged tiles) carry a benign state so that the warp-voted Newton loop is not held up by them
   const double E = valid ? qv[TTT] - qv[PTT] : 1.0;
   const double Mx = valid ? qv[TTX] - qv[PTX] : 0.0, My = valid ? qv[TTY] - qv[PTY] : 0.0, Mn = valid ? qv[TTN] - qv[PTN] : 0.0;
   const double Pi = valid ? qv[BPI] : 0.0;
   const double M2 = Mx * Mx + My * My + tp2 * Mn * Mn;
   bool fail;
-  const double e = newton_single<EOS>(P, E, M2, Pi, A.e_in[c], fail);
+  const double e = newton_single<EOS>(P, E, M2, Pi, ec, fail);
   if (fail) ++nfail;
   const double p0 = eos_p<EOS>(P, e);
   const double Pt = p0 + Pi;

@@ -143,3 +143,25 @@ __device__ __forceinline__ double clip_velocity(double v) {
 }
 
 }  // namespace vh
+
+namespace vh {
+
+// minmod(d1, d2) of Eqs. 67-68 for theta = 1 (the centred difference lies between the one-sided ones and drops out):
+// the argument of smaller magnitude when both have the same sign, else 0 (R10).  One DSETP, the rest on the ALU pipe;
+// the factor 1/2 of the half-cell extrapolation is folded into the caller's FMA.
+__device__ __forceinline__ double minmod2(double d1, double d2) {
+  const double t = (fabs(d1) < fabs(d2)) ? d1 : d2;
+  const bool opposite = (__double2hiint(d1) ^ __double2hiint(d2)) < 0;
+  return opposite ? 0.0 : t;
+}
+// general theta: minmod(theta d1, (d1 + d2)/2, theta d2); `theta` in [1, 2]
+__device__ __forceinline__ double minmod3(double d1, double d2, double theta) {
+  const double t = theta * minmod2(d1, d2);
+  const double c = 0.5 * (d1 + d2);
+  return (fabs(c) < fabs(t)) ? c : t;       // t = 0 (opposite signs) always wins
+}
+template <bool THETA1> __device__ __forceinline__ double minmod_slope(double d1, double d2, double theta) {
+  return THETA1 ? minmod2(d1, d2) : minmod3(d1, d2, theta);
+}
+
+}  // namespace vh
