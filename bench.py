@@ -29,6 +29,9 @@ METRIC = "cell-updates/s (full RK2 KT step, FP64) at 128^3 viscous"
 UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_UPDATE = 856.0      # 107 doubles per cell-update, each state array read/written once per stage
 ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the stage kernel at 128^3 from the committed ncu --set full
+# capture (profiles/r01_ncu_summary.md); None for launches that were not captured
+NCU_TRAFFIC_BYTES = {"stage1": None, "stage2": None}
 
 
 def workload(rank=0):
@@ -208,7 +211,7 @@ def main():
     st = s.status()
 
     # ---------------- per-kernel durations (CUDA events around each launch on the launching stream)
-    prof = s.step_profile(min(K, 10))       # launch order: velocity 1, stage 1, velocity 2, stage 2 (variants 0, 2)
+    prof = s.step_profile(min(K, 10))       # keyed by kernel: velocity1, stage1, velocity2, stage2 (variant 1: stage1, ghost1, stage2, ghost2)
 
     # ---------------- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
@@ -250,10 +253,17 @@ def main():
             except Exception:
                 pass
         flops_cu, plain_cu, mix = algorithmic_flops(prm, init)
-        # dominant kernel: the stage kernels (stage 2 is the longer of the two: it also reads q^n)
-        dom = "stage2" if prof["stage2"] >= prof["stage1"] else "stage1"
+        flops_inv_cu = mix.pop("flops_interface_inversions")
+        # Kernel shares of the algorithmic work: the velocity kernel does the interface-state inversions
+        # (Eq. 72 at every reconstructed state), the stage kernel everything else; one stage = half of a cell-update.
+        variant1 = (args.variant == 1)
+        stage_keys = ("stage1", "stage2")
+        dom = max(stage_keys, key=lambda k: prof[k])            # dominant kernel: the longer of the two stage-kernel launches
         dur = prof[dom] * 1e-3
-        flops_launch = 0.5 * flops_cu * ncell                  # one stage = half of a cell-update's arithmetic
+        flops_stage = 0.5 * (flops_cu if variant1 else flops_cu - flops_inv_cu)
+        flops_launch = flops_stage * ncell
+        # algorithmic bytes of the stage kernel: the state arrays of SURVEY 8(d) (each read / written once per stage) plus,
+        # in the split pipeline, the six state velocities it reads back (they are a by-product, not state: not counted)
         bytes_launch = ALG_BYTES_STAGE[dom] * ncell
         t_alu = flops_launch / (fp64_gflops * 1e9)
         t_hbm = bytes_launch / (hbm_peak * 1e9)
@@ -262,15 +272,19 @@ def main():
         else:
             roof = {"bound": "hbm", "achieved": bytes_launch / dur / 1e9, "peak": hbm_peak, "unit": "GB/s"}
         roof["frac"] = roof["achieved"] / roof["peak"]
+        step_roof_s = max(flops_cu * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9))
         roof.update({
-            "traffic": None, "kernel": "stage_kernel (%s)" % dom, "launch_ms": prof[dom],
+            "traffic": NCU_TRAFFIC_BYTES.get(dom), "kernel": "stage_tile_kernel (%s)" % dom if not variant1 else "stage_cell_kernel (%s)" % dom,
+            "launch_ms": prof[dom],
             "peak_source": "FP64 FMA microbenchmark, same run (vh_measure_peaks)" if roof["bound"] == "alu" else hbm_src,
-            "alg_flops_per_cell_update": flops_cu, "alg_bytes_per_cell_update": ALG_BYTES_PER_CELL_UPDATE,
+            "alg_flops_per_cell_update": flops_cu, "alg_flops_interface_inversions_per_cell_update": flops_inv_cu,
+            "alg_flops_this_kernel_per_cell": flops_stage, "alg_bytes_per_cell_update": ALG_BYTES_PER_CELL_UPDATE,
+            "alg_bytes_this_kernel_per_cell": ALG_BYTES_STAGE[dom],
+            "flop_weights": "add/mul/cmp 1, div 10, sqrt 15, exp 25, pow 30, tanh 40 (SURVEY 8(d)); counted on the oracle, each interface once",
             "op_mix_per_cell_update": {k: round(v, 1) for k, v in mix.items()},
             "hbm_view": {"achieved_gbs": bytes_launch / dur / 1e9, "peak_gbs": hbm_peak, "peak_source": hbm_src, "frac": bytes_launch / dur / 1e9 / hbm_peak,
                          "copy_gbs_same_run": copy_gbs},
-            "step_roofline_ms": max(flops_cu * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9)) * 1e3,
-            "step_frac": max(flops_cu * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9)) / (ms / K * 1e-3),
+            "step_roofline_ms": step_roof_s * 1e3, "step_frac": step_roof_s / (ms / K * 1e-3),
             "per_kernel_ms": prof,
         })
         line = {

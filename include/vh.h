@@ -82,7 +82,8 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
 /* Advance n_steps full RK2 steps (program-flow steps 1-9, :503-529).  Asynchronous on the handle's stream.             */
 int vh_step(vh_handle* h, int n_steps);
 
-/* Same as vh_step, but brackets each of the four launches of a step (stage 1, ghost 1, stage 2, ghost 2) with CUDA events
+/* Same as vh_step, but brackets each of the four launches of a step (default pipeline: velocity kernel 1, stage kernel 1,
+ * velocity kernel 2, stage kernel 2; kernel variant 1: stage 1, ghost 1, stage 2, ghost 2) with CUDA events
  * on the handle's stream and returns their mean durations in milliseconds in ms4[0..3] (for per-kernel roofline numbers;
  * synchronises once per step, so use vh_step for throughput).                                                            */
 int vh_step_profile(vh_handle* h, int n_steps, double* ms4);

@@ -284,8 +284,10 @@ template <class R> class Solver {
       qp[n] = I[n][c + 1] - (dr / R(2)) * sn;     // q^+: Eq. 63 / 65
     }
     R vm[3], vp[3];
+    VHO_COUNTING_SECTION(2);
     state_velocity(qm, t, eI[c], count, vm);      // guess: e of the cell the state was extrapolated from (R6)
     state_velocity(qp, t, eI[c + 1], count, vp);
+    VHO_COUNTING_SECTION(1);
     R a = maxr(absr(vp[r]), absr(vm[r]));         // Eq. 62 with rho = |v_r| (:388)
     for (int n = 0; n < NQ; ++n) H[n] = (vp[r] * qp[n] + vm[r] * qm[n]) / R(2) - a * (qp[n] - qm[n]) / R(2);   // Eq. 61
   }

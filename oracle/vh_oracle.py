@@ -209,26 +209,28 @@ OP_WEIGHTS = dict(add=1, mul=1, div=10, cmp=1, sqrt=15, exp=25, pow=30, tanh=40)
 
 def count_ops(params: dict, e, u4, pi10=None, Pi=None, warm=1, n=1):
     """Operation counts of n RK2 steps with the counting scalar (after `warm` uncounted steps).
-    Returns dict(other={class: count}, flux={class: count}) summed over all cells."""
+    Returns dict(other=..., flux=..., invert=...) of {class: count} summed over all cells: `flux` is the reconstruction and
+    Eq. 61 inside flux(), `invert` the interface-state inversions inside flux() (both evaluated twice per interface)."""
     P = make_params(params)
     shape = (P.n_batch, P.nz, P.ny, P.nx)
     e = np.ascontiguousarray(e, dtype=np.float64).reshape(shape)
     u4 = np.ascontiguousarray(u4, dtype=np.float64).reshape((4,) + shape)
     pi10 = None if pi10 is None else np.ascontiguousarray(pi10, dtype=np.float64).reshape((10,) + shape)
     Pi = None if Pi is None else np.ascontiguousarray(Pi, dtype=np.float64).reshape(shape)
-    out = (C.c_longlong * 16)()
+    out = (C.c_longlong * 24)()
     rc = lib().vho_count_ops(C.byref(P), _dp(e), _dp(u4), _dp(pi10), _dp(Pi), int(warm), int(n), out)
     if rc < 0:
         raise ValueError("vho_count_ops needs n_batch == 1")
     vals = list(out)
-    return dict(other=dict(zip(OP_CLASSES, vals[:8])), flux=dict(zip(OP_CLASSES, vals[8:])))
+    return dict(other=dict(zip(OP_CLASSES, vals[:8])), flux=dict(zip(OP_CLASSES, vals[8:16])), invert=dict(zip(OP_CLASSES, vals[16:24])))
 
 
 def algorithmic_flops_per_cell_update(params: dict, e, u4, pi10=None, Pi=None):
     """Weighted flops per cell per RK2 step with every interface charged once (flux section / 2), and the raw counts."""
     c = count_ops(params, e, u4, pi10, Pi, warm=1, n=1)
     ncell = params["nx"] * params["ny"] * params["nz"]
-    per = {k: (c["other"][k] + 0.5 * c["flux"][k]) / ncell for k in OP_CLASSES}
+    per = {k: (c["other"][k] + 0.5 * c["flux"][k] + 0.5 * c["invert"][k]) / ncell for k in OP_CLASSES}
     flops = sum(OP_WEIGHTS[k] * per[k] for k in OP_CLASSES)
     plain = per["add"] + per["mul"] + per["div"] + per["sqrt"] + per["cmp"]
+    per["flops_interface_inversions"] = sum(OP_WEIGHTS[k] * 0.5 * c["invert"][k] / ncell for k in OP_CLASSES)
     return flops, plain, per

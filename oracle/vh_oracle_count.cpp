@@ -8,8 +8,8 @@
 
 namespace vho_cnt {
 enum { ADD = 0, MUL, DIV, CMP, SQRT, EXP, POW, TANH, NCLASS };
-static long long g_counts[2][NCLASS];
-static int g_section = 0;     // 0: everything else, 1: inside flux()
+static long long g_counts[3][NCLASS];
+static int g_section = 0;     // 0: everything else, 1: inside flux() (reconstruction + Eq. 61), 2: the interface-state inversions inside flux()
 static bool g_on = false;
 inline void tick(int cls, bool live) { if (g_on && live) ++g_counts[g_section][cls]; }
 
@@ -46,7 +46,7 @@ namespace vho { using vho_cnt::sqrt; using vho_cnt::exp; using vho_cnt::tanh; us
 
 extern "C" {
 // Runs `warm` uncounted steps (so that no array holds constant-flagged data), then counts `n` steps.
-// counts: [2][8] = {other, flux} x {add, mul, div, cmp, sqrt, exp, pow, tanh}; totals over all cells and steps.
+// counts: [3][8] = {other, flux, interface inversions} x {add, mul, div, cmp, sqrt, exp, pow, tanh}; totals over all cells and steps.
 int vho_count_ops(const vho::Params* P, const double* e, const double* u4, const double* pi10, const double* Pi, int warm, int n,
                   long long* counts) {
   if (P->n_batch != 1) return -1;

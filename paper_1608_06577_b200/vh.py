@@ -111,6 +111,7 @@ class Solver:
             self.h = None
             raise VHError("vh_create failed (%d): %s" % (rc, msg.decode() if msg else "?"))
         self.shape = (self.P.n_batch, self.P.nz, self.P.ny, self.P.nx)
+        self.variant = 0
 
     def close(self):
         if getattr(self, "h", None):
@@ -172,10 +173,12 @@ class Solver:
         self._check(self.L.vh_step(self.h, int(n)), "vh_step")
 
     def step_profile(self, n=1):
-        """n steps with CUDA events around each launch; mean ms of (stage 1, ghost 1, stage 2, ghost 2)."""
+        """n steps with CUDA events around each of the four launches of a step; mean ms per launch, keyed by kernel:
+        variants 0, 2: velocity1, stage1, velocity2, stage2; variant 1: stage1, ghost1, stage2, ghost2."""
         ms = (C.c_double * 4)()
         self._check(self.L.vh_step_profile(self.h, int(n), ms), "vh_step_profile")
-        return dict(zip(("stage1", "ghost1", "stage2", "ghost2"), list(ms)))
+        names = ("stage1", "ghost1", "stage2", "ghost2") if self.variant == 1 else ("velocity1", "stage1", "velocity2", "stage2")
+        return dict(zip(names, list(ms)))
 
     def get_fields(self, device=None, with_uprev=False, out=None):
         """Returns dict(q [15,...], e, p, u [4,...]) as tensors on `device` ('cpu' -> host buffers, mem_space 0)."""
@@ -205,6 +208,7 @@ class Solver:
 
     def set_kernel_variant(self, v):
         self._check(self.L.vh_set_kernel_variant(self.h, int(v)), "vh_set_kernel_variant")
+        self.variant = int(v)
 
 
 def measure_peaks(n_bytes=1 << 30, repeats=10, stream=None):
