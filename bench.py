@@ -39,6 +39,22 @@ def workload(rank=0):
     return prm, init
 
 
+def max_over_ranks(x, dist, device):
+    """Timing of a multi-rank run = the slowest rank (the only collective of the replica mode; none on the data path)."""
+    if dist is None:
+        return float(x)
+    import torch
+
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(ncell_per_rank, steps, world, seconds):
+    """Whole-job throughput of `world` independent replicas: all ranks' cell-updates / max-over-ranks time."""
+    return ncell_per_rank * steps * world / seconds
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = "index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
@@ -203,11 +219,8 @@ def main():
     launches = s.launch_count() - n0
     clocks = sampler.stop()
     ms = ev0.elapsed_time(ev1)
-    if dist is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = ncell * K * world / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, dev)
+    value = aggregate_value(ncell, K, world, ms * 1e-3)
     st = s.status()
 
     # ---------------- per-kernel durations (CUDA events around each launch on the launching stream)
@@ -234,11 +247,8 @@ def main():
         s.get_fields(out=out)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_value = ncell * E * world / e2e_s
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
+    e2e_value = aggregate_value(ncell, E, world, e2e_s)
 
     # ---------------- peaks measured in the same run by the library's own microbenchmarks
     copy_gbs, fp64_gflops = vh.measure_peaks(n_bytes=1 << 30, repeats=10)
