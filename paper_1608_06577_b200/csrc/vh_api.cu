@@ -1,6 +1,5 @@
 // vh_api.cu -- C ABI (include/vh.h): handle, buffers, buffer rotation (PAPER.md program-flow steps 7, 9), kernel dispatch.
-#include "../../include/vh.h"
-#include "vh_kernels3.cuh"
+#include "vh_internal.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -12,34 +11,7 @@
 
 using namespace vh;
 
-#ifndef VH_STAGE_MINB
-#define VH_STAGE_MINB 2      // resident blocks per SM the stage kernel is compiled for (register cap 65536/(256*MINB))
-#endif
-
 static thread_local std::string g_err;
-
-struct vh_handle {
-  vh_params prm;
-  DevParams P;
-  cudaStream_t stream = nullptr;
-  double* pool = nullptr;            // 67 padded arrays
-  double* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
-  double* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
-  double* e[2] = {nullptr, nullptr};            // e^n / e^{n+1}, e*
-  double* p[2] = {nullptr, nullptr};
-  double* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
-  double* vR = nullptr;              // [3] ... high face
-  Counters* cnt = nullptr;
-  double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
-  double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
-  long long n_steps = 0;
-  long long launches = 0;
-  bool initialised = false;
-  bool two_d = false;
-  int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
-  CUtensorMap mapA, mapZ, mapC;      // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes, box C: the tile)
-  std::string err;
-};
 
 static int fail(vh_handle* h, int code, const std::string& msg) {
   if (h) h->err = msg;
@@ -107,72 +79,20 @@ static int check_params(const vh_params* p, std::string& why) {
 }
 
 // ------------------------------------------------------------------------------------------------ dispatch
-// VH_DEBUG_SYNC=1 in the environment: synchronise after every launch and name the kernel that faulted.
-static cudaError_t debug_sync(vh_handle* h, const char* what) {
-  cudaError_t e = cudaGetLastError();
-  static const bool on = getenv("VH_DEBUG_SYNC") != nullptr;
-  if (e == cudaSuccess && on) {
-    e = cudaStreamSynchronize(h->stream);
-    if (e != cudaSuccess) fprintf(stderr, "[vh] %s faulted at step %lld: %s\n", what, h->n_steps, cudaGetErrorString(e));
+#define debug_sync vh_debug_sync
+// one Euler stage with the handle's kernel variant: the launch units are compiled per (EOS, viscous, Milne) combination
+static cudaError_t launch_stage_any(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+  const int phys = (h->prm.physics != 0) ? 0 : ((h->prm.geometry == 0) ? 1 : 2);
+  switch (h->prm.eos + 2 * phys) {
+    case 0: return vh_launch_stage_combo0(h, stage, A, mid);
+    case 1: return vh_launch_stage_combo1(h, stage, A, mid);
+    case 2: return vh_launch_stage_combo2(h, stage, A, mid);
+    case 3: return vh_launch_stage_combo3(h, stage, A, mid);
+    case 4: return vh_launch_stage_combo4(h, stage, A, mid);
+    default: return vh_launch_stage_combo5(h, stage, A, mid);
   }
-  return e;
-}
-template <int EOS, bool VISC, bool MILNE, bool TWO_D>
-static cudaError_t launch_stage_t(vh_handle* h, int stage, const StageArgs& A) {
-  const DevParams& P = h->P;
-  dim3 block(32, 8);
-  dim3 grid((P.nx + 31) / 32, (P.ny + 7) / 8, P.nz * P.n_batch);
-  if (stage == 1) stage_cell_kernel<EOS, VISC, MILNE, TWO_D, 1><<<grid, block, 0, h->stream>>>(P, A);
-  else stage_cell_kernel<EOS, VISC, MILNE, TWO_D, 2><<<grid, block, 0, h->stream>>>(P, A);
-  h->launches++;
-  return debug_sync(h, stage == 1 ? "stage 1 kernel" : "stage 2 kernel");
-}
-template <int EOS, bool VISC, bool MILNE>
-static cudaError_t launch_stage_d(vh_handle* h, int stage, const StageArgs& A) {
-  return h->two_d ? launch_stage_t<EOS, VISC, MILNE, true>(h, stage, A) : launch_stage_t<EOS, VISC, MILNE, false>(h, stage, A);
-}
-static cudaError_t launch_stage(vh_handle* h, int stage, const StageArgs& A) {
-  const bool visc = h->prm.physics != 0, milne = h->prm.geometry == 0;
-  const int eos = h->prm.eos;
-  if (visc) return eos ? launch_stage_d<1, true, true>(h, stage, A) : launch_stage_d<0, true, true>(h, stage, A);
-  if (milne) return eos ? launch_stage_d<1, false, true>(h, stage, A) : launch_stage_d<0, false, true>(h, stage, A);
-  return eos ? launch_stage_d<1, false, false>(h, stage, A) : launch_stage_d<0, false, false>(h, stage, A);
 }
 
-// ---- split pipeline (variant 0): velocity kernel + stage kernel (vh_kernels2.cuh)
-template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
-static cudaError_t launch_split_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid) {
-  const DevParams& P = h->P;
-  constexpr int BX = 32, BY = TWO_D ? 8 : 4, BZ = TWO_D ? 1 : 2;
-  dim3 block(BX, BY, BZ);
-  dim3 grid((P.nx + BX - 1) / BX, (P.ny + BY - 1) / BY, ((P.nz + BZ - 1) / BZ) * P.n_batch);
-  VelArgs V{S.q_in, S.e_in, h->vL, h->vR, S.cnt, S.t};
-  velocity_kernel<EOS, VISC, MILNE, TWO_D, THETA1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, V);
-  h->launches++;
-  cudaError_t e = debug_sync(h, "velocity kernel");
-  if (e != cudaSuccess) return e;
-  if (mid) cudaEventRecord(mid, h->stream);
-  Stage2Args A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post};
-  if (stage == 1) stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1, BX, BY, BZ, VH_STAGE_MINB><<<grid, block, 0, h->stream>>>(P, A);
-  else stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2, BX, BY, BZ, VH_STAGE_MINB><<<grid, block, 0, h->stream>>>(P, A);
-  h->launches++;
-  return debug_sync(h, stage == 1 ? "stage 1 kernel" : "stage 2 kernel");
-}
-template <int EOS, bool VISC, bool MILNE>
-static cudaError_t launch_split_d(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
-  const bool th1 = h->prm.minmod_theta == 1.0;
-  if (h->two_d) return th1 ? launch_split_t<EOS, VISC, MILNE, true, true>(h, stage, A, mid) : launch_split_t<EOS, VISC, MILNE, true, false>(h, stage, A, mid);
-  return th1 ? launch_split_t<EOS, VISC, MILNE, false, true>(h, stage, A, mid) : launch_split_t<EOS, VISC, MILNE, false, false>(h, stage, A, mid);
-}
-static cudaError_t launch_split(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
-  const bool visc = h->prm.physics != 0, milne = h->prm.geometry == 0;
-  const int eos = h->prm.eos;
-  if (visc) return eos ? launch_split_d<1, true, true>(h, stage, A, mid) : launch_split_d<0, true, true>(h, stage, A, mid);
-  if (milne) return eos ? launch_split_d<1, false, true>(h, stage, A, mid) : launch_split_d<0, false, true>(h, stage, A, mid);
-  return eos ? launch_split_d<1, false, false>(h, stage, A, mid) : launch_split_d<0, false, false>(h, stage, A, mid);
-}
-
-// ---- tile pipeline (variant 0): velocity kernel + TMA tile kernel (vh_kernels3.cuh)
 // One 5-d tensor map (x, y, eta, event, array) over the whole pool of padded arrays per box shape.  cuTensorMapEncodeTiled is a
 // driver-API entry point; it is looked up through the runtime so that the library needs no link-time dependency on libcuda.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -205,53 +125,6 @@ static int make_tensor_maps(vh_handle* h, int n_arrays) {
   return VH_OK;
 }
 
-template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
-static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
-  using T = Tile<TWO_D>;
-  constexpr size_t smem = tile_smem_bytes<TWO_D, VISC>();
-  auto kern = stage_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE>;
-  static bool configured = false;      // one attribute call per instantiation (single device per process)
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  const DevParams& P = h->P;
-  dim3 grid((P.nx + T::TX - 1) / T::TX, (P.ny + T::TY - 1) / T::TY, ((P.nz + T::TZ - 1) / T::TZ) * P.n_batch);
-  kern<<<grid, T::NT, smem, h->stream>>>(P, A, h->mapA, h->mapZ, h->mapC);
-  h->launches++;
-  return debug_sync(h, STAGE == 1 ? "stage 1 tile kernel" : "stage 2 tile kernel");
-}
-template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
-static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid) {
-  const DevParams& P = h->P;
-  constexpr int BX = 32, BY = TWO_D ? 8 : 4, BZ = TWO_D ? 1 : 2;
-  dim3 block(BX, BY, BZ);
-  dim3 grid((P.nx + BX - 1) / BX, (P.ny + BY - 1) / BY, ((P.nz + BZ - 1) / BZ) * P.n_batch);
-  VelArgs V{S.q_in, S.e_in, h->vL, h->vR, S.cnt, S.t};
-  velocity_kernel<EOS, VISC, MILNE, TWO_D, THETA1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, V);
-  h->launches++;
-  cudaError_t e = debug_sync(h, "velocity kernel");
-  if (e != cudaSuccess) return e;
-  if (mid) cudaEventRecord(mid, h->stream);
-  const long long fs = P.fstride;
-  TileArgs A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post,
-             (int)((S.q_in - h->pool) / fs), (int)((S.u_in - h->pool) / fs), (int)((S.p_in - h->pool) / fs)};
-  return (stage == 1) ? launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1>(h, A) : launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2>(h, A);
-}
-template <int EOS, bool VISC, bool MILNE>
-static cudaError_t launch_tile_d(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
-  const bool th1 = h->prm.minmod_theta == 1.0;
-  if (h->two_d) return th1 ? launch_tile_t<EOS, VISC, MILNE, true, true>(h, stage, A, mid) : launch_tile_t<EOS, VISC, MILNE, true, false>(h, stage, A, mid);
-  return th1 ? launch_tile_t<EOS, VISC, MILNE, false, true>(h, stage, A, mid) : launch_tile_t<EOS, VISC, MILNE, false, false>(h, stage, A, mid);
-}
-static cudaError_t launch_tile(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
-  const bool visc = h->prm.physics != 0, milne = h->prm.geometry == 0;
-  const int eos = h->prm.eos;
-  if (visc) return eos ? launch_tile_d<1, true, true>(h, stage, A, mid) : launch_tile_d<0, true, true>(h, stage, A, mid);
-  if (milne) return eos ? launch_tile_d<1, false, true>(h, stage, A, mid) : launch_tile_d<0, false, true>(h, stage, A, mid);
-  return eos ? launch_tile_d<1, false, false>(h, stage, A, mid) : launch_tile_d<0, false, false>(h, stage, A, mid);
-}
 static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, double* u) {
   const DevParams& P = h->P;
   long long W = h->two_d ? (long long)P.ny + P.nx : (long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny;
@@ -438,12 +311,11 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   // variants 0, 2: (velocity kernel, stage kernel) per stage, ghost replicas written by the stage kernel;
   // variant 1: (cell kernel, ghost kernel) per stage.  ev[0..4] bracket the four launches of the step.
   const bool split = (h->variant != 1);
-  const bool tile = (h->variant == 0);
   if (ev) CUDA_TRY(h, cudaEventRecord(ev[0], h->stream));
   if (split) {
-    CUDA_TRY(h, tile ? launch_tile(h, 1, A, ev ? ev[1] : nullptr) : launch_split(h, 1, A, ev ? ev[1] : nullptr));
+    CUDA_TRY(h, launch_stage_any(h, 1, A, ev ? ev[1] : nullptr));
   } else {
-    CUDA_TRY(h, launch_stage(h, 1, A));
+    CUDA_TRY(h, launch_stage_any(h, 1, A, nullptr));
     if (ev) CUDA_TRY(h, cudaEventRecord(ev[1], h->stream));
     CUDA_TRY(h, launch_ghost(h, h->q[1], h->e[1], h->p[1], h->u[2]));
   }
@@ -453,9 +325,9 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
   A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1]; A.t = t1; A.t_post = t1;
   if (split) {
-    CUDA_TRY(h, tile ? launch_tile(h, 2, A, ev ? ev[3] : nullptr) : launch_split(h, 2, A, ev ? ev[3] : nullptr));
+    CUDA_TRY(h, launch_stage_any(h, 2, A, ev ? ev[3] : nullptr));
   } else {
-    CUDA_TRY(h, launch_stage(h, 2, A));
+    CUDA_TRY(h, launch_stage_any(h, 2, A, nullptr));
     if (ev) CUDA_TRY(h, cudaEventRecord(ev[3], h->stream));
     CUDA_TRY(h, launch_ghost(h, h->q[2], h->e[0], h->p[0], h->u[1]));
   }

@@ -1,0 +1,54 @@
+// vh_internal.cuh -- shared between vh_api.cu and the per-physics launch units (vh_launch.cu, compiled once per combination
+// of EOS / viscous / Milne so that the units build in parallel): the handle and the launch entry points.
+#pragma once
+#include "../../include/vh.h"
+#include "vh_kernels3.cuh"
+
+#include <cstdio>
+#include <cstdlib>
+#include <string>
+
+#ifndef VH_STAGE_MINB
+#define VH_STAGE_MINB 2      // resident blocks per SM the stage kernel is compiled for (register cap 65536/(256*MINB))
+#endif
+
+struct vh_handle {
+  vh_params prm;
+  vh::DevParams P;
+  cudaStream_t stream = nullptr;
+  double* pool = nullptr;            // 67 padded arrays
+  double* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
+  double* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
+  double* e[2] = {nullptr, nullptr};            // e^n / e^{n+1}, e*
+  double* p[2] = {nullptr, nullptr};
+  double* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
+  double* vR = nullptr;              // [3] ... high face
+  vh::Counters* cnt = nullptr;
+  double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
+  double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
+  long long n_steps = 0;
+  long long launches = 0;
+  bool initialised = false;
+  bool two_d = false;
+  int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
+  CUtensorMap mapA, mapZ, mapC;      // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes, box C: the tile)
+  std::string err;
+};
+
+
+// VH_DEBUG_SYNC=1 in the environment: synchronise after every launch and name the kernel that faulted.
+inline cudaError_t vh_debug_sync(vh_handle* h, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  static const bool on = getenv("VH_DEBUG_SYNC") != nullptr;
+  if (e == cudaSuccess && on) {
+    e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) fprintf(stderr, "[vh] %s faulted at step %lld: %s\n", what, h->n_steps, cudaGetErrorString(e));
+  }
+  return e;
+}
+
+// One Euler stage (kernels of the handle's variant) for one combination of template parameters; defined in vh_launch.cu.
+// combo = eos + 2 * (0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian).  mid (optional) is recorded between the two launches.
+#define VH_DECLARE_COMBO(K) cudaError_t vh_launch_stage_combo##K(vh_handle* h, int stage, const vh::StageArgs& A, cudaEvent_t mid);
+VH_DECLARE_COMBO(0) VH_DECLARE_COMBO(1) VH_DECLARE_COMBO(2) VH_DECLARE_COMBO(3) VH_DECLARE_COMBO(4) VH_DECLARE_COMBO(5)
+#undef VH_DECLARE_COMBO

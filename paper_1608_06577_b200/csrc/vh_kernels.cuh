@@ -390,12 +390,12 @@ __global__ void __launch_bounds__(256) pressure_kernel(const __grid_constant__ D
 }
 
 // ------------------------------------------------------------------------------------------------ peak microbenchmarks
-__global__ void __launch_bounds__(256) copy_kernel(const double2* __restrict__ src, double2* __restrict__ dst, long long n2) {
+static __global__ void __launch_bounds__(256) copy_kernel(const double2* __restrict__ src, double2* __restrict__ dst, long long n2) {
   long long stride = (long long)gridDim.x * blockDim.x;
   for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < n2; w += stride) dst[w] = src[w];
 }
 
-__global__ void __launch_bounds__(256) fma_kernel(double* out, int iters, double a, double b) {
+static __global__ void __launch_bounds__(256) fma_kernel(double* out, int iters, double a, double b) {
   double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
   for (int it = 0; it < iters; ++it) {
 #pragma unroll

@@ -396,7 +396,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     const double theta = P.theta;
     const bool fx = P.nx > 1, fy = P.ny > 1, fz = !TWO_D;
     const double wt2 = wt * t2;
-#pragma unroll 1
+#pragma unroll
     for (int n = 0; n < NF; ++n) {
       const double* sb = acquire(5 + n);
       const double* s = sb + oc;
