@@ -197,6 +197,129 @@ __device__ __forceinline__ void dissipative_sources3(const DevParams& P, double 
   emit(BPI, dt * fma(-fma(zotP, K.theta, fma(Pi, itP, IPi)), iut, Pi * divv));                  // B.10
 }
 
+// ------------------------------------------------------------------------------------------------ relaxation sources, register-lean
+// Same regrouping as dissipative_sources3, ordered so that few values are live at a time (the 128-register budget of a
+// 512-thread CTA): (1) kinematic tensors sigma (10) and W (6) as scalars (A.5-A.19); (2) the pi-independent part
+// c_pi pi^{mn} + c_S sigma^{mn} goes to the cell's park slot at once; (3) sigma, W are transformed IN PLACE into the 16
+// entries of Y^{ln} (pair (l,n), l < n: Y^{ln} = g_l (b sigma + a W), Y^{nl} = g_n (b sigma - a W)); (4) the contraction with
+// pi is added to the parked value.  pi(s) reads the cell's pi component from shared memory; ld/st access the park slot.
+template <int EOS, class PiGet, class ParkLd, class ParkSt>
+__device__ __forceinline__ void relaxation_sources4(const DevParams& P, double t, const double (&u)[4], const double (&du)[4][4], PiGet pi,
+                                                    double Pi, double e, double divv, double dt, ParkLd ld, ParkSt st) {
+  const double ut = u[0], ux = u[1], uy = u[2], un = u[3];
+  const double t2 = t * t, it = rcp_fast(t), it2 = it * it;
+  const double* dT = du[0]; const double* dX = du[1]; const double* dY = du[2]; const double* dN = du[3];
+  // convective derivatives (A.5-A.8), expansion rate (A.11), covariant acceleration (A.9-A.10)
+  const double dut = ut * dT[0] + ux * dX[0] + uy * dY[0] + un * dN[0];
+  const double dux = ut * dT[1] + ux * dX[1] + uy * dY[1] + un * dN[1];
+  const double duy = ut * dT[2] + ux * dX[2] + uy * dY[2] + un * dN[2];
+  const double dun = ut * dT[3] + ux * dX[3] + uy * dY[3] + un * dN[3];
+  const double th = ut * it + dT[0] + dX[1] + dY[2] + dN[3];
+  const double th3 = th * (1.0 / 3.0);
+  const double un2 = un * un;
+  const double Du0 = dut + t * un2, Du1 = -dux, Du2 = -duy, Du3 = -t2 * dun - 2.0 * t * ut * un;
+  // Z[0..9] = sigma^{mu nu} (A.12; slot order tt tx ty tn xx xy xn yy yn nn), Z[10..15] = W^{tx} W^{ty} W^{tn} W^{xy} W^{xn} W^{yn}
+  double Z[16];
+  Z[0] = -t * ut * un2 + dT[0] - ut * dut + (ut * ut - 1.0) * th3;
+  Z[1] = -0.5 * t * un2 * ux + 0.5 * (dT[1] - dX[0]) - 0.5 * (ut * dux + ux * dut) + ut * ux * th3;
+  Z[2] = -0.5 * t * un2 * uy + 0.5 * (dT[2] - dY[0]) - 0.5 * (ut * duy + uy * dut) + ut * uy * th3;
+  Z[3] = -0.5 * un * it * (2.0 * ut * ut + t2 * un2) + 0.5 * (dT[3] - dN[0] * it2) - 0.5 * (ut * dun + un * dut) + ut * un * th3;
+  Z[4] = -dX[1] - ux * dux + (1.0 + ux * ux) * th3;
+  Z[5] = -0.5 * (dX[2] + dY[1]) - 0.5 * (ux * duy + uy * dux) + ux * uy * th3;
+  Z[6] = -ut * ux * un * it - 0.5 * (dX[3] + dN[1] * it2) - 0.5 * (ux * dun + un * dux) + ux * un * th3;
+  Z[7] = -dY[2] - uy * duy + (1.0 + uy * uy) * th3;
+  Z[8] = -ut * uy * un * it - 0.5 * (dY[3] + dN[2] * it2) - 0.5 * (uy * dun + un * duy) + uy * un * th3;
+  Z[9] = -ut * it2 * it * (1.0 + 2.0 * un2 * t2) - dN[3] * it2 - un * dun + (it2 + un2) * th3;
+  Z[10] = 0.5 * (dT[1] + dX[0]) + 0.5 * (ux * dut - ut * dux) + 0.5 * t * un2 * ux;
+  Z[11] = 0.5 * (dT[2] + dY[0]) + 0.5 * (uy * dut - ut * duy) + 0.5 * t * un2 * uy;
+  Z[12] = un * it + 0.5 * dT[3] + 0.5 * dN[0] * it2 + 0.5 * (un * dut - ut * dun) - ut * ut * un * it + 0.5 * t * un2 * un;
+  Z[13] = 0.5 * (dY[1] - dX[2]) + 0.5 * (uy * dux - ux * duy);
+  Z[14] = 0.5 * dN[1] * it2 - 0.5 * dX[3] + 0.5 * (un * dux - ux * dun) - ux * ut * un * it;
+  Z[15] = 0.5 * dN[2] * it2 - 0.5 * dY[3] + 0.5 * (un * duy - uy * dun) - uy * ut * un * it;
+
+  // transport coefficients (Eqs. 10-16; R14)
+  double p, cs2;
+  eos_p_cs2<EOS>(P, e, p, cs2);
+  const double T = sqrt_fast(sqrt_fast(e * P.eos_a_inv));
+  const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
+  const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
+  double zs = 0.0;
+  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp(-d * d); }
+  else if (P.zeta_model == 2) zs = P.zeta_amp;
+  const double b = (1.0 / 3.0) - cs2;
+  double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi * rcp_fast(zs) : CUDART_INF;
+  itP = fmin(itP, P.relax_clamp);
+  const double zotP = (zs > 0.0) ? zs * ((e + p) * rcp_fast(T)) * itP : 0.0;
+  const double iut = rcp_fast(ut);
+  const double w = dt * iut;
+
+  // pi^{mu nu} sigma_{mu nu}: symmetric double contraction with the metric weights of g = diag(1,-1,-1,-t2)
+  const double pisig = pi(0) * Z[0] - 2.0 * (pi(1) * Z[1] + pi(2) * Z[2]) + pi(4) * Z[4] + 2.0 * pi(5) * Z[5] + pi(7) * Z[7] +
+                       t2 * (2.0 * (pi(6) * Z[6] + pi(8) * Z[8] - pi(3) * Z[3]) + t2 * pi(9) * Z[9]);
+  {     // Pi (B.10, Eq. 41): done first, its coefficients die here
+    const double IPi = P.delta_PiPi * Pi * th - P.lambda_Pipi_coef * b * pisig;
+    st(BPI, dt * fma(-fma(zotP, th, fma(Pi, itP, IPi)), iut, Pi * divv));
+  }
+  {     // (2) pi-independent part: c_pi pi^{mn} + c_S sigma^{mn}
+    const double cpi = dt * fma(-iut, fma(P.delta_pipi, th, itp), divv);
+    const double cS = w * fma(P.lambda_piPi, Pi, eotp2);
+#pragma unroll
+    for (int s = 0; s < 10; ++s) st(PTT + s, fma(cS, Z[s], cpi * pi(s)));
+  }
+  const double beta = P.tau_pipi * pisig * (1.0 / 6.0);
+  // A'^m = pi^{lm} Du_l + beta u^m;  u'^m = w u^m
+  double Ap[4], up[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    Ap[m] = fma(beta, u[m], pi(sym(0, m)) * Du0 + pi(sym(1, m)) * Du1 + pi(sym(2, m)) * Du2 + pi(sym(3, m)) * Du3);
+    up[m] = w * u[m];
+  }
+  // (3) in place: Y[l][n] = g_l (bh sigma^{ln} + am W^{ln}), g = w (1,-1,-1,-t2), W antisymmetric
+  double Y[4][4];
+  {
+    const double gl[4] = {w, -w, -w, -w * t2};
+    const double bh = 0.5 * P.tau_pipi, am = -kVorticitySign;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      Y[l][l] = gl[l] * (bh * Z[sym(l, l)]);
+#pragma unroll
+      for (int n = l + 1; n < 4; ++n) {
+        const int wi = (l == 0) ? 9 + n : ((l == 1) ? 11 + n : 15);      // 01 02 03 12 13 23 -> Z[10..15]
+        const double c1 = bh * Z[sym(l, n)], c2 = am * Z[wi];
+        Y[l][n] = gl[l] * (c1 + c2);
+        Y[n][l] = gl[n] * (c1 - c2);
+      }
+    }
+  }
+  const double k3 = 2.0 * w * beta;
+  const double gi[4] = {1.0, -1.0, -1.0, -it2};
+  const double g1 = w * t * un, g2 = w * ut * it, g3 = w * un * it;      // Christoffel weights of G_pi (:300; R1, R2)
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = m; n < 4; ++n) {
+      const int s = sym(m, n);
+      double J = ld(PTT + s);
+      J = fma(-up[n], Ap[m], J);
+      J = fma(-up[m], Ap[n], J);
+#pragma unroll
+      for (int l = 0; l < 4; ++l) {
+        J = fma(-pi(sym(m, l)), Y[l][n], J);
+        J = fma(-pi(sym(n, l)), Y[l][m], J);
+      }
+      if (m == n) J = fma(k3, gi[m], J);
+      // G_pi = u^a Gamma^mu_{ab} pi^{b nu} + (mu<->nu)
+      if (s == 0) J = fma(-2.0 * g1, pi(3), J);
+      if (s == 1) J = fma(-g1, pi(6), J);
+      if (s == 2) J = fma(-g1, pi(8), J);
+      if (s == 3) J = fma(-g1, pi(9), fma(-g2, pi(3), fma(-g3, pi(0), J)));
+      if (s == 6) J = fma(-g2, pi(6), fma(-g3, pi(1), J));
+      if (s == 8) J = fma(-g2, pi(8), fma(-g3, pi(2), J));
+      if (s == 9) J = fma(-2.0 * g2, pi(9), fma(-2.0 * g3, pi(3), J));
+      st(PTT + s, J);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ the kernel
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
 __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
@@ -368,12 +491,11 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   if (VISC) {
 #pragma unroll
     for (int n = 0; n < 4; ++n) du[0][n] = (uc[n] - upv[n]) * P.inv_dtau;      // backward difference in time (:424)
-    Kin K;
-    kinematics(uc, du[0], du[1], du[2], du[3], t, K);
     mbar_wait(&full[NSTAGE], 0u);
     const double* mine = cen + tid;
-    dissipative_sources3<EOS>(P, t, uc, K, [&](int s) { return mine[s * NT]; }, mine[10 * NT], ec, divv, dt,
-                              [&](int slot, double J) { park[slot * NT + tid] = J; });
+    double* mypark = park + tid;
+    relaxation_sources4<EOS>(P, t, uc, du, [&](int s) { return mine[s * NT]; }, mine[10 * NT], ec, divv, dt,
+                             [&](int slot) { return mypark[slot * NT]; }, [&](int slot, double J) { mypark[slot * NT] = J; });
   }
 
   // ================================================================= phase 3: the q fields (flux divergence + conservation sources)
