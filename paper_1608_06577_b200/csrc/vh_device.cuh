@@ -152,7 +152,9 @@ __device__ __forceinline__ void kinematics(const double u[4], const double dt[4]
 
 // symmetric-slot lookup for 4x4 symmetric tensors stored as 10 (tt tx ty tn xx xy xn yy yn nn)
 __device__ __forceinline__ constexpr int sym(int m, int n) {
-  return (m > n) ? sym(n, m) : (m == 0 ? n : (m == 1 ? 3 + n : (m == 2 ? 5 + n : 9)));
+  // not recursive: a recursive form is not always folded and then costs a real call plus a dynamically indexed local array
+  const int a = (m < n) ? m : n, b = (m < n) ? n : m;
+  return (a == 0) ? b : ((a == 1) ? 3 + b : ((a == 2) ? 5 + b : 9));
 }
 
 // Dissipative source terms J = S + G for the 10 pi components and Pi (B.10-B.12, Eqs. 39-46).
