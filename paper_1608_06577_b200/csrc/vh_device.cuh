@@ -35,6 +35,28 @@ struct DevParams {
   int debug;                    // VH_DEBUG_FLAGS (development only)
 };
 
+// ---------------------------------------------------------------- exp(-x) for the EOS and zeta/s(T)
+// exp(-x) with the argument clamped to [-700, 708] (beyond: 1e304 / 3e-308 instead of inf / 0, never reached by a state
+// that passes the finiteness checks).  -x = k ln2 + r, |r| <= ln2/2, Taylor polynomial of degree 13 (truncation 4e-18), 2^k
+// added into the exponent field.  The coefficients sit in constant memory so that each Horner step is ONE DFMA with a
+// constant-bank operand; the library exp() materialises its 64-bit immediates with two moves per coefficient, which made
+// half of its instructions moves (profiles/r01b_ncu_summary.md).  About 1 ulp, like the library routine.
+static __constant__ double kExpTaylor[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880,
+                                             1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
+static __constant__ double kExpRed[4] = {1.4426950408889634, 6755399441055744.0, 6.93147180369123816490e-01, 1.90821492927058770002e-10};
+__device__ __forceinline__ double exp_neg(double x) {
+  x = fmin(fmax(x, -700.0), 708.0);
+  const double t = fma(-x, kExpRed[0], kExpRed[1]);      // 1.5 * 2^52 + rint(-x log2 e): the integer sits in the low word
+  const int k = __double2loint(t);
+  const double kd = t - kExpRed[1];
+  double r = fma(-kd, kExpRed[2], -x);
+  r = fma(-kd, kExpRed[3], r);
+  double p = kExpTaylor[13];
+#pragma unroll
+  for (int i = 12; i >= 0; --i) p = fma(p, r, kExpTaylor[i]);
+  return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
 // ---------------------------------------------------------------- EOS (BASELINE.json configs) and transport (Eqs. 10-16)
 template <int EOS> __device__ __forceinline__ void eos_p_cs2(const DevParams& P, double e, double& p, double& cs2) {
   if (EOS == 0) {
@@ -42,7 +64,7 @@ template <int EOS> __device__ __forceinline__ void eos_p_cs2(const DevParams& P,
     cs2 = 1.0 / 3.0;
   } else {
     double x = e * P.eos_e0_inv;
-    double aex = P.eos_alpha * exp(-x);
+    double aex = P.eos_alpha * exp_neg(x);
     p = (e * (1.0 / 3.0)) * (1.0 - aex);
     cs2 = (1.0 / 3.0) * (1.0 - aex * (1.0 - x));
   }
@@ -169,7 +191,7 @@ __device__ __forceinline__ void dissipative_sources(const DevParams& P, double t
   double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
   double eotp = (e + p) * P.inv_ctaupi;
   double zs = 0.0;
-  if (P.zeta_model == 1) { double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp(-d * d); }
+  if (P.zeta_model == 1) { double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp_neg(d * d); }
   else if (P.zeta_model == 2) zs = P.zeta_amp;
   double b = (1.0 / 3.0) - cs2;
   double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi / zs : CUDART_INF;

@@ -46,7 +46,7 @@ __device__ __forceinline__ bool cell_index(const DevParams& P, int& i, int& j, i
 
 // ------------------------------------------------------------------------------------------------ velocity kernel
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int BX, int BY, int BZ>
-__global__ void __launch_bounds__(BX* BY* BZ) velocity_kernel(const __grid_constant__ DevParams P, const __grid_constant__ VelArgs A) {
+__global__ void __launch_bounds__(BX* BY* BZ, 4) velocity_kernel(const __grid_constant__ DevParams P, const __grid_constant__ VelArgs A) {
   int i, j, k;
   long long c;
   const bool valid = cell_index<BX, BY, BZ>(P, i, j, k, c);
@@ -239,7 +239,7 @@ __device__ __forceinline__ void dissipative_sources2(const DevParams& P, double 
   const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
   const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
   double zs = 0.0;
-  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp(-d * d); }
+  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp_neg(d * d); }
   else if (P.zeta_model == 2) zs = P.zeta_amp;
   const double b = (1.0 / 3.0) - cs2;
   double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi / zs : CUDART_INF;
