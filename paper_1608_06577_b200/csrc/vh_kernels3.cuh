@@ -509,14 +509,14 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
         if (d < ND) {
           const double* vL = A.vL + d * fs + c;
           const double* vR = A.vR + d * fs + c;
-          face_coefficients(vR[-sd[d]], vL[0], vR[0], vL[sd[d]], w[d], cf[d][0], cf[d][1], cf[d][2], cf[d][3]);
+          const int ext = (d == 0) ? P.nx : ((d == 1) ? P.ny : P.nz);
+          face_coefficients(vR[-sd[d]], vL[0], vR[0], vL[sd[d]], (ext > 1) ? w[d] : 0.0, cf[d][0], cf[d][1], cf[d][2], cf[d][3]);
         } else {
           cf[d][0] = cf[d][1] = cf[d][2] = cf[d][3] = 0.0;
         }
       }
     }
     const double theta = P.theta;
-    const bool fx = P.nx > 1, fy = P.ny > 1, fz = !TWO_D;
     const double wt2 = wt * t2;
 #pragma unroll
     for (int n = 0; n < NF; ++n) {
@@ -531,9 +531,11 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       double r = a2;
       if (VISC && n >= PTT) r += park[n * NT + tid];
       if (MILNE && n < 4) r = fma((n == 3) ? -3.0 * wt : -wt, a2, r);      // G_c (:1013): -T^{tau mu}/tau, -3 T^{tau eta}/tau
-      if (fx) r = flux_line<THETA1>(x0, x1, a2, x3, x4, cf[0][0], cf[0][1], cf[0][2], cf[0][3], theta, r);
-      if (fy) r = flux_line<THETA1>(y0, y1, a2, y3, y4, cf[1][0], cf[1][1], cf[1][2], cf[1][3], theta, r);
-      if (fz) r = flux_line<THETA1>(z0, z1, a2, z3, z4, cf[2][0], cf[2][1], cf[2][2], cf[2][3], theta, r);
+      // three independent chains (the coefficients of a direction of extent 1 are zero: no branch, the fluxes cancel identically)
+      const double rx = flux_line<THETA1>(x0, x1, a2, x3, x4, cf[0][0], cf[0][1], cf[0][2], cf[0][3], theta, 0.0);
+      const double ry = flux_line<THETA1>(y0, y1, a2, y3, y4, cf[1][0], cf[1][1], cf[1][2], cf[1][3], theta, 0.0);
+      if (!TWO_D) r += flux_line<THETA1>(z0, z1, a2, z3, z4, cf[2][0], cf[2][1], cf[2][2], cf[2][3], theta, 0.0);
+      r += rx + ry;
       park[n * NT + tid] = r;
       if (VISC && n >= PTT) {
         // this field's part of A^{i nu} = P (v^i delta^nu_tau - g^{i nu}) - v^i pi^{tau nu} + pi^{i nu}, differenced (B.2-B.5)
