@@ -33,7 +33,7 @@ template <bool TWO_D> struct Tile {
   static constexpr int A_SIZE = AX * AY * TZ;                   // doubles in box A
   static constexpr int Z_SIZE = TWO_D ? 0 : TX * TY * 2;        // doubles in one eta-halo box
   static constexpr int SLOT = A_SIZE + 2 * Z_SIZE;              // doubles per ring slot (13312 B / 5760 B: multiples of 128)
-  static constexpr int NSTAGE = 4;
+  static constexpr int NSTAGE = 6;
   static constexpr int NCEN = 11;                               // centre rows: pi^{mu nu} (10), Pi
 };
 template <bool TWO_D, bool VISC> constexpr size_t tile_smem_bytes() {
