@@ -5,9 +5,9 @@
 // mbarrier ("full") that the loads complete with their byte count.  A slot holds the star-shaped neighbourhood of the
 // tile for one array: box A = (TX+4) x (TY+4) x TZ (the tile with its +-2 halo in x and y) plus, in 3+1d, two boxes of
 // TX x TY x 2 planes below and above the tile (the +-2 halo in eta); ghost edges / corners are never loaded (:453).
-// While array s is consumed the loads of arrays s+1 .. s+NSTAGE-1 are in flight.  A slot is handed back by a counter:
-// lane 0 of every warp adds 1 (release) after the warp's reads, and the warp that completes the count re-arms the
-// barrier and issues the next loads into that slot - no block-wide barrier inside the stream.
+// While array s is consumed the loads of arrays s+1 .. s+NSTAGE-1 are in flight.  A slot is handed back through a second
+// mbarrier ("empty", NW arrivals): lane 0 of every warp arrives after the warp's reads, and the warp whose arrival was the
+// last one pending re-arms "full" and issues the next loads into that slot - no block-wide barrier inside the stream.
 // Per array the thread reads its 13-point star from the slot and accumulates
 //   * the KT flux divergence of that field in x, y, eta (Eqs. 59-68) and
 //   * that field's contribution to the sources of the four conservation laws (B.2-B.5 and G_c, :1013),
@@ -38,8 +38,7 @@ template <bool TWO_D> struct Tile {
 };
 template <bool TWO_D, bool VISC> constexpr size_t tile_smem_bytes() {
   using T = Tile<TWO_D>;
-  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(double) + (T::NSTAGE + 1) * sizeof(uint64_t) +
-         T::NSTAGE * sizeof(unsigned);
+  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(double) + (2 * T::NSTAGE + 1) * sizeof(uint64_t);
 }
 
 struct TileArgs {
@@ -80,11 +79,13 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, u
       "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
       : "memory");
 }
-// counter of warps that are done with a ring slot: +1 with release/acquire ordering at CTA scope, returns the old value
-__device__ __forceinline__ unsigned slot_counter_add(unsigned* p) {
-  unsigned old;
-  asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(p)) : "memory");
-  return old;
+// arrive on a barrier (release) and return the number of arrivals that were still pending BEFORE this one
+__device__ __forceinline__ unsigned mbar_arrive_pending(uint64_t* bar) {
+  uint64_t state;
+  unsigned pending;
+  asm volatile("mbarrier.arrive.shared::cta.b64 %0, [%1];" : "=l"(state) : "r"(smem_u32(bar)) : "memory");
+  asm volatile("mbarrier.pending_count.b64 %0, %1;" : "=r"(pending) : "l"(state));
+  return pending;
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
@@ -320,6 +321,34 @@ __device__ __forceinline__ void relaxation_sources4(const DevParams& P, double t
     }
 }
 
+// ------------------------------------------------------------------------------------------------ regularisation factor
+// tanh(rho)/rho of Eqs. 73-74 (R9) with the branch-free reciprocal / square roots of vh_math.cuh (the IEEE sqrt and division
+// of regulation_factor() each cost a call-like slow path); same case analysis.
+template <bool MILNE>
+__device__ __forceinline__ double regulation_factor_fast(const DevParams& P, const double q[NQ], double e, double p0, const double u[4], double t) {
+  const double t2 = MILNE ? t * t : 1.0;
+  const double* pi = q + PTT;
+  const double Pi = q[BPI];
+  const double pipi = pi[0] * pi[0] - 2.0 * (pi[1] * pi[1] + pi[2] * pi[2] + t2 * pi[3] * pi[3]) + pi[4] * pi[4] + 2.0 * pi[5] * pi[5] +
+                      2.0 * t2 * pi[6] * pi[6] + pi[7] * pi[7] + 2.0 * t2 * pi[8] * pi[8] + t2 * t2 * pi[9] * pi[9];
+  const double tr = pi[0] - pi[4] - pi[7] - t2 * pi[9];
+  const double PP = sqrt_fast(fabs(pipi + 3.0 * Pi * Pi));
+  double rho = PP * P.inv_rho_max * rsqrt_fast(e * e + 3.0 * p0 * p0);
+  const double den1 = P.xi0_rho_max * PP;
+  if (PP > 0.0 && isfinite(den1)) {
+    const double id = rcp_fast(den1);
+    // pi^{l mu} u_mu, u_mu = (ut,-ux,-uy,-t2 un); the l = eta entry is multiplied by tau
+    const double c0 = pi[0] * u[0] - pi[1] * u[1] - pi[2] * u[2] - t2 * pi[3] * u[3];
+    const double c1 = pi[1] * u[0] - pi[4] * u[1] - pi[5] * u[2] - t2 * pi[6] * u[3];
+    const double c2 = pi[2] * u[0] - pi[5] * u[1] - pi[7] * u[2] - t2 * pi[8] * u[3];
+    const double c3 = (pi[3] * u[0] - pi[6] * u[1] - pi[8] * u[2] - t2 * pi[9] * u[3]) * (MILNE ? t : 1.0);
+    const double m = fmax(fmax(fabs(tr), fabs(c0)), fmax(fmax(fabs(c1), fabs(c2)), fabs(c3)));
+    rho = fmax(rho, m * id);
+  }
+  if (!isfinite(rho)) rho = 0.0;
+  return (rho < 1e-8) ? 1.0 : tanh(rho) * rcp_fast(rho);
+}
+
 // ------------------------------------------------------------------------------------------------ the kernel
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
 __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
@@ -336,7 +365,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   double* park = ring + NSTAGE * T::SLOT;                                   // [NF][NT]   running values
   double* cen = park + NF * NT;                                             // [NCEN][NT] the cell's own pi^{mu nu}, Pi (VISC)
   uint64_t* full = reinterpret_cast<uint64_t*>(cen + (VISC ? T::NCEN * NT : 0));   // [NSTAGE] ring slots, [NSTAGE] = centre rows
-  unsigned* used = reinterpret_cast<unsigned*>(full + NSTAGE + 1);          // [NSTAGE] warps done with the slot (monotonic)
+  uint64_t* empty = full + NSTAGE + 1;                                      // [NSTAGE] one arrival per warp that is done with the slot
 
   const int tid = threadIdx.x;
   const int tx = tid % TX, ty = (tid / TX) % TY, tz = tid / (TX * TY);
@@ -366,7 +395,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
 #pragma unroll
     for (int s = 0; s <= NSTAGE; ++s) mbar_init(&full[s], 1);
 #pragma unroll
-    for (int s = 0; s < NSTAGE; ++s) used[s] = 0u;
+    for (int s = 0; s < NSTAGE; ++s) mbar_init(&empty[s], (unsigned)T::NW);
     fence_mbar_init();
   }
   __syncthreads();
@@ -385,11 +414,12 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     mbar_wait(&full[s % NSTAGE], (unsigned)((s / NSTAGE) & 1));
     return ring + (s % NSTAGE) * T::SLOT;
   };
+  const bool lane0 = (tid & 31) == 0;
   auto release = [&](int s) {
     __syncwarp();
-    if ((tid & 31) == 0) {
-      const unsigned old = slot_counter_add(&used[s % NSTAGE]);
-      if ((old + 1u) % (unsigned)T::NW == 0u && s + NSTAGE < NSTREAM) issue(s + NSTAGE);
+    if (lane0 && s + NSTAGE < NSTREAM) {
+      // the arrival that finds one arrival pending is the last one of this use of the slot: that warp refills it
+      if (mbar_arrive_pending(&empty[s % NSTAGE]) == 1u) issue(s + NSTAGE);
     }
   };
 
@@ -590,18 +620,23 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   const double u[4] = {ut, Mx * inv, My * inv, Mn * inv};
   if (!(isfinite(e) && isfinite(ut))) ++nnonf;
   if (VISC) {
-    const double fac = regulation_factor<MILNE>(P, qv, e, p0, u, tp);
+    const double fac = regulation_factor_fast<MILNE>(P, qv, e, p0, u, tp);
     minfac = fmin(minfac, fac);
 #pragma unroll
     for (int n = PTT; n < NQ; ++n) qv[n] *= fac;
   }
   if (valid) {
-    // ghost replicas (Eqs. 75-76): the outermost physical cell is copied into both ghost layers of its face
-    const bool edge = (i == 0) | (i == P.nx - 1) | (j == 0) | (j == P.ny - 1) | (!TWO_D && ((k == 0) | (k == P.nz - 1)));
     const long long sy = P.NXp, sz = P.plane;
-    auto put = [&](double* a, double v) {
-      a[c] = v;
-      if (edge) {
+#pragma unroll
+    for (int n = 0; n < NQ; ++n) A.q_out[n * fs + c] = qv[n];
+    A.e_out[c] = e;
+    A.p_out[c] = p0;
+#pragma unroll
+    for (int n = 0; n < 4; ++n) A.u_out[n * fs + c] = u[n];
+    // ghost replicas (Eqs. 75-76): the outermost physical cell is copied into both ghost layers of its face (one rarely taken block)
+    const bool edge = (i == 0) | (i == P.nx - 1) | (j == 0) | (j == P.ny - 1) | (!TWO_D && ((k == 0) | (k == P.nz - 1)));
+    if (edge) {
+      auto rep = [&](double* a, double v) {
         if (i == 0) { a[c - 1] = v; a[c - 2] = v; }
         if (i == P.nx - 1) { a[c + 1] = v; a[c + 2] = v; }
         if (j == 0) { a[c - sy] = v; a[c - 2 * sy] = v; }
@@ -610,14 +645,14 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
           if (k == 0) { a[c - sz] = v; a[c - 2 * sz] = v; }
           if (k == P.nz - 1) { a[c + sz] = v; a[c + 2 * sz] = v; }
         }
-      }
-    };
+      };
 #pragma unroll
-    for (int n = 0; n < NQ; ++n) put(A.q_out + n * fs, qv[n]);
-    put(A.e_out, e);
-    put(A.p_out, p0);
+      for (int n = 0; n < NQ; ++n) rep(A.q_out + n * fs, qv[n]);
+      rep(A.e_out, e);
+      rep(A.p_out, p0);
 #pragma unroll
-    for (int n = 0; n < 4; ++n) put(A.u_out + n * fs, u[n]);
+      for (int n = 0; n < 4; ++n) rep(A.u_out + n * fs, u[n]);
+    }
   }
   flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0);
 }
