@@ -230,8 +230,11 @@ __device__ __forceinline__ void flush_counters(Counters* cnt, unsigned long long
   if (nfail) atomicAdd(&cnt->n_fail, nfail);
   if (nnonf) atomicAdd(&cnt->n_nonfinite, nnonf);
   // warp minimum of the regularisation factor, then at most one atomic per warp (skipped when it cannot lower the record)
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) minfac = fmin(minfac, __shfl_xor_sync(0xffffffffu, minfac, o));
+  // (positive doubles order like their bit patterns: two integer warp reductions, high word then low word among the ties)
+  const unsigned hi = (unsigned)__double2hiint(minfac), lo = (unsigned)__double2loint(minfac);
+  const unsigned hmin = __reduce_min_sync(0xffffffffu, hi);
+  const unsigned lmin = __reduce_min_sync(0xffffffffu, (hi == hmin) ? lo : 0xffffffffu);
+  minfac = __hiloint2double((int)hmin, (int)lmin);
   if ((threadIdx.x + blockDim.x * threadIdx.y) % 32 == 0 && minfac < 1.0) {
     unsigned long long bits = (unsigned long long)__double_as_longlong(minfac);
     if (bits < *(volatile unsigned long long*)&cnt->min_reg_bits) atomicMin(&cnt->min_reg_bits, bits);
