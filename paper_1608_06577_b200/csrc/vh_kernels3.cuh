@@ -455,19 +455,6 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
 #pragma unroll
     for (int n = 0; n < 4; ++n) upv[n] = A.u_prev[n * fs + c];
   }
-  {      // pull what phases 3 and 4 read directly (state velocities, q^n) towards L2 while the stream runs
-    const long long sd[3] = {1, (long long)P.NXp, P.plane};
-#pragma unroll
-    for (int d = 0; d < ND; ++d) {
-      prefetch_l2(A.vL + d * fs + c); prefetch_l2(A.vR + d * fs + c);
-      if (d > 0) { prefetch_l2(A.vL + d * fs + c + sd[d]); prefetch_l2(A.vR + d * fs + c - sd[d]); }
-    }
-    if (STAGE == 2) {
-#pragma unroll
-      for (int n = 0; n < NF; ++n) prefetch_l2(A.q_n + n * fs + c);
-    }
-  }
-
   // ================================================================= phase 1: u^mu and p (velocity gradients, v^i, p terms)
   double uc[4], du[4][4], vm[3], vp[3], acc[4] = {0.0, 0.0, 0.0, 0.0}, divv = 0.0, gPi = 0.0;
   {
