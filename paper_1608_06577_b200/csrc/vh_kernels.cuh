@@ -226,7 +226,10 @@ __device__ __forceinline__ void post_cell(const DevParams& P, const StageArgs& A
   }
 }
 
-__device__ __forceinline__ void flush_counters(Counters* cnt, unsigned long long nfail, unsigned long long nnonf, double minfac) {
+// `record` is the value of cnt->min_reg_bits the caller read earlier (any earlier value works: the record only ever falls, so a
+// stale one lets a few redundant atomics through but never loses a minimum); reading it at kernel start hides the load latency.
+__device__ __forceinline__ void flush_counters(Counters* cnt, unsigned long long nfail, unsigned long long nnonf, double minfac,
+                                               unsigned long long record = ~0ull) {
   if (nfail) atomicAdd(&cnt->n_fail, nfail);
   if (nnonf) atomicAdd(&cnt->n_nonfinite, nnonf);
   // warp minimum of the regularisation factor, then at most one atomic per warp (skipped when it cannot lower the record)
@@ -237,7 +240,7 @@ __device__ __forceinline__ void flush_counters(Counters* cnt, unsigned long long
   minfac = __hiloint2double((int)hmin, (int)lmin);
   if ((threadIdx.x + blockDim.x * threadIdx.y) % 32 == 0 && minfac < 1.0) {
     unsigned long long bits = (unsigned long long)__double_as_longlong(minfac);
-    if (bits < *(volatile unsigned long long*)&cnt->min_reg_bits) atomicMin(&cnt->min_reg_bits, bits);
+    if (bits < record) atomicMin(&cnt->min_reg_bits, bits);
   }
 }
 
@@ -285,7 +288,7 @@ __global__ void __launch_bounds__(256) stage_cell_kernel(const __grid_constant__
     qo[n] = v;
   }
   post_cell<EOS, VISC, MILNE>(P, A, c, qo, ec, valid, nfail, nnonf, minfac);
-  if (!(P.debug & 1)) flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0);
+  if (!(P.debug & 1)) flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0, *(volatile unsigned long long*)&A.cnt->min_reg_bits);
 }
 
 // ------------------------------------------------------------------------------------------------ ghost cells (Eqs. 75-76)

@@ -416,7 +416,7 @@ __global__ void __launch_bounds__(BX* BY* BZ, MINB) stage_kernel(const __grid_co
 #pragma unroll
     for (int n = 0; n < 4; ++n) put(A.u_out + n * fs, u[n]);
   }
-  flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0);
+  flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0, *(volatile unsigned long long*)&A.cnt->min_reg_bits);
 }
 
 }  // namespace vh
