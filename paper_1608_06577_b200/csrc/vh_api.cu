@@ -122,6 +122,15 @@ static int make_tensor_maps(vh_handle* h, int n_arrays) {
   r = encode(&h->mapC, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxC, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box C) failed with CUresult " + std::to_string((int)r));
+  const cuuint32_t boxVA[5] = {(cuuint32_t)(td ? VTile<true>::AX : VTile<false>::AX), (cuuint32_t)(td ? VTile<true>::AY : VTile<false>::AY),
+                               (cuuint32_t)(td ? VTile<true>::VZ : VTile<false>::VZ), 1, 1};
+  r = encode(&h->mapVA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxVA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box VA) failed with CUresult " + std::to_string((int)r));
+  const cuuint32_t boxVZ[5] = {(cuuint32_t)VTile<false>::VX, (cuuint32_t)VTile<false>::VY, 1, 1, 1};
+  r = encode(&h->mapVZ, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxVZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box VZ) failed with CUresult " + std::to_string((int)r));
   return VH_OK;
 }
 

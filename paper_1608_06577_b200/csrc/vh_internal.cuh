@@ -2,7 +2,7 @@
 // of EOS / viscous / Milne so that the units build in parallel): the handle and the launch entry points.
 #pragma once
 #include "../../include/vh.h"
-#include "vh_kernels3.cuh"
+#include "vh_kernels4.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -31,6 +31,7 @@ struct vh_handle {
   bool initialised = false;
   bool two_d = false;
   int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
+  CUtensorMap mapVA, mapVZ;          // velocity tile kernel: tile + 1-cell y halo, one eta-halo plane
   CUtensorMap mapA, mapZ, mapC;      // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes, box C: the tile)
   std::string err;
 };

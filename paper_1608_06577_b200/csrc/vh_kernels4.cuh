@@ -1,0 +1,147 @@
+// vh_kernels4.cuh -- default velocity kernel ("velocity tile"): the interface-state inversions of one Euler stage with the
+// nine fields that enter Eq. 72 (T^{tau mu}, pi^{tau mu}, Pi) staged in shared memory by TMA.
+//
+// One CTA per VX x VY x VZ tile, one thread per cell.  Thread 0 issues, for each of the NV fields, one tensor-map box of the
+// tile with a 1-cell halo in y (and the 2-cell halo in x that the 16-byte start alignment of a box forces) plus, in 3+1d, one
+// plane below and one above the tile; all loads complete on ONE mbarrier, so the CTA waits once and then works from shared
+// memory only.  With 4-5 KB per field, four CTAs are resident per SM and hide one another's load latency (the register-file
+// limit of the 64-register kernel is four 256-thread CTAs as well).  Arithmetic as in velocity_kernel (vh_kernels2.cuh): per
+// direction the two reconstructed states the cell owns are inverted once, as a pair (Eqs. 63-66, 72; Alg. 3 :667-672).
+#pragma once
+#include "vh_kernels3.cuh"
+
+namespace vh {
+
+template <bool TWO_D> struct VTile {
+  static constexpr int VX = 32;
+  static constexpr int VY = TWO_D ? 8 : 4;
+  static constexpr int VZ = TWO_D ? 1 : 2;
+  static constexpr int NT = VX * VY * VZ;                       // 256 threads
+  static constexpr int AX = VX + 4, AY = VY + 2;
+  static constexpr int A_SIZE = AX * AY * VZ;                   // doubles in box A (tile + halo in x, y)
+  static constexpr int Z_SIZE = TWO_D ? 0 : VX * VY;            // doubles in one eta-halo plane
+  static constexpr int SLOT = (A_SIZE + 2 * Z_SIZE + 15) / 16 * 16;   // doubles per field, every TMA destination 128-byte aligned (3+1d: 688; 2+1d: 368)
+  static_assert(A_SIZE % 16 == 0 || TWO_D, "box Z destinations must stay 128-byte aligned");
+};
+template <bool TWO_D, bool VISC> constexpr size_t vtile_smem_bytes() {
+  return (size_t)((VISC ? 9 : 4) * VTile<TWO_D>::SLOT) * sizeof(double) + sizeof(uint64_t);
+}
+
+struct VelTileArgs {
+  const double* e;               // Newton guess: e of the cell (R6)
+  double* vL; double* vR;        // [3][fstride]: velocity of the state at the cell's low / high face, per direction
+  Counters* cnt;
+  double t;
+  int a_q;                       // index of q_in in the pool of padded arrays (outermost tensor-map coordinate)
+};
+
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
+__global__ void __launch_bounds__(VTile<TWO_D>::NT, 4)
+    velocity_tile_kernel(const __grid_constant__ DevParams P, const __grid_constant__ VelTileArgs A, const __grid_constant__ CUtensorMap mapVA,
+                         const __grid_constant__ CUtensorMap mapVZ) {
+  using T = VTile<TWO_D>;
+  constexpr int VX = T::VX, VY = T::VY, VZ = T::VZ, AX = T::AX, AY = T::AY;
+  constexpr int NV = VISC ? 9 : 4;
+  constexpr int ND = TWO_D ? 2 : 3;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* slots = reinterpret_cast<double*>(smem_raw);                      // [NV][SLOT]
+  uint64_t* full = reinterpret_cast<uint64_t*>(slots + NV * T::SLOT);
+
+  const int tid = threadIdx.x;
+  const int tx = tid % VX, ty = (tid / VX) % VY, tz = tid / (VX * VY);
+  const int nzb = (P.nz + VZ - 1) / VZ;
+  const int b = blockIdx.z / nzb;
+  const int i0 = blockIdx.x * VX, j0 = blockIdx.y * VY, k0 = (blockIdx.z % nzb) * VZ;
+  int i = i0 + tx, j = j0 + ty, k = k0 + tz;
+  const bool valid = (i < P.nx) && (j < P.ny) && (k < P.nz);
+  i = min(i, P.nx - 1); j = min(j, P.ny - 1); k = min(k, P.nz - 1);
+  const long long c = (long long)b * P.bstride + (long long)(k + P.zoff) * P.plane + (long long)(j + 2) * P.NXp + (i + 2);
+  const long long fs = P.fstride;
+
+  if (tid == 0) {
+    mbar_init(full, 1);
+    fence_mbar_init();
+    mbar_arrive_expect_tx(full, (unsigned)(NV * (T::A_SIZE + 2 * T::Z_SIZE) * sizeof(double)));      // the bytes the boxes deliver (SLOT is padded)
+#pragma unroll 1
+    for (int m = 0; m < NV; ++m) {
+      const int arr = A.a_q + ((m < 4) ? m : ((m < 8) ? PTT + (m - 4) : BPI));
+      double* dst = slots + m * T::SLOT;
+      // padded coordinates: physical cell (i0, j0, k0) sits at (i0+2, j0+2, k0+zoff)
+      tma_load_5d(dst, &mapVA, full, i0, j0 + 1, TWO_D ? 0 : k0 + 2, b, arr);
+      if (!TWO_D) {
+        tma_load_5d(dst + T::A_SIZE, &mapVZ, full, i0 + 2, j0 + 2, k0 + 1, b, arr);                   // plane k0-1
+        tma_load_5d(dst + T::A_SIZE + T::Z_SIZE, &mapVZ, full, i0 + 2, j0 + 2, k0 + 2 + VZ, b, arr);   // plane k0+VZ
+      }
+    }
+  }
+  const double guess = A.e[c];
+  __syncthreads();                 // the barrier initialisation is visible to every waiter
+
+  // offsets into a field's slot: centre, and the two eta neighbours (box A, or a halo plane at the tile faces)
+  const int oc = (tz * AY + (ty + 1)) * AX + (tx + 2);
+  int ozm = oc, ozp = oc;
+  if (!TWO_D) {
+    const int zl = T::A_SIZE + ty * VX + tx;
+    ozm = (tz >= 1) ? oc - AX * AY : zl;
+    ozp = (tz + 1 < VZ) ? oc + AX * AY : zl + T::Z_SIZE;
+  }
+  const double t2 = MILNE ? A.t * A.t : 1.0;
+  const double ht = 0.5 * P.theta;
+  unsigned long long nfail = 0;
+  mbar_wait(full, 0u);
+
+#pragma unroll
+  for (int d = 0; d < ND; ++d) {
+    const int om = (d == 0) ? oc - 1 : ((d == 1) ? oc - AX : ozm);
+    const int op = (d == 0) ? oc + 1 : ((d == 1) ? oc + AX : ozp);
+    const long long s = (d == 0) ? 1 : ((d == 1) ? (long long)P.NXp : P.plane);
+    const int pos = (d == 0) ? i : ((d == 1) ? j : k);
+    const int ext = (d == 0) ? P.nx : ((d == 1) ? P.ny : P.nz);
+    // L = state at the low face (q^+_{c-1/2}), R = state at the high face (q^-_{c+1/2})
+    double wL[5], wR[5];     // E, Mx, My, Mn, Pi
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+      const double* f = slots + m * T::SLOT;
+      const double a0 = f[om], a1 = f[oc], a2 = f[op];
+      const double h = half_slope2<THETA1>(a1 - a0, a2 - a1, ht);
+      wL[m] = a1 - h; wR[m] = a1 + h;
+    }
+    wL[4] = 0.0; wR[4] = 0.0;
+    if (VISC) {
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        const double* f = slots + (4 + m) * T::SLOT;
+        const double a0 = f[om], a1 = f[oc], a2 = f[op];
+        const double h = half_slope2<THETA1>(a1 - a0, a2 - a1, ht);
+        wL[m] -= a1 - h; wR[m] -= a1 + h;
+      }
+      const double* f = slots + 8 * T::SLOT;
+      const double a0 = f[om], a1 = f[oc], a2 = f[op];
+      const double h = half_slope2<THETA1>(a1 - a0, a2 - a1, ht);
+      wL[4] = a1 - h; wR[4] = a1 + h;
+    }
+    NewtonState SL, SR;
+    SL.E = wL[0]; SL.Pi = wL[4]; SL.M2 = wL[1] * wL[1] + wL[2] * wL[2] + t2 * wL[3] * wL[3];     // :339
+    SR.E = wR[0]; SR.Pi = wR[4]; SR.M2 = wR[1] * wR[1] + wR[2] * wR[2] + t2 * wR[3] * wR[3];
+    newton_pair<EOS>(P, SL, SR, guess);
+    double vl = wL[d + 1] * SL.rden, vr = wR[d + 1] * SR.rden;      // v^r = M_r/(E + P0 + Pi)  (Eqs. 53-54)
+    if (SL.fail) vl = clip_velocity(vl);
+    if (SR.fail) vr = clip_velocity(vr);
+    // status counter: every state of every interface once (see velocity_kernel); nothing along a direction of extent 1
+    if (ext > 1) {
+      nfail += (SL.fail ? 1u : 0u) + (SR.fail ? 1u : 0u);
+      if (pos == 0 && SL.fail) ++nfail;
+      if (pos == ext - 1 && SR.fail) ++nfail;
+    }
+    if (valid) {
+      double* vL = A.vL + d * fs + c;
+      double* vR = A.vR + d * fs + c;
+      vL[0] = vl; vR[0] = vr;
+      if (pos == 0) vR[-s] = vl;            // state q^-_{-1/2} of the ghost cell equals this cell's low-face state
+      if (pos == ext - 1) vL[s] = vr;
+    }
+  }
+  if (valid && nfail) atomicAdd(&A.cnt->n_fail, nfail);
+}
+
+}  // namespace vh

@@ -71,16 +71,25 @@ static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
 static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid) {
   const DevParams& P = h->P;
-  constexpr int BX = 32, BY = TWO_D ? 8 : 4, BZ = TWO_D ? 1 : 2;
-  dim3 block(BX, BY, BZ);
-  dim3 grid((P.nx + BX - 1) / BX, (P.ny + BY - 1) / BY, ((P.nz + BZ - 1) / BZ) * P.n_batch);
-  VelArgs V{S.q_in, S.e_in, h->vL, h->vR, S.cnt, S.t};
-  velocity_kernel<EOS, VISC, MILNE, TWO_D, THETA1, BX, BY, BZ><<<grid, block, 0, h->stream>>>(P, V);
-  h->launches++;
-  cudaError_t e = debug_sync(h, "velocity kernel");
-  if (e != cudaSuccess) return e;
-  if (mid) cudaEventRecord(mid, h->stream);
   const long long fs = P.fstride;
+  {
+    using V = VTile<TWO_D>;
+    constexpr size_t vsmem = vtile_smem_bytes<TWO_D, VISC>();
+    auto vkern = velocity_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1>;
+    static bool configured = false;      // one attribute call per instantiation (single device per process)
+    if (!configured) {
+      cudaError_t e = cudaFuncSetAttribute(vkern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vsmem);
+      if (e != cudaSuccess) return e;
+      configured = true;
+    }
+    dim3 grid((P.nx + V::VX - 1) / V::VX, (P.ny + V::VY - 1) / V::VY, ((P.nz + V::VZ - 1) / V::VZ) * P.n_batch);
+    VelTileArgs VA{S.e_in, h->vL, h->vR, S.cnt, S.t, (int)((S.q_in - h->pool) / fs)};
+    vkern<<<grid, V::NT, vsmem, h->stream>>>(P, VA, h->mapVA, h->mapVZ);
+    h->launches++;
+    cudaError_t e = debug_sync(h, "velocity tile kernel");
+    if (e != cudaSuccess) return e;
+  }
+  if (mid) cudaEventRecord(mid, h->stream);
   TileArgs A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post,
              (int)((S.q_in - h->pool) / fs), (int)((S.u_in - h->pool) / fs), (int)((S.p_in - h->pool) / fs)};
   return (stage == 1) ? launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1>(h, A) : launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2>(h, A);
