@@ -4,7 +4,7 @@
 // One CTA per VX x VY x VZ tile, one thread per cell.  Thread 0 issues, for each of the NV fields, one tensor-map box of the
 // tile with a 1-cell halo in y (and the 2-cell halo in x that the 16-byte start alignment of a box forces) plus, in 3+1d, one
 // plane below and one above the tile; all loads complete on ONE mbarrier, so the CTA waits once and then works from shared
-// memory only.  With 4-5 KB per field, four CTAs are resident per SM and hide one another's load latency (the register-file
+// memory only.  With 3-5 KB per field several CTAs are resident per SM and hide one another's load latency (the register-file
 // limit of the 64-register kernel is four 256-thread CTAs as well).  Arithmetic as in velocity_kernel (vh_kernels2.cuh): per
 // direction the two reconstructed states the cell owns are inverted once, as a pair (Eqs. 63-66, 72; Alg. 3 :667-672).
 #pragma once
@@ -36,7 +36,7 @@ struct VelTileArgs {
 };
 
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
-__global__ void __launch_bounds__(VTile<TWO_D>::NT, 4)
+__global__ void __launch_bounds__(VTile<TWO_D>::NT, 3)
     velocity_tile_kernel(const __grid_constant__ DevParams P, const __grid_constant__ VelTileArgs A, const __grid_constant__ CUtensorMap mapVA,
                          const __grid_constant__ CUtensorMap mapVZ) {
   using T = VTile<TWO_D>;
