@@ -30,8 +30,8 @@ UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_UPDATE = 856.0      # 107 doubles per cell-update, each state array read/written once per stage
 ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the stage kernel at 128^3 from the committed ncu --set full
-# capture (profiles/r01_ncu_summary.md); None for launches that were not captured
-NCU_TRAFFIC_BYTES = {"stage1": None, "stage2": None}
+# capture (profiles/r01c_ncu_summary.md); valid for the default workload (128^3) only
+NCU_TRAFFIC_BYTES = {"stage1": 629398272 + 358963712, "stage2": 928041984 + 359040768}      # profiles/r01c_ncu_summary.md
 
 
 def workload(rank=0):
@@ -56,52 +56,98 @@ def aggregate_value(ncell_per_rank, steps, world, seconds):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """SM clock, power and throttle reasons sampled WHILE the timed region runs: NVML polled every ~2 ms from a thread (the timed
+    region of a short run is far shorter than nvidia-smi's polling period); falls back to `nvidia-smi -lms 20` without pynvml."""
+    REASONS = (("hw_slowdown", "HwSlowdown"), ("hw_thermal_slowdown", "HwThermalSlowdown"), ("sw_thermal_slowdown", "SwThermalSlowdown"),
+               ("sw_power_cap", "SwPowerCap"))
     Q = "index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, gpu_index):
         self.gpu = gpu_index
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
-        self.p = None
+        self.sm, self.power, self.reasons = [], [], set()
+        self.sm_max = None
+        self.stop_flag = threading.Event()
+        self.thread = None
+        self.proc = None
+        self.file = None
+        self.nvml = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = gpu_index
+            if vis:
+                ids = [x.strip() for x in vis.split(",") if x.strip()]
+                if gpu_index < len(ids) and ids[gpu_index].isdigit():
+                    phys = int(ids[gpu_index])
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
+
+    def _poll(self):
+        nv = self.nvml
+        while not self.stop_flag.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.handle, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.handle) / 1000.0)
+                mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.handle)
+                for name, suffix in self.REASONS:
+                    if mask & getattr(nv, "nvmlClocksEventReason" + suffix):
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
 
     def start(self):
+        if self.nvml is not None:
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"],
-                                      stdout=self.f, stderr=subprocess.DEVNULL)
+            self.file = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "20"],
+                                         stdout=self.file, stderr=subprocess.DEVNULL)
         except Exception:
-            self.p = None
+            self.proc = None
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.p is None:
-            return out
-        self.p.terminate()
-        try:
-            self.p.wait(timeout=5)
-        except Exception:
-            self.p.kill()
-        self.f.flush()
-        self.f.seek(0)
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.f.read().splitlines():
-            c = [x.strip() for x in line.split(",")]
-            if len(c) < 9:
-                continue
+        out = {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0, "power_w_max": None, "source": "nvml" if self.nvml else "nvidia-smi"}
+        if self.thread is not None:
+            self.stop_flag.set()
+            self.thread.join(timeout=2)
+        elif self.proc is not None:
+            self.proc.terminate()
             try:
-                sm.append(float(c[1])); mx.append(float(c[2]))
-            except ValueError:
-                continue
-            for nm, v in zip(names, c[5:9]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
-        try:
-            os.unlink(self.f.name)
-        except OSError:
-            pass
-        if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+            self.file.flush()
+            self.file.seek(0)
+            mx = []
+            for line in self.file.read().splitlines():
+                c = [x.strip() for x in line.split(",")]
+                if len(c) < 9:
+                    continue
+                try:
+                    self.sm.append(float(c[1])); mx.append(float(c[2])); self.power.append(float(c[3]))
+                except ValueError:
+                    continue
+                for (name, _), v in zip(self.REASONS, c[5:9]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(name)
+            try:
+                os.unlink(self.file.name)
+            except OSError:
+                pass
+            if mx:
+                self.sm_max = float(max(mx))
+        if self.sm:
+            out.update(sm_mhz=float(np.median(self.sm)), sm_max_mhz=self.sm_max, reasons=sorted(self.reasons), samples=len(self.sm),
+                       power_w_max=float(max(self.power)) if self.power else None)
         return out
 
 
@@ -284,7 +330,7 @@ def main():
         roof["frac"] = roof["achieved"] / roof["peak"]
         step_roof_s = max(flops_cu * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9))
         roof.update({
-            "traffic": NCU_TRAFFIC_BYTES.get(dom), "kernel": "stage_tile_kernel (%s)" % dom if not variant1 else "stage_cell_kernel (%s)" % dom,
+            "traffic": NCU_TRAFFIC_BYTES.get(dom) if (ncell == 128 ** 3 and not args.variant) else None, "kernel": "stage_tile_kernel (%s)" % dom if not variant1 else "stage_cell_kernel (%s)" % dom,
             "launch_ms": prof[dom],
             "peak_source": "FP64 FMA microbenchmark, same run (vh_measure_peaks)" if roof["bound"] == "alu" else hbm_src,
             "alg_flops_per_cell_update": flops_cu, "alg_flops_interface_inversions_per_cell_update": flops_inv_cu,
@@ -307,7 +353,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": E,
                     "what": "per step: vh_set_initial(host e,u,pi,Pi) + vh_step(1) + vh_get_fields(host q,e,p,u), pinned buffers"},
             "gpu_launches": int(launches),
-            "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"], "samples": clocks["samples"]},
+            "clocks": clocks,
             "roofline": roof,
             "status": {"n_inversion_failures": st["n_inversion_failures"], "n_nonfinite": st["n_nonfinite"], "min_reg_factor": st["min_reg_factor"]},
             "measured_peaks_same_run": {"copy_gbs": copy_gbs, "fp64_fma_gflops": fp64_gflops},

@@ -1,7 +1,7 @@
 // vh_kernels4.cuh -- default velocity kernel ("velocity tile"): the interface-state inversions of one Euler stage with the
 // nine fields that enter Eq. 72 (T^{tau mu}, pi^{tau mu}, Pi) staged in shared memory by TMA.
 //
-// One CTA per VX x VY x VZ tile, one thread per cell.  Thread 0 issues, for each of the NV fields, one tensor-map box of the
+// One CTA per VX x VY x VZ tile, one thread per cell.  Lane 0 of each warp issues, for one of the NV fields, one tensor-map box of the
 // tile with a 1-cell halo in y (and the 2-cell halo in x that the 16-byte start alignment of a box forces) plus, in 3+1d, one
 // plane below and one above the tile; all loads complete on ONE mbarrier, so the CTA waits once and then works from shared
 // memory only.  With 3-5 KB per field several CTAs are resident per SM and hide one another's load latency (the register-file
@@ -62,8 +62,13 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, 3)
     mbar_init(full, 1);
     fence_mbar_init();
     mbar_arrive_expect_tx(full, (unsigned)(NV * (T::A_SIZE + 2 * T::Z_SIZE) * sizeof(double)));      // the bytes the boxes deliver (SLOT is padded)
+  }
+  const double guess = A.e[c];
+  __syncthreads();                 // the barrier is initialised and armed before anybody issues a load or waits on it
+  // lane 0 of every warp issues the boxes of one field (warp 0 also those of the ninth): the loads start in parallel
+  if ((tid & 31) == 0) {
 #pragma unroll 1
-    for (int m = 0; m < NV; ++m) {
+    for (int m = tid >> 5; m < NV; m += T::NT / 32) {
       const int arr = A.a_q + ((m < 4) ? m : ((m < 8) ? PTT + (m - 4) : BPI));
       double* dst = slots + m * T::SLOT;
       // padded coordinates: physical cell (i0, j0, k0) sits at (i0+2, j0+2, k0+zoff)
@@ -74,8 +79,6 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, 3)
       }
     }
   }
-  const double guess = A.e[c];
-  __syncthreads();                 // the barrier initialisation is visible to every waiter
 
   // offsets into a field's slot: centre, and the two eta neighbours (box A, or a halo plane at the tile faces)
   const int oc = (tz * AY + (ty + 1)) * AX + (tx + 2);
