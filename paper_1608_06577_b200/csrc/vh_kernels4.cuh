@@ -4,8 +4,8 @@
 // One CTA per VX x VY x VZ tile, one thread per cell.  Lane 0 of each warp issues, for one of the NV fields, one tensor-map box of the
 // tile with a 1-cell halo in y (and the 2-cell halo in x that the 16-byte start alignment of a box forces) plus, in 3+1d, one
 // plane below and one above the tile; all loads complete on ONE mbarrier, so the CTA waits once and then works from shared
-// memory only.  With 3-5 KB per field several CTAs are resident per SM and hide one another's load latency (the register-file
-// limit of the 64-register kernel is four 256-thread CTAs as well).  Arithmetic as in velocity_kernel (vh_kernels2.cuh): per
+// memory only.  With 3-4 KB per field six 128-thread CTAs (3+1d) are resident per SM and hide one another's load latency.
+// Arithmetic as in velocity_kernel (vh_kernels2.cuh): per
 // direction the two reconstructed states the cell owns are inverted once, as a pair (Eqs. 63-66, 72; Alg. 3 :667-672).
 #pragma once
 #include "vh_kernels3.cuh"
@@ -15,13 +15,13 @@ namespace vh {
 template <bool TWO_D> struct VTile {
   static constexpr int VX = 32;
   static constexpr int VY = TWO_D ? 8 : 4;
-  static constexpr int VZ = TWO_D ? 1 : 2;
-  static constexpr int NT = VX * VY * VZ;                       // 256 threads
+  static constexpr int VZ = 1;                                  // one eta plane per CTA: small CTAs, many per SM
+  static constexpr int NT = VX * VY * VZ;                       // 128 threads (3+1d), 256 (2+1d)
   static constexpr int AX = VX + 4, AY = VY + 2;
   static constexpr int A_SIZE = AX * AY * VZ;                   // doubles in box A (tile + halo in x, y)
   static constexpr int Z_SIZE = TWO_D ? 0 : VX * VY;            // doubles in one eta-halo plane
-  static constexpr int SLOT = (A_SIZE + 2 * Z_SIZE + 15) / 16 * 16;   // doubles per field, every TMA destination 128-byte aligned (3+1d: 688; 2+1d: 368)
-  static_assert(A_SIZE % 16 == 0 || TWO_D, "box Z destinations must stay 128-byte aligned");
+  static constexpr int A_PAD = (A_SIZE + 15) / 16 * 16;         // offset of the eta-halo planes: every TMA destination 128-byte aligned
+  static constexpr int SLOT = (A_PAD + 2 * Z_SIZE + 15) / 16 * 16;   // doubles per field
 };
 template <bool TWO_D, bool VISC> constexpr size_t vtile_smem_bytes() {
   return (size_t)((VISC ? 9 : 4) * VTile<TWO_D>::SLOT) * sizeof(double) + sizeof(uint64_t);
@@ -36,7 +36,7 @@ struct VelTileArgs {
 };
 
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
-__global__ void __launch_bounds__(VTile<TWO_D>::NT, 3)
+__global__ void __launch_bounds__(VTile<TWO_D>::NT, TWO_D ? 3 : 6)
     velocity_tile_kernel(const __grid_constant__ DevParams P, const __grid_constant__ VelTileArgs A, const __grid_constant__ CUtensorMap mapVA,
                          const __grid_constant__ CUtensorMap mapVZ) {
   using T = VTile<TWO_D>;
@@ -74,8 +74,8 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, 3)
       // padded coordinates: physical cell (i0, j0, k0) sits at (i0+2, j0+2, k0+zoff)
       tma_load_5d(dst, &mapVA, full, i0, j0 + 1, TWO_D ? 0 : k0 + 2, b, arr);
       if (!TWO_D) {
-        tma_load_5d(dst + T::A_SIZE, &mapVZ, full, i0 + 2, j0 + 2, k0 + 1, b, arr);                   // plane k0-1
-        tma_load_5d(dst + T::A_SIZE + T::Z_SIZE, &mapVZ, full, i0 + 2, j0 + 2, k0 + 2 + VZ, b, arr);   // plane k0+VZ
+        tma_load_5d(dst + T::A_PAD, &mapVZ, full, i0 + 2, j0 + 2, k0 + 1, b, arr);                   // plane k0-1
+        tma_load_5d(dst + T::A_PAD + T::Z_SIZE, &mapVZ, full, i0 + 2, j0 + 2, k0 + 2 + VZ, b, arr);   // plane k0+VZ
       }
     }
   }
@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, 3)
   const int oc = (tz * AY + (ty + 1)) * AX + (tx + 2);
   int ozm = oc, ozp = oc;
   if (!TWO_D) {
-    const int zl = T::A_SIZE + ty * VX + tx;
+    const int zl = T::A_PAD + ty * VX + tx;
     ozm = (tz >= 1) ? oc - AX * AY : zl;
     ozp = (tz + 1 < VZ) ? oc + AX * AY : zl + T::Z_SIZE;
   }
