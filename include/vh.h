@@ -47,7 +47,8 @@ typedef struct {
   int eos;                          /* 0: p = e/3;  1: p = (e/3)(1 - alpha exp(-e/e0));  T = (e/a)^{1/4} for both          */
   double eos_a, eos_alpha, eos_e0;
   double eta_over_s;                /* constant                                                                         */
-  int zeta_model;                   /* 0: zeta/s = 0; 1: amp*exp(-((T-T0)/width)^2) (BASELINE configs 3-5); 2: constant   */
+  int zeta_model;                   /* 0: zeta/s = 0; 1: amp*exp(-((T-T0)/width)^2) (BASELINE configs 3-5); 2: constant;  */
+                                    /* 3: Eq. 17 (:174-186) times (zeta/s)_norm = zeta_amp with T_c = zeta_T0 (paper: 0.2 GeV) */
   double zeta_amp, zeta_T0, zeta_width;  /* T0, width in fm^-1                                                            */
   double c_tau_pi;                  /* tau_pi = c_tau_pi*eta/(e+p); Eq. 13 -> 5                                          */
   double c_tau_Pi;                  /* tau_Pi = c_tau_Pi*zeta/((e+p)(1/3-cs2)^2); configs 5, Eq. 10 -> 1/15              */

@@ -48,7 +48,7 @@ struct Params {
   int eos;                     // 0: p=e/3; 1: p=(e/3)(1-alpha*exp(-e/e0)); T=(e/a)^(1/4)
   double eos_a, eos_alpha, eos_e0;
   double eta_over_s;
-  int zeta_model;              // 0: zeta/s=0; 1: Gaussian amp*exp(-((T-T0)/width)^2); 2: constant amp
+  int zeta_model;              // 0: zeta/s=0; 1: Gaussian amp*exp(-((T-T0)/width)^2); 2: constant amp; 3: Eq. 17 x amp, T_c = T0
   double zeta_amp, zeta_T0, zeta_width;     // T0, width in fm^-1 (R13)
   double c_tau_pi;             // tau_pi = c_tau_pi*eta/(e+p)                 (Eq. 13 -> 5)
   double c_tau_Pi;             // tau_Pi = c_tau_Pi*zeta/((e+p)(1/3-cs2)^2)   (configs 5; Eq. 10 -> 1/15)
@@ -116,6 +116,13 @@ template <class R> inline Transport<R> transport(const Params& P, R e, const The
     zs = R(P.zeta_amp) * exp(-d * d);
   } else if (P.zeta_model == 2) {
     zs = R(P.zeta_amp);
+  } else if (P.zeta_model == 3) {
+    // Eq. 17 (:174-186) times (zeta/s)_norm = zeta_amp, x = T/T_c with T_c = zeta_T0; ranges T < 0.995 T_c, in between, T > 1.05 T_c (R3)
+    R x = th.T / R(P.zeta_T0);
+    if (x > R(1.05)) zs = R(0.9) * exp(-(x - R(1)) / R(0.025)) + R(0.25) * exp(-(x - R(1)) / R(0.13)) + R(0.001);
+    else if (x < R(0.995)) zs = R(0.9) * exp((x - R(1)) / R(0.0025)) + R(0.22) * exp((x - R(1)) / R(0.022)) + R(0.03);
+    else zs = R(-13.45) + R(27.55) * x + R(-13.77) * x * x;
+    zs = R(P.zeta_amp) * zs;
   }
   R b = R(1) / R(3) - th.cs2;
   R it = (zs > R(0)) ? th.T * b * b / (R(P.c_tau_Pi) * zs) : inf;

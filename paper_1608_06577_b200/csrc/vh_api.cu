@@ -45,7 +45,7 @@ static int fill_dev_params(const vh_params& p, DevParams& P) {
   P.inv_ctaupi_etas = 1.0 / (p.c_tau_pi * p.eta_over_s);
   P.inv_ctaupi = 1.0 / p.c_tau_pi;
   P.zeta_model = p.zeta_model; P.zeta_amp = p.zeta_amp; P.zeta_T0 = p.zeta_T0;
-  P.zeta_inv_width = (p.zeta_model == 1) ? 1.0 / p.zeta_width : 0.0;
+  P.zeta_inv_width = (p.zeta_model == 1) ? 1.0 / p.zeta_width : ((p.zeta_model == 3) ? 1.0 / p.zeta_T0 : 0.0);      // model 3: 1/T_c
   P.inv_ctauPi = 1.0 / p.c_tau_Pi;
   P.delta_pipi = p.delta_pipi; P.tau_pipi = p.tau_pipi; P.lambda_piPi = p.lambda_piPi;
   P.delta_PiPi = p.delta_PiPi; P.lambda_Pipi_coef = p.lambda_Pipi_coef;
@@ -69,7 +69,8 @@ static int check_params(const vh_params* p, std::string& why) {
   if (!(p->eos_a > 0)) { why = "eos_a must be > 0"; return -1; }
   if (p->eos == 1 && !(p->eos_e0 > 0)) { why = "eos_e0 must be > 0"; return -1; }
   if (p->physics != 0 && !(p->eta_over_s > 0 && p->c_tau_pi > 0 && p->c_tau_Pi > 0)) { why = "eta_over_s, c_tau_pi, c_tau_Pi must be > 0"; return -1; }
-  if (p->zeta_model < 0 || p->zeta_model > 2) { why = "zeta_model must be 0, 1 or 2"; return -1; }
+  if (p->zeta_model < 0 || p->zeta_model > 3) { why = "zeta_model must be 0, 1, 2 or 3"; return -1; }
+  if (p->zeta_model == 3 && !(p->zeta_T0 > 0 && p->zeta_amp >= 0)) { why = "zeta_model 3 (Eq. 17) needs zeta_T0 = T_c > 0 and zeta_amp = (zeta/s)_norm >= 0"; return -1; }
   if (p->zeta_model == 1 && !(p->zeta_width > 0)) { why = "zeta_width must be > 0"; return -1; }
   if (!(p->minmod_theta >= 1.0 && p->minmod_theta <= 2.0)) { why = "minmod_theta must lie in [1,2] (Eq. 67)"; return -1; }
   if (!(p->rho_max > 0 && p->xi0 > 0)) { why = "xi0, rho_max must be > 0"; return -1; }

@@ -75,6 +75,24 @@ template <int EOS> __device__ __forceinline__ double eos_p(const DevParams& P, d
   return p;
 }
 
+// ---------------------------------------------------------------- zeta/s(T)
+// zeta_model 0: none; 1: Gaussian amp exp(-((T - T0)/width)^2) (BASELINE.json configs 3-5); 2: constant amp;
+// 3: the paper's parametrisation, Eq. 17 (:174-186), times (zeta/s)_norm = zeta_amp, with T_c = zeta_T0 and the ranges read as
+//    T < 0.995 T_c, 0.995 T_c <= T <= 1.05 T_c, T > 1.05 T_c (the printed inequalities are reversed, reading R3).
+__device__ __forceinline__ double zeta_over_s(const DevParams& P, double T) {
+  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; return P.zeta_amp * exp_neg(d * d); }
+  if (P.zeta_model == 2) return P.zeta_amp;
+  if (P.zeta_model == 3) {
+    const double x = T * P.zeta_inv_width;      // T / T_c (zeta_inv_width holds 1/T_c for this model)
+    double z;
+    if (x > 1.05) z = 0.9 * exp_neg((x - 1.0) * (1.0 / 0.025)) + 0.25 * exp_neg((x - 1.0) * (1.0 / 0.13)) + 0.001;
+    else if (x < 0.995) z = 0.9 * exp_neg((1.0 - x) * (1.0 / 0.0025)) + 0.22 * exp_neg((1.0 - x) * (1.0 / 0.022)) + 0.03;
+    else z = -13.45 + x * (27.55 - 13.77 * x);
+    return P.zeta_amp * z;
+  }
+  return 0.0;
+}
+
 // ---------------------------------------------------------------- Newton-Raphson on Eq. 72 (R6)
 // returns e; fail is set when no acceptable root was found (then e = max(E, tiny)).
 template <int EOS> __device__ __forceinline__ double invert_energy(const DevParams& P, double E, double M2, double Pi, double guess, bool& fail) {
@@ -190,9 +208,7 @@ __device__ __forceinline__ void dissipative_sources(const DevParams& P, double t
   double T = sqrt(sqrt(e * P.eos_a_inv));
   double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
   double eotp = (e + p) * P.inv_ctaupi;
-  double zs = 0.0;
-  if (P.zeta_model == 1) { double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp_neg(d * d); }
-  else if (P.zeta_model == 2) zs = P.zeta_amp;
+  const double zs = zeta_over_s(P, T);
   double b = (1.0 / 3.0) - cs2;
   double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi / zs : CUDART_INF;
   itP = fmin(itP, P.relax_clamp);

@@ -238,9 +238,7 @@ __device__ __forceinline__ void dissipative_sources2(const DevParams& P, double 
   const double T = sqrt_fast(sqrt_fast(e * P.eos_a_inv));
   const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
   const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
-  double zs = 0.0;
-  if (P.zeta_model == 1) { const double d = (T - P.zeta_T0) * P.zeta_inv_width; zs = P.zeta_amp * exp_neg(d * d); }
-  else if (P.zeta_model == 2) zs = P.zeta_amp;
+  const double zs = zeta_over_s(P, T);
   const double b = (1.0 / 3.0) - cs2;
   double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi / zs : CUDART_INF;
   itP = fmin(itP, P.relax_clamp);

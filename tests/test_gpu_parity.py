@@ -113,6 +113,18 @@ def test_shear_only_and_bulk_only(vh, vo, physics):
     assert_parity(fo, so, fg, sg)
 
 
+def test_zeta_over_s_of_eq17(vh, vo):
+    # SURVEY 8(f) NEXT-1 (first half): the paper's own zeta/s(T), Eq. 17; T_c = 180 MeV (footnote 1, :188) puts the state's
+    # temperatures on both sides of the quadratic piece
+    prm = inputs.base_params(nx=36, ny=12, nz=6, tau0=0.6, dtau=0.02, zeta_model=3, zeta_amp=1.0, zeta_T0=0.18 / inputs.HBARC)
+    st = inputs.smooth_random_state(prm, seed=31)
+    T = (st["e"] / prm["eos_a"]) ** 0.25 * inputs.HBARC
+    assert T.min() < 0.995 * 0.18 and T.max() > 1.05 * 0.18      # all three branches of Eq. 17 are exercised
+    fo, so, fg, sg = run_both(vh, vo, prm, st, 10)
+    assert np.max(np.abs(fo["q"][14])) > 0
+    assert_parity(fo, so, fg, sg)
+
+
 def test_batched_2plus1d_events(vh, vo):
     # BASELINE configs[3] physics: independent 2+1d events in one launch; ragged in x and y
     prm, init, _ = inputs.config_batched2d(n_batch=3, n=45, n_hot=5, seed=inputs.BASE_SEED, radius=1.8)

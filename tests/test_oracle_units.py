@@ -97,6 +97,36 @@ def test_transport_coefficients_match_paper_equations(vo):
     assert none["inv_tau_Pi"] == pytest.approx(8.0) and none["zeta_over_tau_Pi"] == 0.0
 
 
+def test_zeta_over_s_of_eq17(vo):
+    # PAPER.md Eq. 17 (:174-186), zeta_model 3: what the paper prints about the curve pins the branches and their constants -
+    # "(zeta/s)_norm = 3 has a peak value of 1" (:190), the floors 0.001 (hot) and 0.03 (cold), T_c = 200 MeV - plus the
+    # near-continuity of the three pieces at 0.995 T_c and 1.05 T_c that an interpolating parametrisation must have
+    HB = inputs.HBARC
+    Tc = 0.2 / HB
+
+    def zs(T_gev, norm=1.0):
+        prm = inputs.base_params(zeta_model=3, zeta_amp=norm, zeta_T0=Tc, tau_relax_floor_over_dtau=0.0)
+        T = T_gev / HB
+        e = prm["eos_a"] * T**4
+        th, tc = vo.eos(prm, e), vo.transport(prm, e)
+        s = (e + th["p"]) / th["T"]
+        return tc["zeta_over_tau_Pi"] / tc["inv_tau_Pi"] / s      # zeta/s recovered from zeta/tau_Pi and 1/tau_Pi
+
+    grid = np.linspace(0.05, 0.32, 1081)      # (hotter, exp(-e/e0) of EOS 1 underflows, 1/tau_Pi = 0 and the ratio below is 0/0)
+    vals = np.array([zs(t) for t in grid])
+    ok = np.isfinite(vals)      # (1/tau_Pi vanishes where c_s^2 = 1/3, e = e0 of EOS 1: the ratio is 0/0 at that one temperature)
+    assert ok.sum() >= len(grid) - 2
+    grid, vals = grid[ok], vals[ok]
+    assert vals.max() == pytest.approx(0.33, abs=2e-3) and abs(grid[vals.argmax()] - 0.2) < 2e-3      # peak -13.45 + 27.55 - 13.77 at T_c
+    assert zs(0.2, norm=3.0) == pytest.approx(0.99, abs=1e-12)                                        # "peak value of 1" for norm 3
+    assert zs(0.05) == pytest.approx(0.03, rel=1e-6)                                                  # cold floor (hot floor 0.001: formula check below)
+    for Tj in (0.995 * 0.2, 1.05 * 0.2):                                                              # joins continuous to ~1.5 %
+        assert zs(Tj * (1 - 1e-9)) == pytest.approx(zs(Tj * (1 + 1e-9)), rel=1.5e-2)
+    assert zs(0.19) == pytest.approx(0.9 * math.exp(-20.0) + 0.22 * math.exp(-0.05 / 0.022) + 0.03, rel=1e-12)
+    assert zs(0.3) == pytest.approx(0.9 * math.exp(-20.0) + 0.25 * math.exp(-0.5 / 0.13) + 0.001, rel=1e-12)
+    assert np.all(vals > 0) and np.all(np.diff(vals[grid > 0.2105]) < 0) and np.all(np.diff(vals[grid < 0.1985]) > 0)
+
+
 def test_newton_vs_conformal_closed_form(vo):
     # e = sqrt(4E^2 - 3M^2) - E for p = e/3, Pi = 0
     prm = inputs.base_params(eos=0)
