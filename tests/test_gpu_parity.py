@@ -305,3 +305,78 @@ def test_full_size_config3_sampled_subboxes(vh, vo):
         for m in range(4):
             worst = max(worst, np.max(np.abs(fo["u"][m][0][sl] - fg["u"][m][0][gl])) / max(np.max(np.abs(fo["u"][m])), NOISE))
     assert worst <= TOL, worst
+
+
+def _subbox_worst(vo, prm, init, fg, boxes, B, H, n_steps):
+    """Oracle on sub-boxes cut out of the same initial data; compares the inner cells (H cells away from every cut face that is not
+    a domain boundary) with the GPU fields fg (numpy arrays or CUDA tensors of the full grid).  Returns the worst R18 error."""
+    nz, ny, nx = prm["nz"], prm["ny"], prm["nx"]
+    worst = 0.0
+    for (x0, y0, z0) in boxes:
+        bz = min(B, nz)
+        sub = dict(prm, nx=B, ny=B, nz=bz, n_batch=1)
+        cut = lambda a: np.ascontiguousarray(a[..., 0:1, z0:z0 + bz, y0:y0 + B, x0:x0 + B])
+        o = vo.Oracle(sub)
+        o.set_initial(cut(init["e"]), cut(init["u"]))
+        o.step(n_steps)
+        fo = o.get_fields()
+        lo = lambda c0: 0 if c0 == 0 else H
+        hi = lambda c0, n, b: b if c0 + b == n else b - H
+        sl = (slice(lo(z0), hi(z0, nz, bz)), slice(lo(y0), hi(y0, ny, B)), slice(lo(x0), hi(x0, nx, B)))
+        gl = (slice(z0 + sl[0].start, z0 + sl[0].stop), slice(y0 + sl[1].start, y0 + sl[1].stop), slice(x0 + sl[2].start, x0 + sl[2].stop))
+        g = lambda t: np.asarray(t[gl].cpu()) if hasattr(t, "cpu") else t[gl]
+        S = np.max(np.abs(fo["q"][0]))
+        for n in range(15):
+            worst = max(worst, np.max(np.abs(fo["q"][n][0][sl] - g(fg["q"][n][0]))) / max(np.max(np.abs(fo["q"][n])), NOISE * S))
+        worst = max(worst, np.max(np.abs(fo["e"][0][sl] - g(fg["e"][0]))) / np.max(np.abs(fo["e"])))
+        for m in range(4):
+            worst = max(worst, np.max(np.abs(fo["u"][m][0][sl] - g(fg["u"][m][0]))) / max(np.max(np.abs(fo["u"][m])), NOISE))
+    return worst
+
+
+def test_full_size_config4_sampled_events(vh, vo):
+    """BASELINE configs[3] at its full size (256 events x 201 x 201 in ONE launch): 3 steps on the GPU; the oracle recomputes whole
+    sampled events (events are independent, so an event of the batch equals a single-event run of the same seed)."""
+    import torch
+    prm, init, _ = inputs.config_batched2d()
+    s = vh.Solver(prm)
+    s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+    s.step(3)
+    fg = s.get_fields()
+    sg = s.status()
+    assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
+    worst = 0.0
+    for b in (0, 1, 127, 255):
+        one = dict(prm, n_batch=1)
+        o = vo.Oracle(one)
+        o.set_initial(init["e"][b:b + 1], init["u"][:, b:b + 1])
+        o.step(3)
+        fo = o.get_fields()
+        S = np.max(np.abs(fo["q"][0]))
+        for n in range(15):
+            worst = max(worst, np.max(np.abs(fo["q"][n][0] - fg["q"][n][b].cpu().numpy())) / max(np.max(np.abs(fo["q"][n])), NOISE * S))
+        worst = max(worst, np.max(np.abs(fo["e"][0] - fg["e"][b].cpu().numpy())) / np.max(np.abs(fo["e"])))
+        for m in range(4):
+            worst = max(worst, np.max(np.abs(fo["u"][m][0] - fg["u"][m][b].cpu().numpy())) / max(np.max(np.abs(fo["u"][m])), NOISE))
+    s.close()
+    assert worst <= TOL, worst
+
+
+def test_full_size_config5_sampled_subboxes(vh, vo):
+    """BASELINE configs[4] at its full size (512 x 512 x 128, 19 GB of state): 2 steps on the GPU, sampled sub-boxes on the oracle
+    (domain of dependence of 2 steps: 8 cells).  The fields stay on the device; only the sampled boxes come back."""
+    import torch
+    prm, init, _ = inputs.config_large3d()
+    s = vh.Solver(prm)
+    s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+    s.step(2)
+    fg = s.get_fields()
+    sg = s.status()
+    assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
+    assert bool(torch.isfinite(fg["q"]).all()) and bool((fg["e"] > 0).all())
+    B, H = 24, 8
+    boxes = [(0, 0, 0), (488, 488, 104), (244, 250, 52), (300, 180, 70), (488, 0, 40), (100, 488, 0)]
+    worst = _subbox_worst(vo, prm, init, fg, boxes, B, H, 2)
+    s.close()
+    print("config 5 sampled sub-boxes: worst R18 error %.3e" % worst)
+    assert 0.0 < worst <= TOL, worst      # (> 0: the comparison is not vacuous - FMA contraction alone separates the two sides)
