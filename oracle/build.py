@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(HERE, "libvh_oracle.so")
 SRCS = [os.path.join(HERE, "vh_oracle_capi.cpp"), os.path.join(HERE, "vh_oracle_count.cpp")]
-DEPS = SRCS + [os.path.join(HERE, "vh_oracle.hpp")]
+DEPS = SRCS + [os.path.join(HERE, "vh_oracle.hpp"), os.path.join(HERE, "vh_oracle_lattice.hpp")]
 
 
 def build(force: bool = False) -> str:

@@ -31,6 +31,8 @@
 #include <limits>
 #include <vector>
 
+#include "vh_oracle_lattice.hpp"
+
 namespace vho {
 
 using std::exp; using std::pow; using std::sqrt; using std::tanh;
@@ -45,7 +47,7 @@ struct Params {
   double tau0, dtau;           // fm
   int geometry;                // 0 Milne, 1 Cartesian (ideal only, R12)
   int physics;                 // bit0 shear, bit1 bulk; 0 ideal
-  int eos;                     // 0: p=e/3; 1: p=(e/3)(1-alpha*exp(-e/e0)); T=(e/a)^(1/4)
+  int eos;                     // 0: p=e/3; 1: p=(e/3)(1-alpha*exp(-e/e0)), T=(e/a)^(1/4) for both; 2: lattice EOS (Eqs. 19-20), T(e) from its table
   double eos_a, eos_alpha, eos_e0;
   double eta_over_s;
   int zeta_model;              // 0: zeta/s=0; 1: Gaussian amp*exp(-((T-T0)/width)^2); 2: constant amp; 3: Eq. 17 x amp, T_c = T0
@@ -84,6 +86,12 @@ template <class R> inline Thermo<R> eos(const Params& P, R e) {
   if (P.eos == 0) {
     t.p = e / R(3);
     t.cs2 = R(1) / R(3);
+  } else if (P.eos == 2) {
+    // lattice EOS of section 2.3 (Eqs. 19-20): table + cubic Hermite interpolation, vh_oracle_lattice.hpp (evaluated in double)
+    double pp, cc, TT;
+    lattice::table().eval((double)e, pp, cc, TT);
+    t.p = R(pp);
+    t.cs2 = R(cc);
   } else {
     R x = e / R(P.eos_e0);
     R ex = exp(-x);
@@ -93,7 +101,10 @@ template <class R> inline Thermo<R> eos(const Params& P, R e) {
   t.T = R(0);     // filled by temperature() where it is needed (transport coefficients only)
   return t;
 }
-template <class R> inline R temperature(const Params& P, R e) { return pow(e / R(P.eos_a), R(0.25)); }   // e = a T^4
+template <class R> inline R temperature(const Params& P, R e) {
+  if (P.eos == 2) { double pp, cc, TT; lattice::table().eval((double)e, pp, cc, TT); return R(TT); }      // T(e) of the lattice EOS
+  return pow(e / R(P.eos_a), R(0.25));                                                                    // e = a T^4
+}
 
 template <class R> struct Transport {
   R inv_tau_pi, eta_over_tau_pi;        // 1/tau_pi, eta/tau_pi
