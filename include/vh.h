@@ -44,7 +44,8 @@ typedef struct {
   double tau0, dtau;                /* fm                                                                               */
   int geometry;                     /* 0 Milne (Eqs. 27-29); 1 Cartesian, ideal only: G terms off, tau^2 -> 1 (:684)      */
   int physics;                      /* bit0 shear pi^{mu nu}, bit1 bulk Pi; 0 = ideal (pi, Pi stay 0)                     */
-  int eos;                          /* 0: p = e/3;  1: p = (e/3)(1 - alpha exp(-e/e0));  T = (e/a)^{1/4} for both          */
+  int eos;                          /* 0: p = e/3;  1: p = (e/3)(1 - alpha exp(-e/e0));  T = (e/a)^{1/4} for both;         */
+                                    /* 2: lattice EOS of Eqs. 19-20 (:200-215) with T(e), c_s^2 from its table (DESIGN R19, R20) */
   double eos_a, eos_alpha, eos_e0;
   double eta_over_s;                /* constant                                                                         */
   int zeta_model;                   /* 0: zeta/s = 0; 1: amp*exp(-((T-T0)/width)^2) (BASELINE configs 3-5); 2: constant;  */

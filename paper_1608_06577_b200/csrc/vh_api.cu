@@ -1,5 +1,6 @@
 // vh_api.cu -- C ABI (include/vh.h): handle, buffers, buffer rotation (PAPER.md program-flow steps 7, 9), kernel dispatch.
 #include "vh_internal.cuh"
+#include "vh_eos_lattice.hpp"
 
 #include <cmath>
 #include <cstdio>
@@ -65,8 +66,8 @@ static int check_params(const vh_params* p, std::string& why) {
   if (p->geometry == 1 && p->physics != 0) { why = "Cartesian geometry supports ideal physics only (PAPER.md:684)"; return -1; }
   if (p->geometry == 0 && !(p->tau0 > 0)) { why = "Milne geometry needs tau0 > 0"; return -1; }
   if (p->physics < 0 || p->physics > 3) { why = "physics must be a combination of bit0 (shear) and bit1 (bulk)"; return -1; }
-  if (p->eos != 0 && p->eos != 1) { why = "eos must be 0 or 1"; return -1; }
-  if (!(p->eos_a > 0)) { why = "eos_a must be > 0"; return -1; }
+  if (p->eos < 0 || p->eos > 2) { why = "eos must be 0, 1 or 2"; return -1; }
+  if (p->eos != 2 && !(p->eos_a > 0)) { why = "eos_a must be > 0"; return -1; }
   if (p->eos == 1 && !(p->eos_e0 > 0)) { why = "eos_e0 must be > 0"; return -1; }
   if (p->physics != 0 && !(p->eta_over_s > 0 && p->c_tau_pi > 0 && p->c_tau_Pi > 0)) { why = "eta_over_s, c_tau_pi, c_tau_Pi must be > 0"; return -1; }
   if (p->zeta_model < 0 || p->zeta_model > 3) { why = "zeta_model must be 0, 1, 2 or 3"; return -1; }
@@ -84,13 +85,16 @@ static int check_params(const vh_params* p, std::string& why) {
 // one Euler stage with the handle's kernel variant: the launch units are compiled per (EOS, viscous, Milne) combination
 static cudaError_t launch_stage_any(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
   const int phys = (h->prm.physics != 0) ? 0 : ((h->prm.geometry == 0) ? 1 : 2);
-  switch (h->prm.eos + 2 * phys) {
+  switch (h->prm.eos + 3 * phys) {
     case 0: return vh_launch_stage_combo0(h, stage, A, mid);
     case 1: return vh_launch_stage_combo1(h, stage, A, mid);
     case 2: return vh_launch_stage_combo2(h, stage, A, mid);
     case 3: return vh_launch_stage_combo3(h, stage, A, mid);
     case 4: return vh_launch_stage_combo4(h, stage, A, mid);
-    default: return vh_launch_stage_combo5(h, stage, A, mid);
+    case 5: return vh_launch_stage_combo5(h, stage, A, mid);
+    case 6: return vh_launch_stage_combo6(h, stage, A, mid);
+    case 7: return vh_launch_stage_combo7(h, stage, A, mid);
+    default: return vh_launch_stage_combo8(h, stage, A, mid);
   }
 }
 
@@ -182,6 +186,21 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
     cudaFree(h->pool); cudaFree(h->cnt); delete h;
     return fail(nullptr, VH_ERR_CUDA, msg);
   }
+  if (p->eos == 2) {      // lattice EOS: build the table on the host (milliseconds), keep it in global memory
+    const vh_eos::LatticeTable tab = vh_eos::Builder().build();
+    const size_t tb = tab.node.size() * sizeof(double);
+    ce = cudaMalloc((void**)&h->eos_tab, tb);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(h->eos_tab, tab.node.data(), tb, cudaMemcpyHostToDevice, h->stream);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);      // tab lives on this stack frame
+    if (ce != cudaSuccess) { cudaFree(h->eos_tab); cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_ALLOC, "EOS table upload failed"); }
+    const int n = vh_eos::VH_EOS_N;
+    const double* nd = tab.node.data();
+    const double e0 = std::pow(tab.x0, 4), eN = std::pow(tab.xN, 4);
+    h->P.eos_tab = reinterpret_cast<const double2*>(h->eos_tab);
+    h->P.eos_n = n; h->P.eos_x0 = tab.x0; h->P.eos_xN = tab.xN; h->P.eos_inv_h = 1.0 / tab.h;
+    h->P.eos_lo_slope = nd[0] / e0; h->P.eos_pN = nd[4 * n]; h->P.eos_eN = eN;
+    h->P.eos_T0_over_x0 = nd[2] / tab.x0; h->P.eos_TN_over_xN = nd[4 * n + 2] / tab.xN;
+  }
   *out = h;
   return VH_OK;
 }
@@ -191,6 +210,7 @@ void vh_destroy(vh_handle* h) {
   cudaStreamSynchronize(h->stream);
   cudaFree(h->pool);
   cudaFree(h->cnt);
+  cudaFree(h->eos_tab);
   cudaFree(h->stage_in);
   cudaFree(h->stage_out);
   delete h;
@@ -243,7 +263,8 @@ int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double
     de = s; du = s + np; dpi = pi10 ? s + 5 * np : nullptr; dPi = Pi ? s + 15 * np : nullptr;
   }
   unsigned nb = (unsigned)((np + 255) / 256);
-  if (h->prm.eos) init_kernel<1><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
+  if (h->prm.eos == 2) init_kernel<2><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
+  else if (h->prm.eos == 1) init_kernel<1><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
   else init_kernel<0><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
   h->launches++;
   CUDA_TRY(h, cudaGetLastError());
@@ -279,7 +300,8 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
     h->launches++;
     CUDA_TRY(h, cudaGetLastError());
   }
-  if (h->prm.eos) pressure_kernel<1><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
+  if (h->prm.eos == 2) pressure_kernel<2><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
+  else if (h->prm.eos == 1) pressure_kernel<1><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
   else pressure_kernel<0><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
   h->launches++;
   CUDA_TRY(h, cudaGetLastError());

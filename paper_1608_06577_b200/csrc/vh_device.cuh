@@ -24,6 +24,8 @@ struct DevParams {
   double inv_dx, inv_dy, inv_dz, inv_dtau;
   int shear, bulk;              // physics bits
   double eos_a_inv, eos_alpha, eos_e0_inv;
+  // EOS 2 (lattice, Eqs. 19-20; R19, R20): table of kN + 1 nodes uniform in x = e^{1/4}, node k = (P, h dP/dx, T, h dT/dx)
+  const double2* eos_tab; int eos_n; double eos_x0, eos_xN, eos_inv_h, eos_lo_slope, eos_pN, eos_eN, eos_T0_over_x0, eos_TN_over_xN;
   double inv_ctaupi_etas;       // 1/(c_tau_pi * eta/s)
   double inv_ctaupi;            // 1/c_tau_pi
   int zeta_model; double zeta_amp, zeta_T0, zeta_inv_width, inv_ctauPi;
@@ -68,6 +70,33 @@ template <int EOS> __device__ __forceinline__ void eos_p_cs2(const DevParams& P,
     p = (e * (1.0 / 3.0)) * (1.0 - aex);
     cs2 = (1.0 / 3.0) * (1.0 - aex * (1.0 - x));
   }
+}
+// EOS 2: cubic Hermite interpolation in x = e^{1/4} of the tabulated lattice pressure and temperature (R20); c_s^2 is the
+// derivative of the pressure interpolant.  Below the table P = (P_0/e_0) e, T = (T_0/x_0) x; above it P = P_N + (e - e_N)/3.
+__device__ __forceinline__ void eos_lattice(const DevParams& P, double e, double& p, double& cs2, double& T) {
+  const double x = (e > 0.0) ? sqrt(sqrt(e)) : 0.0;            // (e <= 0 or NaN falls into the first branch)
+  if (!(x >= P.eos_x0)) { p = P.eos_lo_slope * e; cs2 = P.eos_lo_slope; T = P.eos_T0_over_x0 * x; return; }
+  if (x >= P.eos_xN) { p = fma(e - P.eos_eN, 1.0 / 3.0, P.eos_pN); cs2 = 1.0 / 3.0; T = P.eos_TN_over_xN * x; return; }
+  const double u = (x - P.eos_x0) * P.eos_inv_h;
+  const int k = min((int)u, P.eos_n - 1);
+  const double s = u - (double)k, s2 = s * s, s3 = s2 * s;
+  const double2 ap = __ldg(P.eos_tab + 2 * k), at = __ldg(P.eos_tab + 2 * k + 1), bp = __ldg(P.eos_tab + 2 * k + 2), bt = __ldg(P.eos_tab + 2 * k + 3);
+  const double h00 = 2.0 * s3 - 3.0 * s2 + 1.0, h10 = s3 - 2.0 * s2 + s, h01 = 3.0 * s2 - 2.0 * s3, h11 = s3 - s2;
+  p = h00 * ap.x + h10 * ap.y + h01 * bp.x + h11 * bp.y;
+  T = h00 * at.x + h10 * at.y + h01 * bt.x + h11 * bt.y;
+  const double d00 = 6.0 * (s2 - s), d10 = 3.0 * s2 - 4.0 * s + 1.0, d11 = 3.0 * s2 - 2.0 * s;
+  const double dpdx = (d00 * (ap.x - bp.x) + d10 * ap.y + d11 * bp.y) * P.eos_inv_h;
+  cs2 = dpdx / (4.0 * x * x * x);
+}
+template <> __device__ __forceinline__ void eos_p_cs2<2>(const DevParams& P, double e, double& p, double& cs2) {
+  double T;
+  eos_lattice(P, e, p, cs2, T);
+}
+// temperature for the transport coefficients: T = (e/a)^{1/4} for the analytic EOS, T(e) of the table for EOS 2
+template <int EOS> __device__ __forceinline__ double eos_temperature(const DevParams& P, double e) {
+  if (EOS == 2) { double p, c, T; eos_lattice(P, e, p, c, T); return T; }
+  const double y = e * P.eos_a_inv;
+  return sqrt(sqrt(y));
 }
 template <int EOS> __device__ __forceinline__ double eos_p(const DevParams& P, double e) {
   double p, c;
@@ -205,7 +234,7 @@ __device__ __forceinline__ void dissipative_sources(const DevParams& P, double t
   const double t2 = t * t, it = 1.0 / t;
   const double g[4] = {1.0, -1.0, -1.0, -t2};
   // transport coefficients (Eqs. 10-16; R14)
-  double T = sqrt(sqrt(e * P.eos_a_inv));
+  double T = eos_temperature<EOS>(P, e);
   double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
   double eotp = (e + p) * P.inv_ctaupi;
   const double zs = zeta_over_s(P, T);

@@ -24,6 +24,7 @@ struct vh_handle {
   double* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
   double* vR = nullptr;              // [3] ... high face
   vh::Counters* cnt = nullptr;
+  double* eos_tab = nullptr;         // EOS 2: the lattice table (vh_eos_lattice.hpp) in global memory
   double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
   double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
   long long n_steps = 0;
@@ -49,7 +50,8 @@ inline cudaError_t vh_debug_sync(vh_handle* h, const char* what) {
 }
 
 // One Euler stage (kernels of the handle's variant) for one combination of template parameters; defined in vh_launch.cu.
-// combo = eos + 2 * (0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian).  mid (optional) is recorded between the two launches.
+// combo = eos + 3 * (0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian), eos = 0, 1, 2.  mid (optional) is recorded between the two launches.
 #define VH_DECLARE_COMBO(K) cudaError_t vh_launch_stage_combo##K(vh_handle* h, int stage, const vh::StageArgs& A, cudaEvent_t mid);
 VH_DECLARE_COMBO(0) VH_DECLARE_COMBO(1) VH_DECLARE_COMBO(2) VH_DECLARE_COMBO(3) VH_DECLARE_COMBO(4) VH_DECLARE_COMBO(5)
+VH_DECLARE_COMBO(6) VH_DECLARE_COMBO(7) VH_DECLARE_COMBO(8)
 #undef VH_DECLARE_COMBO

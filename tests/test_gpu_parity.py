@@ -125,6 +125,25 @@ def test_zeta_over_s_of_eq17(vh, vo):
     assert_parity(fo, so, fg, sg)
 
 
+def test_lattice_eos_and_the_papers_own_physics(vh, vo):
+    # the lattice EOS of Eqs. 19-20 (eos = 2; both sides build the table of DESIGN.md R20 independently) with the
+    # zeta/s of Eq. 17 (T_c = 200 MeV): the physics of the paper's own benchmark (:840).  A generic all-terms state, then hotspots
+    prm = inputs.base_params(nx=36, ny=12, nz=6, tau0=0.6, dtau=0.02, eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC)
+    st = inputs.smooth_random_state(prm, seed=41)
+    fo, so, fg, sg = run_both(vh, vo, prm, st, 10)
+    assert so["n_inversion_failures"] == 0 and np.max(np.abs(fo["q"][14])) > 0
+    assert_parity(fo, so, fg, sg)
+    prm, init, _ = inputs.config_3d(40, 20, 8, n_hot=5, width=0.5, seed=inputs.BASE_SEED + 2, radius=1.5, eta_half=0.3,
+                                    eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, 10)
+    assert so["n_inversion_failures"] == 0 and np.max(np.abs(fo["u"][1:])) > 0.05
+    assert_parity(fo, so, fg, sg)
+    # ideal hydrodynamics with the lattice EOS (the instantiations without viscous terms)
+    prm, init, _ = inputs.config_3d(18, 14, 9, n_hot=3, width=0.4, seed=3, physics=0, eos=2, radius=0.6, eta_half=0.3)
+    fo, so, fg, sg = run_both(vh, vo, prm, init, 8)
+    assert_parity(fo, so, fg, sg)
+
+
 def test_batched_2plus1d_events(vh, vo):
     # BASELINE configs[3] physics: independent 2+1d events in one launch; ragged in x and y
     prm, init, _ = inputs.config_batched2d(n_batch=3, n=45, n_hot=5, seed=inputs.BASE_SEED, radius=1.8)
