@@ -34,8 +34,11 @@ ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
 NCU_TRAFFIC_BYTES = {"stage1": 629814528 + 361090048, "stage2": 928152576 + 360787456}      # profiles/r01c_ncu_summary.md
 
 
-def workload(rank=0):
-    prm, init, _ = inputs.config_3d(seed=inputs.BASE_SEED + rank)
+def workload(rank=0, physics="config3"):
+    """configs[2] of BASELINE.json (default); physics="paper": the same grid and hotspots with the paper's own equation of state
+    (lattice, Eqs. 19-20) and zeta/s(T) (Eq. 17, T_c = 200 MeV) - SURVEY 8(f) NEXT-1 - for a second, labelled bench line."""
+    over = dict(eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC) if physics == "paper" else {}
+    prm, init, _ = inputs.config_3d(seed=inputs.BASE_SEED + rank, **over)
     return prm, init
 
 
@@ -188,7 +191,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    prm, init = workload(0)
+    prm, init = workload(0, args.physics)
     dims = (64, 64, 32)
     warm = min(args.warmup, 1)
     value, dt, sample = time_oracle(prm, init, dims, args.steps, warmup=warm)
@@ -213,6 +216,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0, help="stage-kernel variant (vh_set_kernel_variant), 0 = default")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--physics", default="config3", choices=["config3", "paper"], help="paper: lattice EOS + Eq. 17 zeta/s on the config-3 grid")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -236,7 +240,7 @@ def main():
     W = max(args.warmup, 3)
     K = args.steps
 
-    prm, init = workload(rank)
+    prm, init = workload(rank, args.physics)
     ncell = prm["nx"] * prm["ny"] * prm["nz"] * prm["n_batch"]
     s = vh.Solver(prm, device=dev)
     if args.variant:
@@ -330,7 +334,7 @@ def main():
         roof["frac"] = roof["achieved"] / roof["peak"]
         step_roof_s = max(flops_cu * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9))
         roof.update({
-            "traffic": NCU_TRAFFIC_BYTES.get(dom) if (ncell == 128 ** 3 and not args.variant) else None, "kernel": "stage_tile_kernel (%s)" % dom if not variant1 else "stage_cell_kernel (%s)" % dom,
+            "traffic": NCU_TRAFFIC_BYTES.get(dom) if (ncell == 128 ** 3 and not args.variant and args.physics == "config3") else None, "kernel": "stage_tile_kernel (%s)" % dom if not variant1 else "stage_cell_kernel (%s)" % dom,
             "launch_ms": prof[dom],
             "peak_source": "FP64 FMA microbenchmark, same run (vh_measure_peaks)" if roof["bound"] == "alu" else hbm_src,
             "alg_flops_per_cell_update": flops_cu, "alg_flops_interface_inversions_per_cell_update": flops_inv_cu,
@@ -346,8 +350,10 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
-                                   "dtau=0.025, one independent replica per GPU (no sharding, no collective)",
+            "config": {"workload": ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
+                                    "dtau=0.025, one independent replica per GPU (no sharding, no collective)") if args.physics == "config3" else
+                                   ("configs[2] grid and hotspots with the paper's own physics: lattice EOS (Eqs. 19-20), zeta/s of Eq. 17 (T_c = 200 MeV), "
+                                    "eta/s=0.2; one independent replica per GPU"),
                        "l2": "state (61 arrays, 1.34 GB) exceeds the 126 MB L2; no flush needed", "kernel_variant": args.variant,
                        "paper_context": "GTX 980 Ti, FP32, lattice EOS: 244.45 ms/step = 8.58e6 cell-updates/s (PAPER.md Table 3; another machine, not a target)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": E,
