@@ -99,6 +99,19 @@ int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, d
 int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long* n_inversion_failures,
                   long long* n_nonfinite, double* min_reg_factor);
 
+/* On-device diagnostics of the current state, maxima over all physical cells and events, written to
+ * out6[0..5]:  [0] max T in fm^-1 (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  [1] max |u.u - 1| (:489);
+ * [2] max |g_{mu nu} pi^{mu nu}|/(e+p) and [3] max over lambda of |pi^{lambda mu} u_mu|/(e+p) (the constraints of Eqs. 47-51,
+ * :318-331, which are propagated, not enforced; the lambda = eta entry is multiplied by tau);  [4] max R_pi^-1 =
+ * sqrt(pi^{mu nu} pi_{mu nu})/P0 and [5] max R_Pi^-1 = |Pi|/P0 (inverse Reynolds numbers, Eq. 89, :826).  One reduction
+ * kernel; synchronises the stream.  out6 is a HOST pointer.                                                               */
+int vh_get_diagnostics(vh_handle* h, double* out6);
+
+/* Program-flow steps 6-8 (:492-494): advance until T < T_f (fm^-1) everywhere or max_steps steps have been taken, testing the
+ * temperature every check_every steps (>= 1) with the reduction of vh_get_diagnostics.  *steps_done (may be NULL) receives the
+ * number of steps taken by this call; returns VH_OK in both cases (compare vh_get_diagnostics()[0] with T_f to tell them apart). */
+int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long long* steps_done);
+
 /* Number of kernels launched on the handle since vh_create (for bench.py's gpu_launches).                             */
 long long vh_launch_count(vh_handle* h);
 

@@ -248,6 +248,39 @@ template <class R> class Solver {
     }
   }
 
+  // ------------------------------------------------------------ diagnostics, maxima over the physical cells
+  // out[0] max T (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  out[1] max |u.u - 1| (:489);
+  // out[2] max |g_{mu nu} pi^{mu nu}|/(e+p), out[3] max_lambda |pi^{lambda mu} u_mu|/(e+p) (Eqs. 47-51, :318-331; the lambda = eta
+  // entry times tau);  out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826)
+  void diagnostics(double out[6]) const {
+    for (int i = 0; i < 6; ++i) out[i] = 0.0;
+    const double t = (double)tau, t2 = (double)tau2(tau);
+    const double g[4] = {1.0, -1.0, -1.0, -t2};
+    for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i) {
+      const size_t s = idx(i, j, k);
+      const double ee = (double)e[s], pp = (double)p[s];
+      const double T = (double)temperature(P, e[s]);
+      double uu[4], pim[4][4];
+      for (int m = 0; m < 4; ++m) uu[m] = (double)u[m][s];
+      for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pim[m][n] = (double)q[PI_SLOT[m][n]][s];
+      double norm = 0.0, tr = 0.0, pipi = 0.0, orth = 0.0;
+      for (int m = 0; m < 4; ++m) { norm += g[m] * uu[m] * uu[m]; tr += g[m] * pim[m][m]; }
+      for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pipi += g[m] * g[n] * pim[m][n] * pim[m][n];
+      for (int l = 0; l < 4; ++l) {
+        double c = 0.0;
+        for (int m = 0; m < 4; ++m) c += pim[l][m] * g[m] * uu[m];
+        if (l == 3 && milne()) c *= t;
+        orth = std::fmax(orth, std::fabs(c));
+      }
+      out[0] = std::fmax(out[0], T);
+      out[1] = std::fmax(out[1], std::fabs(norm - 1.0));
+      out[2] = std::fmax(out[2], std::fabs(tr) / (ee + pp));
+      out[3] = std::fmax(out[3], orth / (ee + pp));
+      out[4] = std::fmax(out[4], std::sqrt(std::fabs(pipi)) / pp);
+      out[5] = std::fmax(out[5], std::fabs((double)q[14][s]) / pp);
+    }
+  }
+
   // ------------------------------------------------------------ ghost cells, Eqs. 75-76 (:459-466)
   void ghost_one(std::vector<R>& a) {
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) {

@@ -63,6 +63,7 @@ def lib():
         L.vho_get_fields.argtypes = [C.c_void_p, dp, dp, dp, dp, dp]
         L.vho_get_status.argtypes = [C.c_void_p, dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), dp]
         L.vho_last_failure.argtypes = [C.c_void_p, C.c_int, dp]
+        L.vho_diagnostics.argtypes = [C.c_void_p, dp]
         L.vho_raw.restype = dp
         L.vho_raw.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.vho_set_tau.argtypes = [C.c_void_p, C.c_double]
@@ -145,6 +146,11 @@ class Oracle:
         self.L.vho_get_status(self.h, C.byref(tau), C.byref(a), C.byref(b), C.byref(c), C.byref(mr))
         return {"tau": tau.value, "n_steps": a.value, "n_inversion_failures": b.value, "n_nonfinite": c.value, "min_reg_factor": mr.value}
 
+    def diagnostics(self):
+        out = np.empty(6)
+        self.L.vho_diagnostics(self.h, _dp(out))
+        return dict(zip(DIAG_NAMES, out))
+
     def last_failure(self, ev=0):
         out = np.empty(4)
         self.L.vho_last_failure(self.h, ev, _dp(out))
@@ -202,6 +208,7 @@ def invert(params: dict, E, M2, Pi, guess):
     return e, it.value, fl.value
 
 
+DIAG_NAMES = ("max_T", "max_norm_violation", "max_trace_violation", "max_transversality_violation", "max_inv_reynolds_shear", "max_inv_reynolds_bulk")
 OP_CLASSES = ("add", "mul", "div", "cmp", "sqrt", "exp", "pow", "tanh")
 # flop weights of SURVEY.md 8(d): add/mul/compare 1, div 10, sqrt 15, exp 25, tanh 40; pow(x, 1/4) = two sqrt
 OP_WEIGHTS = dict(add=1, mul=1, div=10, cmp=1, sqrt=15, exp=25, pow=30, tanh=40)

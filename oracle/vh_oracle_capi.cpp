@@ -70,6 +70,11 @@ int vho_get_status(vho_handle* h, double* tau, long long* n_steps, long long* n_
   return 0;
 }
 
+// maxima over all events of Solver::diagnostics (double instantiation only)
+void vho_diagnostics(vho_handle* h, double* out6) {
+  for (int i = 0; i < 6; ++i) out6[i] = 0.0;
+  for (Sol* s : h->ev) { double o[6]; s->diagnostics(o); for (int i = 0; i < 6; ++i) if (o[i] > out6[i]) out6[i] = o[i]; }
+}
 void vho_last_failure(vho_handle* h, int ev, double* out4) { for (int i = 0; i < 4; ++i) out4[i] = h->ev[ev]->last_fail[i]; }
 
 // ---- raw access to the padded arrays of one event, for unit pins.  which: 0 q 1 qS 2 Q 3 u 4 up 5 uS 6 e 7 p

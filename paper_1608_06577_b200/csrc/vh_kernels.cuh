@@ -395,6 +395,56 @@ __global__ void __launch_bounds__(256) pressure_kernel(const __grid_constant__ D
   p[c] = eos_p<EOS>(P, e[c]);
 }
 
+// ------------------------------------------------------------------------------------------------ diagnostics
+// Maxima over the physical cells, accumulated with atomicMax on the bit patterns (non-negative doubles order like integers):
+// out[0] max T (freeze-out test "T < T_f everywhere", program-flow step 8, :494); out[1] max |u.u - 1| (:489);
+// out[2] max |g_{mu nu} pi^{mu nu}|/(e+p), out[3] max_lambda |pi^{lambda mu} u_mu|/(e+p) (Eqs. 47-51, :318-331; lambda = eta entry
+// times tau); out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826).
+template <int EOS, bool MILNE>
+__global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant__ DevParams P, const double* __restrict__ q, const double* __restrict__ e,
+                                                          const double* __restrict__ p, const double* __restrict__ u, double t,
+                                                          unsigned long long* __restrict__ out) {
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  const long long fs = P.fstride;
+  const double t2 = MILNE ? t * t : 1.0;
+  double m[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < np; n += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(n % P.nx);
+    const int j = (int)((n / P.nx) % P.ny);
+    const int k = (int)((n / ((long long)P.nx * P.ny)) % P.nz);
+    const int b = (int)(n / ((long long)P.nx * P.ny * P.nz));
+    const long long c = (long long)b * P.bstride + (long long)(k + P.zoff) * P.plane + (long long)(j + 2) * P.NXp + (i + 2);
+    const double ee = e[c], pp = p[c];
+    const double ut = u[c], ux = u[fs + c], uy = u[2 * fs + c], un = u[3 * fs + c];
+    double pi[10];
+#pragma unroll
+    for (int s = 0; s < 10; ++s) pi[s] = q[(PTT + s) * fs + c];
+    const double Pi = q[BPI * fs + c];
+    const double norm = ut * ut - ux * ux - uy * uy - t2 * un * un;
+    const double tr = pi[0] - pi[4] - pi[7] - t2 * pi[9];
+    const double pipi = pi[0] * pi[0] - 2.0 * (pi[1] * pi[1] + pi[2] * pi[2] + t2 * pi[3] * pi[3]) + pi[4] * pi[4] + 2.0 * pi[5] * pi[5] +
+                        2.0 * t2 * pi[6] * pi[6] + pi[7] * pi[7] + 2.0 * t2 * pi[8] * pi[8] + t2 * t2 * pi[9] * pi[9];
+    const double c0 = pi[0] * ut - pi[1] * ux - pi[2] * uy - t2 * pi[3] * un;
+    const double c1 = pi[1] * ut - pi[4] * ux - pi[5] * uy - t2 * pi[6] * un;
+    const double c2 = pi[2] * ut - pi[5] * ux - pi[7] * uy - t2 * pi[8] * un;
+    const double c3 = (pi[3] * ut - pi[6] * ux - pi[8] * uy - t2 * pi[9] * un) * (MILNE ? t : 1.0);
+    const double iw = 1.0 / (ee + pp), ip = 1.0 / pp;
+    m[0] = fmax(m[0], eos_temperature<EOS>(P, ee));
+    m[1] = fmax(m[1], fabs(norm - 1.0));
+    m[2] = fmax(m[2], fabs(tr) * iw);
+    m[3] = fmax(m[3], fmax(fmax(fabs(c0), fabs(c1)), fmax(fabs(c2), fabs(c3))) * iw);
+    m[4] = fmax(m[4], sqrt(fabs(pipi)) * ip);
+    m[5] = fmax(m[5], fabs(Pi) * ip);
+  }
+#pragma unroll
+  for (int s = 0; s < 6; ++s) {
+    double v = m[s];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0 && v > 0.0) atomicMax(out + s, (unsigned long long)__double_as_longlong(v));
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ peak microbenchmarks
 static __global__ void __launch_bounds__(256) copy_kernel(const double2* __restrict__ src, double2* __restrict__ dst, long long n2) {
   long long stride = (long long)gridDim.x * blockDim.x;

@@ -30,7 +30,7 @@ class vh_params(C.Structure):
 
 
 # every symbol include/vh.h declares
-EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_launch_count",
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_run_until", "vh_launch_count",
            "vh_set_kernel_variant", "vh_measure_peaks", "vh_last_error", "vh_destroy"]
 
 _lib = None
@@ -55,6 +55,8 @@ def load_library():
     L.vh_step_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.vh_get_fields.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
     L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
+    L.vh_get_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
+    L.vh_run_until.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
     L.vh_launch_count.argtypes = [vp]
     L.vh_launch_count.restype = C.c_longlong
     L.vh_set_kernel_variant.argtypes = [vp, C.c_int]
@@ -202,6 +204,20 @@ class Solver:
         a, b, c = C.c_longlong(), C.c_longlong(), C.c_longlong()
         self._check(self.L.vh_get_status(self.h, C.byref(tau), C.byref(a), C.byref(b), C.byref(c), C.byref(mr)), "vh_get_status")
         return {"tau": tau.value, "n_steps": a.value, "n_inversion_failures": b.value, "n_nonfinite": c.value, "min_reg_factor": mr.value}
+
+    DIAG_NAMES = ("max_T", "max_norm_violation", "max_trace_violation", "max_transversality_violation", "max_inv_reynolds_shear",
+                  "max_inv_reynolds_bulk")
+
+    def diagnostics(self):
+        out = (C.c_double * 6)()
+        self._check(self.L.vh_get_diagnostics(self.h, out), "vh_get_diagnostics")
+        return dict(zip(self.DIAG_NAMES, list(out)))
+
+    def run_until(self, T_f, max_steps, check_every=10):
+        """Advance until T < T_f everywhere or max_steps steps (PAPER.md :494); returns the number of steps taken."""
+        done = C.c_longlong()
+        self._check(self.L.vh_run_until(self.h, float(T_f), int(max_steps), int(check_every), C.byref(done)), "vh_run_until")
+        return done.value
 
     def launch_count(self):
         return int(self.L.vh_launch_count(self.h))

@@ -399,3 +399,31 @@ def test_full_size_config5_sampled_subboxes(vh, vo):
     s.close()
     print("config 5 sampled sub-boxes: worst R18 error %.3e" % worst)
     assert 0.0 < worst <= TOL, worst      # (> 0: the comparison is not vacuous - FMA contraction alone separates the two sides)
+
+
+def test_diagnostics_and_freeze_out_termination(vh, vo):
+    # vh_get_diagnostics against the oracle's maxima; vh_run_until stops at the step at which T < T_f everywhere
+    # (program-flow step 8, :494) - the same step the oracle finds by testing after every step
+    import torch
+    for over in (dict(), dict(eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC)):
+        prm, init, _ = inputs.config_3d(40, 20, 8, n_hot=5, width=0.5, seed=inputs.BASE_SEED + 3, radius=1.5, eta_half=0.3, **over)
+        o = vo.Oracle(prm)
+        o.set_initial(init["e"], init["u"])
+        s = vh.Solver(prm)
+        s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+        o.step(6); s.step(6)
+        do, dg = o.diagnostics(), s.diagnostics()
+        for k in do:
+            if k == "max_norm_violation":
+                assert dg[k] < 1e-14 and do[k] < 1e-14
+            else:
+                assert dg[k] == pytest.approx(do[k], rel=1e-9), k
+        T_f = 0.97 * do["max_T"]             # a freeze-out temperature the cooling system crosses within a few steps
+        n_o = 0
+        while o.diagnostics()["max_T"] >= T_f and n_o < 200:
+            o.step(1); n_o += 1
+        n_g = s.run_until(T_f, 200, check_every=1)
+        assert 0 < n_o < 200 and n_g == n_o
+        assert s.diagnostics()["max_T"] < T_f and s.status()["n_steps"] == 6 + n_g
+        assert s.run_until(T_f, 5, check_every=2) == 0          # already frozen out: no step taken
+        s.close()

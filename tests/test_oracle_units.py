@@ -237,3 +237,28 @@ def test_regularisation_factor_values(vo):
     o.set_initial(np.full(shp, e0), inputs.rest_velocity(shp), pi)
     o.post(1.3)
     assert o.raw("q", 8)[2, 2, 2] == pytest.approx(1e-6 * math.tanh(10.0) / 10.0, rel=1e-12)
+
+
+def test_diagnostics_against_their_definitions(vo):
+    # the maxima of the oracle's diagnostics() re-derived with numpy from the exported fields - T from e = a T^4,
+    # u.u with g = diag(1,-1,-1,-tau^2) (:243), the constraints of Eqs. 47-51, the inverse Reynolds numbers of Eq. 89
+    prm = inputs.base_params(nx=12, ny=8, nz=6, tau0=0.6, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=3)
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], st["pi"], st["Pi"])
+    o.step(3)
+    d, f, tau = o.diagnostics(), o.get_fields(), o.status()["tau"]
+    g = np.array([1.0, -1.0, -1.0, -tau * tau])
+    u, e, p = f["u"], f["e"], f["p"]
+    slot = [[4, 5, 6, 7], [5, 8, 9, 10], [6, 9, 11, 12], [7, 10, 12, 13]]
+    pi = np.array([[f["q"][slot[m][n]] for n in range(4)] for m in range(4)])
+    assert d["max_T"] == pytest.approx(np.max((e / prm["eos_a"]) ** 0.25), rel=1e-14)
+    assert d["max_norm_violation"] == pytest.approx(np.max(np.abs(np.einsum("m,m...->...", g, u * u) - 1)), abs=1e-15)
+    assert d["max_trace_violation"] == pytest.approx(np.max(np.abs(np.einsum("m,mm...->...", g, pi)) / (e + p)), rel=1e-12)
+    c = np.abs(np.einsum("lm...,m,m...->l...", pi, g, u))
+    c[3] *= tau
+    assert d["max_transversality_violation"] == pytest.approx(np.max(c.max(axis=0) / (e + p)), rel=1e-12)
+    pipi = np.einsum("mn...,m,n,mn...->...", pi, g, g, pi)
+    assert d["max_inv_reynolds_shear"] == pytest.approx(np.max(np.sqrt(np.abs(pipi)) / p), rel=1e-12)
+    assert d["max_inv_reynolds_bulk"] == pytest.approx(np.max(np.abs(f["q"][14]) / p), rel=1e-14)
+    assert d["max_norm_violation"] < 1e-14 and 0 < d["max_trace_violation"] < 0.05      # u.u = 1 after inversion (:489); constraints drift slowly (:333)
