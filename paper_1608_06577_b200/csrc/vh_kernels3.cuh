@@ -603,6 +603,14 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   const double inv = rcp_fast((e + Pt) * ut);                    // Eq. 54
   const double u[4] = {ut, Mx * inv, My * inv, Mn * inv};
   if (!(isfinite(e) && isfinite(ut))) ++nnonf;
+  if (valid) {      // results that the regularisation does not touch go out first: their stores drain while rho is being computed
+#pragma unroll
+    for (int n = 0; n < 4; ++n) A.q_out[n * fs + c] = qv[n];
+    A.e_out[c] = e;
+    A.p_out[c] = p0;
+#pragma unroll
+    for (int n = 0; n < 4; ++n) A.u_out[n * fs + c] = u[n];
+  }
   if (VISC) {
     const double fac = regulation_factor_fast<MILNE>(P, qv, e, p0, u, tp);
     minfac = fmin(minfac, fac);
@@ -612,11 +620,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   if (valid) {
     const long long sy = P.NXp, sz = P.plane;
 #pragma unroll
-    for (int n = 0; n < NQ; ++n) A.q_out[n * fs + c] = qv[n];
-    A.e_out[c] = e;
-    A.p_out[c] = p0;
-#pragma unroll
-    for (int n = 0; n < 4; ++n) A.u_out[n * fs + c] = u[n];
+    for (int n = 4; n < NQ; ++n) A.q_out[n * fs + c] = qv[n];
     // ghost replicas (Eqs. 75-76): the outermost physical cell is copied into both ghost layers of its face (one rarely taken block)
     const bool edge = (i == 0) | (i == P.nx - 1) | (j == 0) | (j == P.ny - 1) | (!TWO_D && ((k == 0) | (k == P.nz - 1)));
     if (edge) {
