@@ -92,18 +92,17 @@ __device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, 
     const double gA = fma(-A.M2 * cA, rA * rA, 1.0), gB = fma(-B.M2 * cB, rB * rB, 1.0);
     const double dA = fA * rcp_fast(gA), dB = fB * rcp_fast(gB);
     const double eA = A.e - dA, eB = B.e - dB;
-    if (!doneA) {
-      A.e = eA;
-      A.p = fma(-cA, dA, pA);                    // P0(e - de) = P0(e) - cs2 de + O(de^2), de <= rtol e at convergence
-      A.rden = fma(rA * rA, cA * dA, rA);        // 1/(den - cs2 de) to the same order
-      if (fabs(dA) <= P.newton_rtol * fabs(eA)) { convA = true; doneA = true; }
-    }
-    if (!doneB) {
-      B.e = eB;
-      B.p = fma(-cB, dB, pB);
-      B.rden = fma(rB * rB, cB * dB, rB);
-      if (fabs(dB) <= P.newton_rtol * fabs(eB)) { convB = true; doneB = true; }
-    }
+    // A state that has converged keeps being iterated while the warp is still busy: at the root the correction is at rounding
+    // level, so this costs no accuracy and saves the selects that would freeze it.  Only a state with bad input is held (its
+    // iterates are not finite and it takes the failure path below anyway).
+    A.e = badA ? A.e : eA;
+    B.e = badB ? B.e : eB;
+    A.p = fma(-cA, dA, pA);                      // P0(e - de) = P0(e) - cs2 de + O(de^2), de <= rtol e at convergence
+    B.p = fma(-cB, dB, pB);
+    A.rden = fma(rA * rA, cA * dA, rA);          // 1/(den - cs2 de) to the same order
+    B.rden = fma(rB * rB, cB * dB, rB);
+    if (fabs(dA) <= P.newton_rtol * fabs(eA)) { convA = true; doneA = true; }
+    if (fabs(dB) <= P.newton_rtol * fabs(eB)) { convB = true; doneB = true; }
   }
   A.fail = badA || !convA || !(A.e > 0.0) || !isfinite(A.e);
   B.fail = badB || !convB || !(B.e > 0.0) || !isfinite(B.e);
