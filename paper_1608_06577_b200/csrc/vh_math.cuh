@@ -125,10 +125,8 @@ __device__ __forceinline__ double newton_single(const DevParams& P, double E, do
     const double g = fma(-M2 * c, r * r, 1.0);
     const double d = f * rcp_fast(g);
     const double en = e - d;
-    if (!done) {
-      e = en;
-      if (fabs(d) <= P.newton_rtol * fabs(en)) { conv = true; done = true; }
-    }
+    e = bad ? e : en;      // (a converged cell keeps iterating with its warp: see newton_pair)
+    if (fabs(d) <= P.newton_rtol * fabs(en)) { conv = true; done = true; }
   }
   fail = bad || !conv || !(e > 0.0) || !isfinite(e);
   if (fail) e = fmax(E, 1e-300);
