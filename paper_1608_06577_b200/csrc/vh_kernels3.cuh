@@ -87,7 +87,6 @@ __device__ __forceinline__ unsigned mbar_arrive_pending(uint64_t* bar) {
   asm volatile("mbarrier.pending_count.b64 %0, %1;" : "=r"(pending) : "l"(state));
   return pending;
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // ------------------------------------------------------------------------------------------------ flux of one field, one direction
 // r -= dtau/dr (H_{+1/2} - H_{-1/2}) from the five values a0..a4 along the direction (Eqs. 61-68): H = cp q^+ + cm q^- with
@@ -113,91 +112,13 @@ __device__ __forceinline__ void face_coefficients(double vm_lo, double vp_lo, do
   cpl = hw * (vp_lo - a_lo); cml = hw * (vm_lo + a_lo);
 }
 
-// ------------------------------------------------------------------------------------------------ relaxation sources
-// dtau * (S + G) for pi^{mu nu} (10) and Pi (B.10-B.12, Eqs. 39-46), one component at a time: emit(slot, dtau*J).
-// pi(s) returns the cell's pi component s (kept in shared memory, not in registers).  The terms of Eq. 42 are regrouped:
+// ------------------------------------------------------------------------------------------------ relaxation sources, register-lean
+// dtau * (S + G) for pi^{mu nu} (10) and Pi (B.10-B.12, Eqs. 39-46), one component at a time.  The terms of Eq. 42 are regrouped:
 //   dtau J^{mn} = c_pi pi^{mn} + c_S sigma^{mn} - (u'^n A'^m + u'^m A'^n) - sum_l (pi^{ml} Y^{ln} + pi^{nl} Y^{lm}) + k3 g^{mn} - w G^{mn}
 // with w = dtau/u^tau, u' = w u, A'^m = pi^{lm} Du_l + (tau_pipi pi:sigma / 6) u^m  (I_1 and the u u part of I_4's projector),
 // Y^{ln} = w g_ll (0.5 tau_pipi sigma^{ln} - s_omega W^{ln})  (I_4 and -I_3 share the contraction with pi), k3 = w tau_pipi pi:sigma / 3,
 // c_pi = dtau (div v - (1/tau_pi + delta_pipi theta)/u^tau), c_S = w (2 eta/tau_pi + lambda_piPi Pi).
-template <int EOS, class PiGet, class Emit>
-__device__ __forceinline__ void dissipative_sources3(const DevParams& P, double t, const double u[4], const Kin& K, PiGet pi, double Pi, double e,
-                                                     double divv, double dt, Emit emit) {
-  const double t2 = t * t, it = rcp_fast(t), it2 = it * it;
-  // transport coefficients (Eqs. 10-16; R14)
-  double p, cs2;
-  eos_p_cs2<EOS>(P, e, p, cs2);
-  const double T = (EOS == 2) ? eos_temperature<EOS>(P, e) : sqrt_fast(sqrt_fast(e * P.eos_a_inv));
-  const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
-  const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
-  const double zs = zeta_over_s(P, T);
-  const double b = (1.0 / 3.0) - cs2;
-  double itP = (zs > 0.0) ? T * b * b * P.inv_ctauPi * rcp_fast(zs) : CUDART_INF;
-  itP = fmin(itP, P.relax_clamp);
-  const double zotP = (zs > 0.0) ? zs * ((e + p) * rcp_fast(T)) * itP : 0.0;
-  const double lPp = P.lambda_Pipi_coef * b;
-  const double iut = rcp_fast(u[0]);
-  const double w = dt * iut;
-  const double* S = K.sig;
-
-  // pi^{mu nu} sigma_{mu nu}: symmetric double contraction with the metric weights of g = diag(1,-1,-1,-t2)
-  const double pisig = pi(0) * S[0] - 2.0 * (pi(1) * S[1] + pi(2) * S[2]) + pi(4) * S[4] + 2.0 * pi(5) * S[5] + pi(7) * S[7] +
-                       t2 * (2.0 * (pi(6) * S[6] + pi(8) * S[8] - pi(3) * S[3]) + t2 * pi(9) * S[9]);
-  const double beta = P.tau_pipi * pisig * (1.0 / 6.0);
-  const double k3 = 2.0 * w * beta;
-  double Ap[4], up[4];
-#pragma unroll
-  for (int m = 0; m < 4; ++m) {
-    Ap[m] = fma(beta, u[m], pi(sym(0, m)) * K.Du[0] + pi(sym(1, m)) * K.Du[1] + pi(sym(2, m)) * K.Du[2] + pi(sym(3, m)) * K.Du[3]);
-    up[m] = w * u[m];
-  }
-  // Y^{ln} = w g_ll (0.5 tau_pipi sigma^{ln} - s_omega W^{ln})
-  double Y[4][4];
-  {
-    const double gl[4] = {w, -w, -w, -w * t2};
-    const double Wm[4][4] = {{0.0, K.W[0], K.W[1], K.W[2]}, {-K.W[0], 0.0, K.W[3], K.W[4]}, {-K.W[1], -K.W[3], 0.0, K.W[5]}, {-K.W[2], -K.W[4], -K.W[5], 0.0}};
-#pragma unroll
-    for (int l = 0; l < 4; ++l) {
-      const double a = -kVorticitySign * gl[l], bb = 0.5 * P.tau_pipi * gl[l];
-#pragma unroll
-      for (int n = 0; n < 4; ++n) Y[l][n] = (l == n) ? bb * S[sym(l, n)] : fma(a, Wm[l][n], bb * S[sym(l, n)]);
-    }
-  }
-  const double cpi = dt * fma(-iut, fma(P.delta_pipi, K.theta, itp), divv);
-  const double cS = w * fma(P.lambda_piPi, Pi, eotp2);
-  const double gi[4] = {1.0, -1.0, -1.0, -it2};
-  const double g1 = w * t * u[3], g2 = w * u[0] * it, g3 = w * u[3] * it;      // Christoffel weights of G_pi (:300; R1, R2)
-#pragma unroll
-  for (int m = 0; m < 4; ++m)
-#pragma unroll
-    for (int n = m; n < 4; ++n) {
-      const int s = sym(m, n);
-      double J = cpi * pi(s);
-      J = fma(cS, S[s], J);
-      J = fma(-up[n], Ap[m], J);
-      J = fma(-up[m], Ap[n], J);
-#pragma unroll
-      for (int l = 0; l < 4; ++l) {
-        J = fma(-pi(sym(m, l)), Y[l][n], J);
-        J = fma(-pi(sym(n, l)), Y[l][m], J);
-      }
-      if (m == n) J = fma(k3, gi[m], J);
-      // G_pi = u^a Gamma^mu_{ab} pi^{b nu} + (mu<->nu)
-      if (s == 0) J = fma(-2.0 * g1, pi(3), J);
-      if (s == 1) J = fma(-g1, pi(6), J);
-      if (s == 2) J = fma(-g1, pi(8), J);
-      if (s == 3) J = fma(-g1, pi(9), fma(-g2, pi(3), fma(-g3, pi(0), J)));
-      if (s == 6) J = fma(-g2, pi(6), fma(-g3, pi(1), J));
-      if (s == 8) J = fma(-g2, pi(8), fma(-g3, pi(2), J));
-      if (s == 9) J = fma(-2.0 * g2, pi(9), fma(-2.0 * g3, pi(3), J));
-      emit(PTT + s, J);
-    }
-  const double IPi = P.delta_PiPi * Pi * K.theta - lPp * pisig;                                // Eq. 41
-  emit(BPI, dt * fma(-fma(zotP, K.theta, fma(Pi, itP, IPi)), iut, Pi * divv));                  // B.10
-}
-
-// ------------------------------------------------------------------------------------------------ relaxation sources, register-lean
-// Same regrouping as dissipative_sources3, ordered so that few values are live at a time (the 128-register budget of a
+// The evaluation is ordered so that few values are live at a time (the 128-register budget of a
 // 512-thread CTA): (1) kinematic tensors sigma (10) and W (6) as scalars (A.5-A.19); (2) the pi-independent part
 // c_pi pi^{mn} + c_S sigma^{mn} goes to the cell's park slot at once; (3) sigma, W are transformed IN PLACE into the 16
 // entries of Y^{ln} (pair (l,n), l < n: Y^{ln} = g_l (b sigma + a W), Y^{nl} = g_n (b sigma - a W)); (4) the contraction with
