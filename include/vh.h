@@ -100,12 +100,14 @@ int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long*
                   long long* n_nonfinite, double* min_reg_factor);
 
 /* On-device diagnostics of the current state, maxima over all physical cells and events, written to
- * out6[0..5]:  [0] max T in fm^-1 (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  [1] max |u.u - 1| (:489);
+ * out8[0..7]:  [0] max T in fm^-1 (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  [1] max |u.u - 1| (:489);
  * [2] max |g_{mu nu} pi^{mu nu}|/(e+p) and [3] max over lambda of |pi^{lambda mu} u_mu|/(e+p) (the constraints of Eqs. 47-51,
  * :318-331, which are propagated, not enforced; the lambda = eta entry is multiplied by tau);  [4] max R_pi^-1 =
- * sqrt(pi^{mu nu} pi_{mu nu})/P0 and [5] max R_Pi^-1 = |Pi|/P0 (inverse Reynolds numbers, Eq. 89, :826).  One reduction
- * kernel; synchronises the stream.  out6 is a HOST pointer.                                                               */
-int vh_get_diagnostics(vh_handle* h, double* out6);
+ * sqrt(pi^{mu nu} pi_{mu nu})/P0 and [5] max R_Pi^-1 = |Pi|/P0 (inverse Reynolds numbers, Eq. 89, :826);  [6] max Kn = tau_pi |theta|
+ * and [7] max tau_Pi |theta| (Knudsen numbers, :830; theta of A.11 with the finite differences of the source terms, :424, and the
+ * relaxation times the solver uses; cells with 1/tau = 0 do not count; 0 if the sector is off).  One reduction kernel;
+ * synchronises the stream.  out8 is a HOST pointer to 8 doubles.                                                          */
+int vh_get_diagnostics(vh_handle* h, double* out8);
 
 /* Program-flow steps 6-8 (:492-494): advance until T < T_f (fm^-1) everywhere or max_steps steps have been taken, testing the
  * temperature every check_every steps (>= 1) with the reduction of vh_get_diagnostics.  *steps_done (may be NULL) receives the

@@ -251,9 +251,14 @@ template <class R> class Solver {
   // ------------------------------------------------------------ diagnostics, maxima over the physical cells
   // out[0] max T (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  out[1] max |u.u - 1| (:489);
   // out[2] max |g_{mu nu} pi^{mu nu}|/(e+p), out[3] max_lambda |pi^{lambda mu} u_mu|/(e+p) (Eqs. 47-51, :318-331; the lambda = eta
-  // entry times tau);  out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826)
-  void diagnostics(double out[6]) const {
-    for (int i = 0; i < 6; ++i) out[i] = 0.0;
+  // entry times tau);  out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826);
+  // out[6] max Kn_{theta pi} = tau_pi |theta|, out[7] max Kn_{theta Pi} = tau_Pi |theta| (:830) with theta of A.11 discretised as in the
+  // sources (backward difference in time, central in space, :424) and the relaxation times the solver uses (R14); a cell whose
+  // quotient is not finite (1/tau = 0) does not count; 0 when the sector is switched off
+  void diagnostics(double out[8]) const {
+    for (int i = 0; i < 8; ++i) out[i] = 0.0;
+    const size_t stride[3] = {1, (size_t)NX, (size_t)NX * NY};
+    const double dr[3] = {P.dx, P.dy, P.dz};
     const double t = (double)tau, t2 = (double)tau2(tau);
     const double g[4] = {1.0, -1.0, -1.0, -t2};
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i) {
@@ -278,6 +283,14 @@ template <class R> class Solver {
       out[3] = std::fmax(out[3], orth / (ee + pp));
       out[4] = std::fmax(out[4], std::sqrt(std::fabs(pipi)) / pp);
       out[5] = std::fmax(out[5], std::fabs((double)q[14][s]) / pp);
+      double theta = (milne() ? uu[0] / t : 0.0) + (uu[0] - (double)up[0][s]) / P.dtau;
+      for (int d = 0; d < 3; ++d) theta += ((double)u[d + 1][s + stride[d]] - (double)u[d + 1][s - stride[d]]) / (2.0 * dr[d]);
+      Thermo<double> th = eos<double>(P, ee);
+      th.T = T;
+      const Transport<double> tc = transport<double>(P, ee, th);
+      const double kp = std::fabs(theta) / tc.inv_tau_pi, kP = std::fabs(theta) / tc.inv_tau_Pi;
+      if ((P.physics & 1) && std::isfinite(kp)) out[6] = std::fmax(out[6], kp);
+      if ((P.physics & 2) && std::isfinite(kP)) out[7] = std::fmax(out[7], kP);
     }
   }
 

@@ -71,9 +71,9 @@ int vho_get_status(vho_handle* h, double* tau, long long* n_steps, long long* n_
 }
 
 // maxima over all events of Solver::diagnostics (double instantiation only)
-void vho_diagnostics(vho_handle* h, double* out6) {
-  for (int i = 0; i < 6; ++i) out6[i] = 0.0;
-  for (Sol* s : h->ev) { double o[6]; s->diagnostics(o); for (int i = 0; i < 6; ++i) if (o[i] > out6[i]) out6[i] = o[i]; }
+void vho_diagnostics(vho_handle* h, double* out8) {
+  for (int i = 0; i < 8; ++i) out8[i] = 0.0;
+  for (Sol* s : h->ev) { double o[8]; s->diagnostics(o); for (int i = 0; i < 8; ++i) if (o[i] > out8[i]) out8[i] = o[i]; }
 }
 void vho_last_failure(vho_handle* h, int ev, double* out4) { for (int i = 0; i < 4; ++i) out4[i] = h->ev[ev]->last_fail[i]; }
 

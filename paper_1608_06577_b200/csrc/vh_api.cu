@@ -156,8 +156,8 @@ static void launch_diag(vh_handle* h, double t) {
   const DevParams& P = h->P;
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const unsigned nb = (unsigned)std::min<long long>((np + 255) / 256, 2048LL);      // grid-stride loop
-  if (h->prm.geometry == 0) diagnostics_kernel<EOS, true><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], t, h->diag);
-  else diagnostics_kernel<EOS, false><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], t, h->diag);
+  if (h->prm.geometry == 0) diagnostics_kernel<EOS, true><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1], t, h->diag);
+  else diagnostics_kernel<EOS, false><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1], t, h->diag);
   h->launches++;
 }
 
@@ -451,19 +451,19 @@ int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long*
   return VH_OK;
 }
 
-int vh_get_diagnostics(vh_handle* h, double* out6) {
+int vh_get_diagnostics(vh_handle* h, double* out8) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostics before vh_set_initial");
-  if (!out6) return fail(h, VH_ERR_ARG, "out6 is NULL");
-  if (!h->diag && cudaMalloc((void**)&h->diag, 6 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
-  CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 6 * sizeof(unsigned long long), h->stream));
+  if (!out8) return fail(h, VH_ERR_ARG, "out8 is NULL");
+  if (!h->diag && cudaMalloc((void**)&h->diag, 8 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
+  CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 8 * sizeof(unsigned long long), h->stream));
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
   if (h->prm.eos == 2) launch_diag<2>(h, t); else if (h->prm.eos == 1) launch_diag<1>(h, t); else launch_diag<0>(h, t);
   CUDA_TRY(h, cudaGetLastError());
-  unsigned long long bits[6];
+  unsigned long long bits[8];
   CUDA_TRY(h, cudaMemcpyAsync(bits, h->diag, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-  std::memcpy(out6, bits, sizeof(bits));
+  std::memcpy(out8, bits, sizeof(bits));
   return VH_OK;
 }
 
@@ -472,7 +472,7 @@ int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long 
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_run_until before vh_set_initial");
   if (max_steps < 0 || check_every < 1 || !(T_f >= 0.0)) return fail(h, VH_ERR_ARG, "max_steps >= 0, check_every >= 1, T_f >= 0 required");
   long long done = 0;
-  double d[6];
+  double d[8];
   while (done < max_steps) {
     int rc = vh_get_diagnostics(h, d);
     if (rc) return rc;

@@ -399,15 +399,17 @@ __global__ void __launch_bounds__(256) pressure_kernel(const __grid_constant__ D
 // Maxima over the physical cells, accumulated with atomicMax on the bit patterns (non-negative doubles order like integers):
 // out[0] max T (freeze-out test "T < T_f everywhere", program-flow step 8, :494); out[1] max |u.u - 1| (:489);
 // out[2] max |g_{mu nu} pi^{mu nu}|/(e+p), out[3] max_lambda |pi^{lambda mu} u_mu|/(e+p) (Eqs. 47-51, :318-331; lambda = eta entry
-// times tau); out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826).
+// times tau); out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826); out[6], out[7] max Knudsen
+// numbers tau_pi |theta|, tau_Pi |theta| (:830): theta of A.11 with the differences of the sources (:424) and the solver's relaxation
+// times (R14); cells with a non-finite quotient do not count, a switched-off sector gives 0.
 template <int EOS, bool MILNE>
 __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant__ DevParams P, const double* __restrict__ q, const double* __restrict__ e,
-                                                          const double* __restrict__ p, const double* __restrict__ u, double t,
-                                                          unsigned long long* __restrict__ out) {
+                                                          const double* __restrict__ p, const double* __restrict__ u, const double* __restrict__ u_prev,
+                                                          double t, unsigned long long* __restrict__ out) {
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const long long fs = P.fstride;
   const double t2 = MILNE ? t * t : 1.0;
-  double m[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  double m[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < np; n += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(n % P.nx);
     const int j = (int)((n / P.nx) % P.ny);
@@ -435,9 +437,22 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     m[3] = fmax(m[3], fmax(fmax(fabs(c0), fabs(c1)), fmax(fabs(c2), fabs(c3))) * iw);
     m[4] = fmax(m[4], sqrt(fabs(pipi)) * ip);
     m[5] = fmax(m[5], fabs(Pi) * ip);
+    // Knudsen numbers: theta = u^tau/tau + d_tau u^tau + d_i u^i (A.11), backward in time, central in space (:424)
+    double theta = (MILNE ? ut / t : 0.0) + (ut - u_prev[c]) * P.inv_dtau;
+    theta += (u[fs + c + 1] - u[fs + c - 1]) * (0.5 * P.inv_dx) + (u[2 * fs + c + P.NXp] - u[2 * fs + c - P.NXp]) * (0.5 * P.inv_dy);
+    if (P.NZp > 1) theta += (u[3 * fs + c + P.plane] - u[3 * fs + c - P.plane]) * (0.5 * P.inv_dz);
+    const double T = eos_temperature<EOS>(P, ee);
+    double p0, cs2;
+    eos_p_cs2<EOS>(P, ee, p0, cs2);
+    const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
+    const double zs = zeta_over_s(P, T), bb = (1.0 / 3.0) - cs2;
+    const double itP = fmin((zs > 0.0) ? T * bb * bb * P.inv_ctauPi / zs : CUDART_INF, P.relax_clamp);
+    const double kp = fabs(theta) / itp, kP = fabs(theta) / itP;
+    if (P.shear && isfinite(kp)) m[6] = fmax(m[6], kp);
+    if (P.bulk && isfinite(kP)) m[7] = fmax(m[7], kP);
   }
 #pragma unroll
-  for (int s = 0; s < 6; ++s) {
+  for (int s = 0; s < 8; ++s) {
     double v = m[s];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));

@@ -206,10 +206,10 @@ class Solver:
         return {"tau": tau.value, "n_steps": a.value, "n_inversion_failures": b.value, "n_nonfinite": c.value, "min_reg_factor": mr.value}
 
     DIAG_NAMES = ("max_T", "max_norm_violation", "max_trace_violation", "max_transversality_violation", "max_inv_reynolds_shear",
-                  "max_inv_reynolds_bulk")
+                  "max_inv_reynolds_bulk", "max_knudsen_shear", "max_knudsen_bulk")
 
     def diagnostics(self):
-        out = (C.c_double * 6)()
+        out = (C.c_double * 8)()
         self._check(self.L.vh_get_diagnostics(self.h, out), "vh_get_diagnostics")
         return dict(zip(self.DIAG_NAMES, list(out)))
 

@@ -261,4 +261,13 @@ def test_diagnostics_against_their_definitions(vo):
     pipi = np.einsum("mn...,m,n,mn...->...", pi, g, g, pi)
     assert d["max_inv_reynolds_shear"] == pytest.approx(np.max(np.sqrt(np.abs(pipi)) / p), rel=1e-12)
     assert d["max_inv_reynolds_bulk"] == pytest.approx(np.max(np.abs(f["q"][14]) / p), rel=1e-14)
+    # Knudsen numbers (:830): theta of A.11 from the exported u^n, u^{n-1} with numpy differences (ghost = copy of the boundary cell)
+    fu = o.get_fields(with_uprev=True)
+    pad = lambda a, ax: np.concatenate([np.take(a, [0], axis=ax), a, np.take(a, [-1], axis=ax)], axis=ax)
+    cd = lambda a, ax, h: (np.take(pad(a, ax), range(2, a.shape[ax] + 2), axis=ax) - np.take(pad(a, ax), range(0, a.shape[ax]), axis=ax)) / (2 * h)
+    theta = u[0] / tau + (u[0] - fu["up"][0]) / prm["dtau"] + cd(u[1], 3, prm["dx"]) + cd(u[2], 2, prm["dy"]) + cd(u[3], 1, prm["dz"])
+    it_pi = np.vectorize(lambda ee: vo.transport(prm, ee)["inv_tau_pi"])(e)
+    it_Pi = np.vectorize(lambda ee: vo.transport(prm, ee)["inv_tau_Pi"])(e)
+    assert d["max_knudsen_shear"] == pytest.approx(np.max(np.abs(theta) / it_pi), rel=1e-12)
+    assert d["max_knudsen_bulk"] == pytest.approx(np.max(np.abs(theta) / it_Pi), rel=1e-12)
     assert d["max_norm_violation"] < 1e-14 and 0 < d["max_trace_violation"] < 0.05      # u.u = 1 after inversion (:489); constraints drift slowly (:333)
