@@ -38,7 +38,7 @@ struct DevParams {
 };
 
 // ---------------------------------------------------------------- exp(-x) for the EOS and zeta/s(T)
-// exp(-x) with the argument clamped to [-700, 708] (beyond: 1e304 / 3e-308 instead of inf / 0, never reached by a state
+// exp(-x) with the argument clamped to [-700, 700] (beyond: 1e304 / 1e-304 instead of inf / 0, never reached by a state
 // that passes the finiteness checks).  -x = k ln2 + r, |r| <= ln2/2, Taylor polynomial of degree 13 (truncation 4e-18), 2^k
 // added into the exponent field.  The coefficients sit in constant memory so that each Horner step is ONE DFMA with a
 // constant-bank operand; the library exp() materialises its 64-bit immediates with two moves per coefficient, which made
@@ -47,7 +47,7 @@ static __constant__ double kExpTaylor[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 2
                                              1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
 static __constant__ double kExpRed[4] = {1.4426950408889634, 6755399441055744.0, 6.93147180369123816490e-01, 1.90821492927058770002e-10};
 __device__ __forceinline__ double exp_neg(double x) {
-  x = fmin(fmax(x, -700.0), 708.0);
+  x = (fabs(x) < 700.0) ? x : copysign(700.0, x);      // one compare and a select (fmin/fmax with their NaN rules cost four times that); NaN -> 700
   const double t = fma(-x, kExpRed[0], kExpRed[1]);      // 1.5 * 2^52 + rint(-x log2 e): the integer sits in the low word
   const int k = __double2loint(t);
   const double kd = t - kExpRed[1];
