@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, TWO_D ? 3 : 6)
     ozp = (tz + 1 < VZ) ? oc + AX * AY : zl + T::Z_SIZE;
   }
   const double t2 = MILNE ? A.t * A.t : 1.0;
-  const double ht = 0.5 * P.theta;
+  const double theta = P.theta;
   unsigned long long nfail = 0;
   mbar_wait(full, 0u);
 
@@ -106,8 +106,8 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, TWO_D ? 3 : 6)
     for (int m = 0; m < 4; ++m) {
       const double* f = slots + m * T::SLOT;
       const double a0 = f[om], a1 = f[oc], a2 = f[op];
-      const double h = half_slope2<THETA1>(a1 - a0, a2 - a1, ht);
-      wL[m] = a1 - h; wR[m] = a1 + h;
+      const double sl = minmod_slope<THETA1>(a1 - a0, a2 - a1, theta);      // Eqs. 67-68; the half-cell factor 1/2 sits in the FMAs
+      wL[m] = fma(-0.5, sl, a1); wR[m] = fma(0.5, sl, a1);
     }
     wL[4] = 0.0; wR[4] = 0.0;
     if (VISC) {
@@ -115,13 +115,13 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, TWO_D ? 3 : 6)
       for (int m = 0; m < 4; ++m) {
         const double* f = slots + (4 + m) * T::SLOT;
         const double a0 = f[om], a1 = f[oc], a2 = f[op];
-        const double h = half_slope2<THETA1>(a1 - a0, a2 - a1, ht);
-        wL[m] -= a1 - h; wR[m] -= a1 + h;
+        const double sl = minmod_slope<THETA1>(a1 - a0, a2 - a1, theta);
+        wL[m] -= fma(-0.5, sl, a1); wR[m] -= fma(0.5, sl, a1);
       }
       const double* f = slots + 8 * T::SLOT;
       const double a0 = f[om], a1 = f[oc], a2 = f[op];
-      const double h = half_slope2<THETA1>(a1 - a0, a2 - a1, ht);
-      wL[4] = a1 - h; wR[4] = a1 + h;
+      const double sl = minmod_slope<THETA1>(a1 - a0, a2 - a1, theta);
+      wL[4] = fma(-0.5, sl, a1); wR[4] = fma(0.5, sl, a1);
     }
     NewtonState SL, SR;
     SL.E = wL[0]; SL.Pi = wL[4]; SL.M2 = wL[1] * wL[1] + wL[2] * wL[2] + t2 * wL[3] * wL[3];     // :339

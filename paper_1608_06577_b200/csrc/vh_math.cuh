@@ -76,8 +76,9 @@ struct NewtonState {
 template <int EOS>
 __device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, NewtonState& B, double guess) {
   const bool gok = (guess > 0.0) && isfinite(guess);
-  bool badA = !(A.E > 0.0) || !isfinite(A.E) || !isfinite(A.M2) || !isfinite(A.Pi);
-  bool badB = !(B.E > 0.0) || !isfinite(B.E) || !isfinite(B.M2) || !isfinite(B.Pi);
+  // (one finiteness test on the sum: it is finite exactly when E, M2 and Pi all are, short of an overflow that no state reaches)
+  bool badA = !(A.E > 0.0) || !isfinite(A.E + A.M2 + A.Pi);
+  bool badB = !(B.E > 0.0) || !isfinite(B.E + B.M2 + B.Pi);
   A.e = gok ? guess : A.E;
   B.e = gok ? guess : B.E;
   bool doneA = badA, doneB = badB, convA = false, convB = false;
