@@ -114,7 +114,7 @@ __device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, 
 // single state (cell inversion in the stage epilogue)
 template <int EOS>
 __device__ __forceinline__ double newton_single(const DevParams& P, double E, double M2, double Pi, double guess, bool& fail) {
-  const bool bad = !(E > 0.0) || !isfinite(E) || !isfinite(M2) || !isfinite(Pi);
+  const bool bad = !(E > 0.0) || !isfinite(E + M2 + Pi);      // (see newton_pair)
   double e = ((guess > 0.0) && isfinite(guess)) ? guess : E;
   bool done = bad, conv = false;
   for (int it = 0; it < P.newton_max_iter; ++it) {
