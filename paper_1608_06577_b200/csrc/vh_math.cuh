@@ -82,29 +82,30 @@ __device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, 
   A.e = gok ? guess : A.E;
   B.e = gok ? guess : B.E;
   bool doneA = badA, doneB = badB, convA = false, convB = false;
-  A.p = 0.0; B.p = 0.0; A.rden = 0.0; B.rden = 0.0;
+  double pA = 0.0, cA = 0.0, rA = 0.0, dA = 0.0, pB = 0.0, cB = 0.0, rB = 0.0, dB = 0.0;      // last iterate's P0, cs2, 1/(E + P0 + Pi), correction
   for (int it = 0; it < P.newton_max_iter; ++it) {
     if (__all_sync(0xffffffffu, doneA && doneB)) break;
-    double pA, cA, pB, cB;
     eos_p_cs2<EOS>(P, A.e, pA, cA);
     eos_p_cs2<EOS>(P, B.e, pB, cB);
-    const double rA = rcp_fast(A.E + pA + A.Pi), rB = rcp_fast(B.E + pB + B.Pi);
+    rA = rcp_fast(A.E + pA + A.Pi); rB = rcp_fast(B.E + pB + B.Pi);
     const double fA = A.e - A.E + A.M2 * rA, fB = B.e - B.E + B.M2 * rB;
     const double gA = fma(-A.M2 * cA, rA * rA, 1.0), gB = fma(-B.M2 * cB, rB * rB, 1.0);
-    const double dA = fA * rcp_fast(gA), dB = fB * rcp_fast(gB);
+    dA = fA * rcp_half(gA); dB = fB * rcp_half(gB);      // f' in (0, 1] only steers the iteration: 40 bits are plenty
     const double eA = A.e - dA, eB = B.e - dB;
     // A state that has converged keeps being iterated while the warp is still busy: at the root the correction is at rounding
     // level, so this costs no accuracy and saves the selects that would freeze it.  Only a state with bad input is held (its
     // iterates are not finite and it takes the failure path below anyway).
     A.e = badA ? A.e : eA;
     B.e = badB ? B.e : eB;
-    A.p = fma(-cA, dA, pA);                      // P0(e - de) = P0(e) - cs2 de + O(de^2), de <= rtol e at convergence
-    B.p = fma(-cB, dB, pB);
-    A.rden = fma(rA * rA, cA * dA, rA);          // 1/(den - cs2 de) to the same order
-    B.rden = fma(rB * rB, cB * dB, rB);
     if (fabs(dA) <= P.newton_rtol * fabs(eA)) { convA = true; doneA = true; }
     if (fabs(dB) <= P.newton_rtol * fabs(eB)) { convB = true; doneB = true; }
   }
+  // P0 and 1/(E + P0 + Pi) at the returned e, extrapolated from the last iterate over its correction (once, after the loop):
+  // P0(e - d) = P0(e) - cs2 d + O(d^2), 1/(den - cs2 d) = r + r^2 cs2 d + O(d^2), |d| <= rtol e at convergence
+  A.p = fma(-cA, dA, pA);
+  B.p = fma(-cB, dB, pB);
+  A.rden = fma(rA * rA, cA * dA, rA);
+  B.rden = fma(rB * rB, cB * dB, rB);
   A.fail = badA || !convA || !(A.e > 0.0) || !isfinite(A.e);
   B.fail = badB || !convB || !(B.e > 0.0) || !isfinite(B.e);
   if (A.fail) { A.e = fmax(A.E, 1e-300); A.p = eos_p<EOS>(P, A.e); A.rden = 1.0 / (A.E + A.p + A.Pi); }
@@ -124,7 +125,7 @@ __device__ __forceinline__ double newton_single(const DevParams& P, double E, do
     const double r = rcp_fast(E + p + Pi);
     const double f = e - E + M2 * r;
     const double g = fma(-M2 * c, r * r, 1.0);
-    const double d = f * rcp_fast(g);
+    const double d = f * rcp_half(g);      // (f' only steers the iteration)
     const double en = e - d;
     e = bad ? e : en;      // (a converged cell keeps iterating with its warp: see newton_pair)
     if (fabs(d) <= P.newton_rtol * fabs(en)) { conv = true; done = true; }
