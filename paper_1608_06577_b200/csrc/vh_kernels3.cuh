@@ -545,22 +545,24 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     // ghost replicas (Eqs. 75-76): the outermost physical cell is copied into both ghost layers of its face (one rarely taken block)
     const bool edge = (i == 0) | (i == P.nx - 1) | (j == 0) | (j == P.ny - 1) | (!TWO_D && ((k == 0) | (k == P.nz - 1)));
     if (edge) {
-      auto rep = [&](double* a, double v) {
-        if (i == 0) { a[c - 1] = v; a[c - 2] = v; }
-        if (i == P.nx - 1) { a[c + 1] = v; a[c + 2] = v; }
-        if (j == 0) { a[c - sy] = v; a[c - 2 * sy] = v; }
-        if (j == P.ny - 1) { a[c + sy] = v; a[c + 2 * sy] = v; }
-        if (!TWO_D) {
-          if (k == 0) { a[c - sz] = v; a[c - 2 * sz] = v; }
-          if (k == P.nz - 1) { a[c + sz] = v; a[c + 2 * sz] = v; }
-        }
+      // one block per face, each testing its condition ONCE and then writing all 21 arrays: a warp on an x face (half of all warps
+      // at 128^3) runs one block with one active lane and skips the other five
+      auto replicate = [&](long long o1, long long o2) {
+#pragma unroll
+        for (int n = 0; n < NQ; ++n) { double* a = A.q_out + n * fs + c; a[o1] = qv[n]; a[o2] = qv[n]; }
+        A.e_out[c + o1] = e; A.e_out[c + o2] = e;
+        A.p_out[c + o1] = p0; A.p_out[c + o2] = p0;
+#pragma unroll
+        for (int n = 0; n < 4; ++n) { double* a = A.u_out + n * fs + c; a[o1] = u[n]; a[o2] = u[n]; }
       };
-#pragma unroll
-      for (int n = 0; n < NQ; ++n) rep(A.q_out + n * fs, qv[n]);
-      rep(A.e_out, e);
-      rep(A.p_out, p0);
-#pragma unroll
-      for (int n = 0; n < 4; ++n) rep(A.u_out + n * fs, u[n]);
+      if (i == 0) replicate(-1, -2);
+      if (i == P.nx - 1) replicate(1, 2);
+      if (j == 0) replicate(-sy, -2 * sy);
+      if (j == P.ny - 1) replicate(sy, 2 * sy);
+      if (!TWO_D) {
+        if (k == 0) replicate(-sz, -2 * sz);
+        if (k == P.nz - 1) replicate(sz, 2 * sz);
+      }
     }
   }
   flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0, record);
