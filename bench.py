@@ -31,7 +31,7 @@ ALG_BYTES_PER_CELL_UPDATE = 856.0      # 107 doubles per cell-up
 ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the stage kernel at 128^3 from the committed ncu --set full
 # capture (profiles/r01c_ncu_summary.md); valid for the default workload (128^3) only
-NCU_TRAFFIC_BYTES = {"stage1": 629097472 + 357730048, "stage2": 927127040 + 358041088}      # profiles/r01c_ncu_summary.md
+NCU_TRAFFIC_BYTES = {"stage1": 629327104 + 353338112, "stage2": 932169216 + 358881024}      # profiles/r01c_ncu_summary.md
 
 
 def workload(rank=0, physics="config3"):
