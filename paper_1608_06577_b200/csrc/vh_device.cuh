@@ -37,6 +37,43 @@ struct DevParams {
   int debug;                    // VH_DEBUG_FLAGS (development only)
 };
 
+// ---------------------------------------------------------------- branch-free reciprocal / square roots on the MUFU seeds
+// 1/x to ~1 ulp: MUFU.RCP64H seed (~20 bits) + two Newton steps.  No denormal / overflow slow path: callers pass
+// well-scaled positive quantities; inf/NaN/0 propagate as NaN/inf and are caught by the callers' finiteness checks.
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = fma(-x, y, 1.0);
+  y = fma(y, t, y);
+  t = fma(-x, y, 1.0);
+  return fma(y, t, y);
+}
+// one Newton step only (~40 bits): enough wherever the quotient only steers an iteration
+__device__ __forceinline__ double rcp_half(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = fma(-x, y, 1.0);
+  return fma(y, t, y);
+}
+// 1/sqrt(x) to ~1 ulp: MUFU.RSQ64H seed + two Newton steps
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double hx = 0.5 * x;
+  double t = fma(-hx * y, y, 0.5);
+  y = fma(y, t, y);
+  t = fma(-hx * y, y, 0.5);
+  return fma(y, t, y);
+}
+// sqrt(x) for x > 0 (x = 0 gives 0): x * rsqrt(x) with one correction step
+__device__ __forceinline__ double sqrt_fast(double x) {
+  double r = rsqrt_fast(x);
+  double s = x * r;
+  double d = fma(-s, s, x);
+  s = fma(0.5 * r, d, s);
+  return (x > 0.0) ? s : 0.0;
+}
+
 // ---------------------------------------------------------------- exp(-x) for the EOS and zeta/s(T)
 // exp(-x) with the argument clamped to [-700, 700] (beyond: 1e304 / 1e-304 instead of inf / 0, never reached by a state
 // that passes the finiteness checks).  -x = k ln2 + r, |r| <= ln2/2, Taylor polynomial of degree 13 (truncation 4e-18), 2^k
@@ -74,7 +111,10 @@ template <int EOS> __device__ __forceinline__ void eos_p_cs2(const DevParams& P,
 // EOS 2: cubic Hermite interpolation in x = e^{1/4} of the tabulated lattice pressure and temperature (R20); c_s^2 is the
 // derivative of the pressure interpolant.  Below the table P = (P_0/e_0) e, T = (T_0/x_0) x; above it P = P_N + (e - e_N)/3.
 __device__ __forceinline__ void eos_lattice(const DevParams& P, double e, double& p, double& cs2, double& T) {
-  const double x = (e > 0.0) ? sqrt(sqrt(e)) : 0.0;            // (e <= 0 or NaN falls into the first branch)
+  // x = e^{1/4} as rsqrt(rsqrt(e)), y = e^{-1/2}: two MUFU seeds with two Newton steps each, no IEEE square-root slow path, and
+  // 1/x^3 = x y^2 comes for free (e <= 0 or NaN falls into the first branch below)
+  const double y = rsqrt_fast(e);
+  const double x = (e > 0.0) ? rsqrt_fast(y) : 0.0;
   if (!(x >= P.eos_x0)) { p = P.eos_lo_slope * e; cs2 = P.eos_lo_slope; T = P.eos_T0_over_x0 * x; return; }
   if (x >= P.eos_xN) { p = fma(e - P.eos_eN, 1.0 / 3.0, P.eos_pN); cs2 = 1.0 / 3.0; T = P.eos_TN_over_xN * x; return; }
   const double u = (x - P.eos_x0) * P.eos_inv_h;
@@ -86,7 +126,7 @@ __device__ __forceinline__ void eos_lattice(const DevParams& P, double e, double
   T = h00 * at.x + h10 * at.y + h01 * bt.x + h11 * bt.y;
   const double d00 = 6.0 * (s2 - s), d10 = 3.0 * s2 - 4.0 * s + 1.0, d11 = 3.0 * s2 - 2.0 * s;
   const double dpdx = (d00 * (ap.x - bp.x) + d10 * ap.y + d11 * bp.y) * P.eos_inv_h;
-  cs2 = dpdx / (4.0 * x * x * x);
+  cs2 = dpdx * (0.25 * x) * (y * y);
 }
 template <> __device__ __forceinline__ void eos_p_cs2<2>(const DevParams& P, double e, double& p, double& cs2) {
   double T;

@@ -6,41 +6,7 @@
 
 namespace vh {
 
-// 1/x to ~1 ulp: MUFU.RCP64H seed (~20 bits) + two Newton steps.  No denormal / overflow slow path: callers pass
-// well-scaled positive quantities; inf/NaN/0 propagate as NaN/inf and are caught by the callers' finiteness checks.
-__device__ __forceinline__ double rcp_fast(double x) {
-  double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double t = fma(-x, y, 1.0);
-  y = fma(y, t, y);
-  t = fma(-x, y, 1.0);
-  return fma(y, t, y);
-}
-// one Newton step only (~40 bits): enough wherever the quotient only steers an iteration
-__device__ __forceinline__ double rcp_half(double x) {
-  double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double t = fma(-x, y, 1.0);
-  return fma(y, t, y);
-}
-// 1/sqrt(x) to ~1 ulp: MUFU.RSQ64H seed + two Newton steps
-__device__ __forceinline__ double rsqrt_fast(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double hx = 0.5 * x;
-  double t = fma(-hx * y, y, 0.5);
-  y = fma(y, t, y);
-  t = fma(-hx * y, y, 0.5);
-  return fma(y, t, y);
-}
-// sqrt(x) for x > 0 (x = 0 gives 0): x * rsqrt(x) with one correction step
-__device__ __forceinline__ double sqrt_fast(double x) {
-  double r = rsqrt_fast(x);
-  double s = x * r;
-  double d = fma(-s, s, x);
-  s = fma(0.5 * r, d, s);
-  return (x > 0.0) ? s : 0.0;
-}
+// (rcp_fast, rcp_half, rsqrt_fast, sqrt_fast live in vh_device.cuh: the EOS lookup uses them too)
 
 // (dr/2) * minmod(theta d1/dr, (d1+d2)/(2 dr), theta d2/dr) with d1 = q0 - qm, d2 = qp - q0   (Eqs. 67-68, R10).
 // When d1, d2 have the same sign the centred difference has it too and |d1+d2|/2 = (|d1|+|d2|)/2; for theta = 1 it lies
