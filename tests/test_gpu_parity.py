@@ -142,6 +142,14 @@ def test_lattice_eos_and_the_papers_own_physics(vh, vo):
     prm, init, _ = inputs.config_3d(18, 14, 9, n_hot=3, width=0.4, seed=3, physics=0, eos=2, radius=0.6, eta_half=0.3)
     fo, so, fg, sg = run_both(vh, vo, prm, init, 8)
     assert_parity(fo, so, fg, sg)
+    # both continuations outside the table (R20): a cold rim below T = 30 MeV (e < 1e-4 fm^-4) and a core above T = 2 GeV
+    prm = inputs.base_params(nx=24, ny=10, nz=6, tau0=1.0, dtau=0.01, physics=0, eos=2)
+    x = inputs.centred_axis(24, prm["dx"])
+    e = np.empty((1, 6, 10, 24))
+    e[...] = 2e-5 + 4.0e5 * np.exp(-(x / 0.2) ** 2)
+    assert vo.eos(prm, e.min())["T"] * inputs.HBARC < 0.03 and vo.eos(prm, e.max())["T"] * inputs.HBARC > 2.0
+    fo, so, fg, sg = run_both(vh, vo, prm, dict(e=e, u=inputs.rest_velocity(e.shape)), 5)
+    assert_parity(fo, so, fg, sg)
 
 
 def test_batched_2plus1d_events(vh, vo):
