@@ -114,6 +114,13 @@ int vh_get_diagnostics(vh_handle* h, double* out8);
  * number of steps taken by this call; returns VH_OK in both cases (compare vh_get_diagnostics()[0] with T_f to tell them apart). */
 int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long long* steps_done);
 
+/* The table of EOS 2 as the library builds it on the host (no CUDA call; for inspection and for the CPU-side test that compares it
+ * with the independently built table of the test oracle): VH_EOS_TABLE_NODES = 2049 nodes uniform in x = e^{1/4}, node k at
+ * x0 + k h holding (P, h dP/dx, T, h dT/dx) in nodes4[4k .. 4k+3] (fm^-4, fm^-1; R19, R20).  nodes4 must hold
+ * 4 * 2049 doubles (host pointer); x0, h may be NULL.                                                                      */
+#define VH_EOS_TABLE_NODES 2049
+int vh_eos_table(double* nodes4, double* x0, double* h);
+
 /* Number of kernels launched on the handle since vh_create (for bench.py's gpu_launches).                             */
 long long vh_launch_count(vh_handle* h);
 

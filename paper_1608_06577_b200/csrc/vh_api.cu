@@ -451,6 +451,16 @@ int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long*
   return VH_OK;
 }
 
+int vh_eos_table(double* nodes4, double* x0, double* h) {
+  if (!nodes4) return fail(nullptr, VH_ERR_ARG, "nodes4 is NULL");
+  static_assert(VH_EOS_TABLE_NODES == vh_eos::VH_EOS_N + 1, "header and builder disagree on the table size");
+  const vh_eos::LatticeTable tab = vh_eos::Builder().build();
+  std::memcpy(nodes4, tab.node.data(), tab.node.size() * sizeof(double));
+  if (x0) *x0 = tab.x0;
+  if (h) *h = tab.h;
+  return VH_OK;
+}
+
 int vh_get_diagnostics(vh_handle* h, double* out8) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostics before vh_set_initial");

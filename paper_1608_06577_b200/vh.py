@@ -30,7 +30,7 @@ class vh_params(C.Structure):
 
 
 # every symbol include/vh.h declares
-EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_run_until", "vh_launch_count",
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_run_until", "vh_eos_table", "vh_launch_count",
            "vh_set_kernel_variant", "vh_measure_peaks", "vh_last_error", "vh_destroy"]
 
 _lib = None
@@ -57,6 +57,7 @@ def load_library():
     L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     L.vh_get_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
     L.vh_run_until.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
+    L.vh_eos_table.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.vh_launch_count.argtypes = [vp]
     L.vh_launch_count.restype = C.c_longlong
     L.vh_set_kernel_variant.argtypes = [vp, C.c_int]
@@ -225,6 +226,19 @@ class Solver:
     def set_kernel_variant(self, v):
         self._check(self.L.vh_set_kernel_variant(self.h, int(v)), "vh_set_kernel_variant")
         self.variant = int(v)
+
+
+def eos_table():
+    """(nodes [2049, 4] = (P, h dP/dx, T, h dT/dx), x0, h) of EOS 2 as the library builds it on the host (no GPU needed)."""
+    import numpy as np
+
+    L = load_library()
+    nodes = np.empty((2049, 4))
+    x0, h = C.c_double(), C.c_double()
+    rc = L.vh_eos_table(nodes.ctypes.data_as(C.POINTER(C.c_double)), C.byref(x0), C.byref(h))
+    if rc != VH_OK:
+        raise VHError("vh_eos_table failed (%d)" % rc)
+    return nodes, x0.value, h.value
 
 
 def measure_peaks(n_bytes=1 << 30, repeats=10, stream=None):

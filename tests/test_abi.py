@@ -98,3 +98,24 @@ def test_inputs_are_seeded_and_reproducible():
     assert a["e"].min() >= 0.05 / inputs.HBARC * (1 - 1e-12)       # pedestal (reading R14)
     _, c, _ = inputs.config_batched2d(n_batch=2, n=12, n_hot=3)
     assert not np.array_equal(c["e"][0], c["e"][1])                 # event b uses seed + b
+
+
+def test_lattice_eos_table_of_the_product_matches_the_oracle(vo):
+    """EOS 2 (R19, R20): the CUDA library builds its table on the host with its own quadrature and root finder
+    (csrc/vh_eos_lattice.hpp); the oracle builds its own (oracle/vh_oracle_lattice.hpp).  No code is shared, so agreement of the node
+    values - here against the oracle's interpolant evaluated AT the nodes, where Hermite interpolation returns the node value -
+    checks both builders against each other before any kernel runs."""
+    import numpy as np
+    from paper_1608_06577_b200 import inputs, vh
+
+    nodes, x0, h = vh.eos_table()
+    assert nodes.shape == (2049, 4) and np.all(np.isfinite(nodes)) and np.all(np.diff(nodes[:, 0]) > 0) and np.all(np.diff(nodes[:, 2]) > 0)
+    prm = inputs.base_params(eos=2)
+    for k in (0, 1, 7, 100, 511, 1024, 1777, 2047):
+        xk = x0 + k * h
+        xe = xk * (1 + 1e-13) if k == 0 else xk          # (stay inside the table at its first node)
+        r = vo.eos(prm, xe**4)
+        assert r["p"] == pytest.approx(nodes[k, 0], rel=1e-10)
+        assert r["T"] == pytest.approx(nodes[k, 2], rel=1e-10)
+        assert r["cs2"] == pytest.approx(nodes[k, 1] / h / (4 * xk**3), rel=1e-8)
+    assert nodes[0, 2] * inputs.HBARC == pytest.approx(0.03, rel=1e-12) and nodes[-1, 2] * inputs.HBARC == pytest.approx(2.0, rel=1e-12)
