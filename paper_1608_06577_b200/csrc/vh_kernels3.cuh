@@ -159,8 +159,9 @@ __device__ __forceinline__ void relaxation_sources4(const DevParams& P, double t
 
   // transport coefficients (Eqs. 10-16; R14)
   double p, cs2;
-  eos_p_cs2<EOS>(P, e, p, cs2);
-  const double T = (EOS == 2) ? eos_temperature<EOS>(P, e) : sqrt_fast(sqrt_fast(e * P.eos_a_inv));
+  double T;
+  if (EOS == 2) eos_lattice(P, e, p, cs2, T);      // one table lookup gives all three
+  else { eos_p_cs2<EOS>(P, e, p, cs2); T = sqrt_fast(sqrt_fast(e * P.eos_a_inv)); }
   const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
   const double eotp2 = 2.0 * (e + p) * P.inv_ctaupi;
   const double zs = zeta_over_s(P, T);
