@@ -109,6 +109,12 @@ int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long*
  * synchronises the stream.  out8 is a HOST pointer to 8 doubles.                                                          */
 int vh_get_diagnostics(vh_handle* h, double* out8);
 
+/* The same eight quantities cell by cell (the maps of the paper's Figs. 15-17, :826-834, are slices of [4]..[7]):
+ * maps8[m * np + c], m = 0..7 as in vh_get_diagnostics, np = n_batch*nz*ny*nx, c = ((b*nz + k)*ny + j)*nx + i (physical cells,
+ * the layout of vh_get_fields).  maps8 holds 8*np doubles in mem_space (0 host, 1 device; a host destination goes
+ * through a temporary device buffer of that size).  One kernel; synchronises the stream.                                  */
+int vh_get_diagnostic_maps(vh_handle* h, double* maps8, int mem_space);
+
 /* Program-flow steps 6-8 (:492-494): advance until T < T_f (fm^-1) everywhere or max_steps steps have been taken, testing the
  * temperature every check_every steps (>= 1) with the reduction of vh_get_diagnostics.  *steps_done (may be NULL) receives the
  * number of steps taken by this call; returns VH_OK in both cases (compare vh_get_diagnostics()[0] with T_f to tell them apart). */

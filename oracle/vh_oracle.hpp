@@ -257,42 +257,55 @@ template <class R> class Solver {
   // out[6] max Kn_{theta pi} = tau_pi |theta|, out[7] max Kn_{theta Pi} = tau_Pi |theta| (:830) with theta of A.11 discretised as in the
   // sources (backward difference in time, central in space, :424) and the relaxation times the solver uses (R14); a cell whose
   // quotient is not finite (1/tau = 0) does not count; 0 when the sector is switched off
-  void diagnostics(double out[8]) const {
-    for (int i = 0; i < 8; ++i) out[i] = 0.0;
+  void cell_diagnostics(size_t s, double v[8]) const {      // the eight quantities at one cell (see diagnostics())
     const size_t stride[3] = {1, (size_t)NX, (size_t)NX * NY};
     const double dr[3] = {P.dx, P.dy, P.dz};
     const double t = (double)tau, t2 = (double)tau2(tau);
     const double g[4] = {1.0, -1.0, -1.0, -t2};
+    const double ee = (double)e[s], pp = (double)p[s];
+    const double T = (double)temperature(P, e[s]);
+    double uu[4], pim[4][4];
+    for (int m = 0; m < 4; ++m) uu[m] = (double)u[m][s];
+    for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pim[m][n] = (double)q[PI_SLOT[m][n]][s];
+    double norm = 0.0, tr = 0.0, pipi = 0.0, orth = 0.0;
+    for (int m = 0; m < 4; ++m) { norm += g[m] * uu[m] * uu[m]; tr += g[m] * pim[m][m]; }
+    for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pipi += g[m] * g[n] * pim[m][n] * pim[m][n];
+    for (int l = 0; l < 4; ++l) {
+      double c = 0.0;
+      for (int m = 0; m < 4; ++m) c += pim[l][m] * g[m] * uu[m];
+      if (l == 3 && milne()) c *= t;
+      orth = std::fmax(orth, std::fabs(c));
+    }
+    v[0] = T;
+    v[1] = std::fabs(norm - 1.0);
+    v[2] = std::fabs(tr) / (ee + pp);
+    v[3] = orth / (ee + pp);
+    v[4] = std::sqrt(std::fabs(pipi)) / pp;
+    v[5] = std::fabs((double)q[14][s]) / pp;
+    double theta = (milne() ? uu[0] / t : 0.0) + (uu[0] - (double)up[0][s]) / P.dtau;
+    for (int d = 0; d < 3; ++d) theta += ((double)u[d + 1][s + stride[d]] - (double)u[d + 1][s - stride[d]]) / (2.0 * dr[d]);
+    Thermo<double> th = eos<double>(P, ee);
+    th.T = T;
+    const Transport<double> tc = transport<double>(P, ee, th);
+    const double kp = std::fabs(theta) / tc.inv_tau_pi, kP = std::fabs(theta) / tc.inv_tau_Pi;
+    v[6] = ((P.physics & 1) && std::isfinite(kp)) ? kp : 0.0;
+    v[7] = ((P.physics & 2) && std::isfinite(kP)) ? kP : 0.0;
+  }
+  void diagnostics(double out[8]) const {
+    for (int i = 0; i < 8; ++i) out[i] = 0.0;
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i) {
-      const size_t s = idx(i, j, k);
-      const double ee = (double)e[s], pp = (double)p[s];
-      const double T = (double)temperature(P, e[s]);
-      double uu[4], pim[4][4];
-      for (int m = 0; m < 4; ++m) uu[m] = (double)u[m][s];
-      for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pim[m][n] = (double)q[PI_SLOT[m][n]][s];
-      double norm = 0.0, tr = 0.0, pipi = 0.0, orth = 0.0;
-      for (int m = 0; m < 4; ++m) { norm += g[m] * uu[m] * uu[m]; tr += g[m] * pim[m][m]; }
-      for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pipi += g[m] * g[n] * pim[m][n] * pim[m][n];
-      for (int l = 0; l < 4; ++l) {
-        double c = 0.0;
-        for (int m = 0; m < 4; ++m) c += pim[l][m] * g[m] * uu[m];
-        if (l == 3 && milne()) c *= t;
-        orth = std::fmax(orth, std::fabs(c));
-      }
-      out[0] = std::fmax(out[0], T);
-      out[1] = std::fmax(out[1], std::fabs(norm - 1.0));
-      out[2] = std::fmax(out[2], std::fabs(tr) / (ee + pp));
-      out[3] = std::fmax(out[3], orth / (ee + pp));
-      out[4] = std::fmax(out[4], std::sqrt(std::fabs(pipi)) / pp);
-      out[5] = std::fmax(out[5], std::fabs((double)q[14][s]) / pp);
-      double theta = (milne() ? uu[0] / t : 0.0) + (uu[0] - (double)up[0][s]) / P.dtau;
-      for (int d = 0; d < 3; ++d) theta += ((double)u[d + 1][s + stride[d]] - (double)u[d + 1][s - stride[d]]) / (2.0 * dr[d]);
-      Thermo<double> th = eos<double>(P, ee);
-      th.T = T;
-      const Transport<double> tc = transport<double>(P, ee, th);
-      const double kp = std::fabs(theta) / tc.inv_tau_pi, kP = std::fabs(theta) / tc.inv_tau_Pi;
-      if ((P.physics & 1) && std::isfinite(kp)) out[6] = std::fmax(out[6], kp);
-      if ((P.physics & 2) && std::isfinite(kP)) out[7] = std::fmax(out[7], kP);
+      double v[8];
+      cell_diagnostics(idx(i, j, k), v);
+      for (int m = 0; m < 8; ++m) out[m] = std::fmax(out[m], v[m]);
+    }
+  }
+  // the same eight quantities cell by cell (Figs. 15-17 of the paper are such maps): maps8[m * np + c], physical cells, x fastest
+  void diagnostic_maps(double* maps8, size_t np, size_t offset) const {
+    size_t c = offset;
+    for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i, ++c) {
+      double v[8];
+      cell_diagnostics(idx(i, j, k), v);
+      for (int m = 0; m < 8; ++m) maps8[m * np + c] = v[m];
     }
   }
 

@@ -64,6 +64,7 @@ def lib():
         L.vho_get_status.argtypes = [C.c_void_p, dp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), dp]
         L.vho_last_failure.argtypes = [C.c_void_p, C.c_int, dp]
         L.vho_diagnostics.argtypes = [C.c_void_p, dp]
+        L.vho_diagnostic_maps.argtypes = [C.c_void_p, dp]
         L.vho_raw.restype = dp
         L.vho_raw.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.vho_set_tau.argtypes = [C.c_void_p, C.c_double]
@@ -150,6 +151,11 @@ class Oracle:
         out = np.empty(8)
         self.L.vho_diagnostics(self.h, _dp(out))
         return dict(zip(DIAG_NAMES, out))
+
+    def diagnostic_maps(self):
+        out = np.empty((8,) + self.shape)
+        self.L.vho_diagnostic_maps(self.h, _dp(out))
+        return out
 
     def last_failure(self, ev=0):
         out = np.empty(4)

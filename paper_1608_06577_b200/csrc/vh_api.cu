@@ -152,12 +152,12 @@ static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, d
 }
 
 template <int EOS>
-static void launch_diag(vh_handle* h, double t) {
+static void launch_diag(vh_handle* h, double t, double* maps) {
   const DevParams& P = h->P;
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const unsigned nb = (unsigned)std::min<long long>((np + 255) / 256, 2048LL);      // grid-stride loop
-  if (h->prm.geometry == 0) diagnostics_kernel<EOS, true><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1], t, h->diag);
-  else diagnostics_kernel<EOS, false><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1], t, h->diag);
+  if (h->prm.geometry == 0) diagnostics_kernel<EOS, true><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1], t, h->diag, maps);
+  else diagnostics_kernel<EOS, false><<<nb, 256, 0, h->stream>>>(P, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1], t, h->diag, maps);
   h->launches++;
 }
 
@@ -468,12 +468,36 @@ int vh_get_diagnostics(vh_handle* h, double* out8) {
   if (!h->diag && cudaMalloc((void**)&h->diag, 8 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
   CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 8 * sizeof(unsigned long long), h->stream));
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
-  if (h->prm.eos == 2) launch_diag<2>(h, t); else if (h->prm.eos == 1) launch_diag<1>(h, t); else launch_diag<0>(h, t);
+  if (h->prm.eos == 2) launch_diag<2>(h, t, nullptr); else if (h->prm.eos == 1) launch_diag<1>(h, t, nullptr); else launch_diag<0>(h, t, nullptr);
   CUDA_TRY(h, cudaGetLastError());
   unsigned long long bits[8];
   CUDA_TRY(h, cudaMemcpyAsync(bits, h->diag, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   std::memcpy(out8, bits, sizeof(bits));
+  return VH_OK;
+}
+
+int vh_get_diagnostic_maps(vh_handle* h, double* maps8, int mem_space) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!maps8) return fail(h, VH_ERR_ARG, "maps8 is NULL");
+  if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
+  if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostic_maps before vh_set_initial");
+  if (!h->diag && cudaMalloc((void**)&h->diag, 8 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
+  const size_t bytes = (size_t)8 * h->P.nx * h->P.ny * h->P.nz * h->P.n_batch * sizeof(double);
+  double* dev = maps8;
+  if (mem_space == 0) {
+    if (cudaMalloc(&dev, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, VH_ERR_ALLOC, "device allocation for the maps failed"); }
+  }
+  cudaError_t ce = cudaMemsetAsync(h->diag, 0, 8 * sizeof(unsigned long long), h->stream);
+  const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
+  if (ce == cudaSuccess) {
+    if (h->prm.eos == 2) launch_diag<2>(h, t, dev); else if (h->prm.eos == 1) launch_diag<1>(h, t, dev); else launch_diag<0>(h, t, dev);
+    ce = cudaGetLastError();
+  }
+  if (ce == cudaSuccess && mem_space == 0) ce = cudaMemcpyAsync(maps8, dev, bytes, cudaMemcpyDeviceToHost, h->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
+  if (mem_space == 0) cudaFree(dev);
+  if (ce != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string("vh_get_diagnostic_maps: ") + cudaGetErrorString(ce));
   return VH_OK;
 }
 

@@ -405,7 +405,7 @@ __global__ void __launch_bounds__(256) pressure_kernel(const __grid_constant__ D
 template <int EOS, bool MILNE>
 __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant__ DevParams P, const double* __restrict__ q, const double* __restrict__ e,
                                                           const double* __restrict__ p, const double* __restrict__ u, const double* __restrict__ u_prev,
-                                                          double t, unsigned long long* __restrict__ out) {
+                                                          double t, unsigned long long* __restrict__ out, double* __restrict__ maps) {
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const long long fs = P.fstride;
   const double t2 = MILNE ? t * t : 1.0;
@@ -431,25 +431,32 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     const double c2 = pi[2] * ut - pi[5] * ux - pi[7] * uy - t2 * pi[8] * un;
     const double c3 = (pi[3] * ut - pi[6] * ux - pi[8] * uy - t2 * pi[9] * un) * (MILNE ? t : 1.0);
     const double iw = 1.0 / (ee + pp), ip = 1.0 / pp;
-    m[0] = fmax(m[0], eos_temperature<EOS>(P, ee));
-    m[1] = fmax(m[1], fabs(norm - 1.0));
-    m[2] = fmax(m[2], fabs(tr) * iw);
-    m[3] = fmax(m[3], fmax(fmax(fabs(c0), fabs(c1)), fmax(fabs(c2), fabs(c3))) * iw);
-    m[4] = fmax(m[4], sqrt(fabs(pipi)) * ip);
-    m[5] = fmax(m[5], fabs(Pi) * ip);
+    double v[8];
+    v[1] = fabs(norm - 1.0);
+    v[2] = fabs(tr) * iw;
+    v[3] = fmax(fmax(fabs(c0), fabs(c1)), fmax(fabs(c2), fabs(c3))) * iw;
+    v[4] = sqrt(fabs(pipi)) * ip;
+    v[5] = fabs(Pi) * ip;
     // Knudsen numbers: theta = u^tau/tau + d_tau u^tau + d_i u^i (A.11), backward in time, central in space (:424)
     double theta = (MILNE ? ut / t : 0.0) + (ut - u_prev[c]) * P.inv_dtau;
     theta += (u[fs + c + 1] - u[fs + c - 1]) * (0.5 * P.inv_dx) + (u[2 * fs + c + P.NXp] - u[2 * fs + c - P.NXp]) * (0.5 * P.inv_dy);
     if (P.NZp > 1) theta += (u[3 * fs + c + P.plane] - u[3 * fs + c - P.plane]) * (0.5 * P.inv_dz);
     const double T = eos_temperature<EOS>(P, ee);
+    v[0] = T;
     double p0, cs2;
     eos_p_cs2<EOS>(P, ee, p0, cs2);
     const double itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
     const double zs = zeta_over_s(P, T), bb = (1.0 / 3.0) - cs2;
     const double itP = fmin((zs > 0.0) ? T * bb * bb * P.inv_ctauPi / zs : CUDART_INF, P.relax_clamp);
     const double kp = fabs(theta) / itp, kP = fabs(theta) / itP;
-    if (P.shear && isfinite(kp)) m[6] = fmax(m[6], kp);
-    if (P.bulk && isfinite(kP)) m[7] = fmax(m[7], kP);
+    v[6] = (P.shear && isfinite(kp)) ? kp : 0.0;
+    v[7] = (P.bulk && isfinite(kP)) ? kP : 0.0;
+#pragma unroll
+    for (int s = 0; s < 8; ++s) m[s] = fmax(m[s], v[s]);
+    if (maps) {                      // the same quantities cell by cell: maps[s * np + n], physical cells, x fastest
+#pragma unroll
+      for (int s = 0; s < 8; ++s) maps[s * np + n] = v[s];
+    }
   }
 #pragma unroll
   for (int s = 0; s < 8; ++s) {

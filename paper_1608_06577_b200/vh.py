@@ -30,7 +30,7 @@ class vh_params(C.Structure):
 
 
 # every symbol include/vh.h declares
-EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_run_until", "vh_eos_table", "vh_launch_count",
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_run_until", "vh_eos_table", "vh_launch_count",
            "vh_set_kernel_variant", "vh_measure_peaks", "vh_last_error", "vh_destroy"]
 
 _lib = None
@@ -56,6 +56,7 @@ def load_library():
     L.vh_get_fields.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
     L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     L.vh_get_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
+    L.vh_get_diagnostic_maps.argtypes = [vp, vp, C.c_int]
     L.vh_run_until.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
     L.vh_eos_table.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.vh_launch_count.argtypes = [vp]
@@ -213,6 +214,14 @@ class Solver:
         out = (C.c_double * 8)()
         self._check(self.L.vh_get_diagnostics(self.h, out), "vh_get_diagnostics")
         return dict(zip(self.DIAG_NAMES, list(out)))
+
+    def diagnostic_maps(self, device=None):
+        """The eight quantities of diagnostics() cell by cell: tensor [8, n_batch, nz, ny, nx] (order of DIAG_NAMES, without 'max_')."""
+        torch = self.torch
+        dev = self.device if device is None else torch.device(device)
+        out = torch.empty((8,) + self.shape, dtype=torch.float64, device=dev)
+        self._check(self.L.vh_get_diagnostic_maps(self.h, _ptr(out), self._space([out])), "vh_get_diagnostic_maps")
+        return out
 
     def run_until(self, T_f, max_steps, check_every=10):
         """Advance until T < T_f everywhere or max_steps steps (PAPER.md :494); returns the number of steps taken."""

@@ -426,6 +426,20 @@ def test_diagnostics_and_freeze_out_termination(vh, vo):
                 assert dg[k] < 1e-14 and do[k] < 1e-14
             else:
                 assert dg[k] == pytest.approx(do[k], rel=1e-9), k
+        # the same quantities cell by cell (vh_get_diagnostic_maps), to a device and to a host destination
+        mo = o.diagnostic_maps()
+        # 1/tau_Pi carries (1/3 - c_s^2)^2 (Eq. 18): where the EOS is conformal to within 1e-9 the rounding of c_s^2 is amplified
+        # by (1/3)/|1/3 - c_s^2| in the bulk Knudsen number - a per-cell allowance of 16 ulp of c_s^2 times that factor
+        bb = np.abs(1.0 / 3.0 - np.vectorize(lambda ee: vo.eos(prm, ee)["cs2"])(o.get_fields()["e"]))
+        slack = {"max_knudsen_bulk": 16 * np.finfo(float).eps / 3.0 / np.maximum(bb, 1e-300) * mo[7]}
+        for dev in ("cuda:0", "cpu"):
+            mg = s.diagnostic_maps(device=dev).cpu().numpy()
+            for k, name in enumerate(do):
+                if name == "max_norm_violation":
+                    assert mg[k].max() < 1e-14
+                else:
+                    assert np.all(np.abs(mg[k] - mo[k]) <= 1e-9 * mo[k].max() + slack.get(name, 0.0)), name
+                    assert mg[k].max() == dg[name]
         T_f = 0.97 * do["max_T"]             # a freeze-out temperature the cooling system crosses within a few steps
         n_o = 0
         while o.diagnostics()["max_T"] >= T_f and n_o < 200:

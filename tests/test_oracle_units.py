@@ -270,4 +270,11 @@ def test_diagnostics_against_their_definitions(vo):
     it_Pi = np.vectorize(lambda ee: vo.transport(prm, ee)["inv_tau_Pi"])(e)
     assert d["max_knudsen_shear"] == pytest.approx(np.max(np.abs(theta) / it_pi), rel=1e-12)
     assert d["max_knudsen_bulk"] == pytest.approx(np.max(np.abs(theta) / it_Pi), rel=1e-12)
+    # the per-cell maps (Figs. 15-17 are slices of such maps) against the same numpy expressions, cell by cell
+    m = o.diagnostic_maps()[:, 0]
+    ref = [(e / prm["eos_a"]) ** 0.25, np.abs(np.einsum("m,m...->...", g, u * u) - 1), np.abs(np.einsum("m,mm...->...", g, pi)) / (e + p),
+           c.max(axis=0) / (e + p), np.sqrt(np.abs(pipi)) / p, np.abs(f["q"][14]) / p, np.abs(theta) / it_pi, np.abs(theta) / it_Pi]
+    for k, r in enumerate(ref):
+        np.testing.assert_allclose(m[k], r[0], rtol=1e-11, atol=1e-13 * max(np.max(r), 1e-3), err_msg=str(k))
+        assert np.max(m[k]) == list(d.values())[k]
     assert d["max_norm_violation"] < 1e-14 and 0 < d["max_trace_violation"] < 0.05      # u.u = 1 after inversion (:489); constraints drift slowly (:333)
