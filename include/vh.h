@@ -100,20 +100,24 @@ int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long*
                   long long* n_nonfinite, double* min_reg_factor);
 
 /* On-device diagnostics of the current state, maxima over all physical cells and events, written to
- * out8[0..7]:  [0] max T in fm^-1 (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  [1] max |u.u - 1| (:489);
+ * out10[0..9]:  [0] max T in fm^-1 (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  [1] max |u.u - 1| (:489);
  * [2] max |g_{mu nu} pi^{mu nu}|/(e+p) and [3] max over lambda of |pi^{lambda mu} u_mu|/(e+p) (the constraints of Eqs. 47-51,
  * :318-331, which are propagated, not enforced; the lambda = eta entry is multiplied by tau);  [4] max R_pi^-1 =
  * sqrt(pi^{mu nu} pi_{mu nu})/P0 and [5] max R_Pi^-1 = |Pi|/P0 (inverse Reynolds numbers, Eq. 89, :826);  [6] max Kn = tau_pi |theta|
  * and [7] max tau_Pi |theta| (Knudsen numbers, :830; theta of A.11 with the finite differences of the source terms, :424, and the
- * relaxation times the solver uses; cells with 1/tau = 0 do not count; 0 if the sector is off).  One reduction kernel;
- * synchronises the stream.  out8 is a HOST pointer to 8 doubles.                                                          */
-int vh_get_diagnostics(vh_handle* h, double* out8);
+ * relaxation times the solver uses; cells with 1/tau = 0 do not count; 0 if the sector is off);  [8] max (R_pi^(2))^-1 =
+ * sqrt(J^{mu nu} J_{mu nu})/(2 eta sqrt(sigma^{mu nu} sigma_{mu nu})) and [9] max (R_Pi^(2))^-1 = |J|/(zeta |theta|), the second-order
+ * inverse Reynolds numbers of Eq. 90 (:831) with J^{mu nu}, J of Eq. 5 at n^mu = 0, built from the terms I2, I3, I4 of Eqs. 41-46
+ * and the kinematics of App. A exactly as the source terms build them (cells with 0/0 do not count; 0 if the sector is off).
+ * One reduction kernel; synchronises the stream.  out10 is a HOST pointer to VH_N_DIAGNOSTICS = 10 doubles.               */
+#define VH_N_DIAGNOSTICS 10
+int vh_get_diagnostics(vh_handle* h, double* out10);
 
-/* The same eight quantities cell by cell (the maps of the paper's Figs. 15-17, :826-834, are slices of [4]..[7]):
- * maps8[m * np + c], m = 0..7 as in vh_get_diagnostics, np = n_batch*nz*ny*nx, c = ((b*nz + k)*ny + j)*nx + i (physical cells,
- * the layout of vh_get_fields).  maps8 holds 8*np doubles in mem_space (0 host, 1 device; a host destination goes
+/* The same ten quantities cell by cell (the maps of the paper's Figs. 15-16, :826-834, are slices of [4]..[9]):
+ * maps10[m * np + c], m = 0..9 as in vh_get_diagnostics, np = n_batch*nz*ny*nx, c = ((b*nz + k)*ny + j)*nx + i (physical cells,
+ * the layout of vh_get_fields).  maps10 holds 10*np doubles in mem_space (0 host, 1 device; a host destination goes
  * through a temporary device buffer of that size).  One kernel; synchronises the stream.                                  */
-int vh_get_diagnostic_maps(vh_handle* h, double* maps8, int mem_space);
+int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space);
 
 /* Program-flow steps 6-8 (:492-494): advance until T < T_f (fm^-1) everywhere or max_steps steps have been taken, testing the
  * temperature every check_every steps (>= 1) with the reduction of vh_get_diagnostics.  *steps_done (may be NULL) receives the

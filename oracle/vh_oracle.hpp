@@ -19,7 +19,7 @@
 //     (Eqs. 73-74, reading R9) is pinned only through hand-computed values of rho for simple states
 //     (tests/test_oracle_units.py): "parity unpinned" beyond that - no printed solution exercises rho >~ 1; applied literally it makes
 //     the discrete Gubser run ill-conditioned ("config 2").  The lattice EOS (eos = 2, vh_oracle_lattice.hpp,
-//     readings R19, R20) is pinned by tests/test_oracle_lattice.py, zeta/s of Eq. 17 and diagnostics() by tests/test_oracle_units.py.
+//     readings R19, R20) is pinned by tests/test_oracle_lattice.py, zeta/s of Eq. 17 and diagnostics() (incl. Eq. 90, reading R21) by tests/test_oracle_units.py.
 //
 // The scalar type is a template parameter so that an operation-counting type can be
 // substituted (oracle/vh_oracle_capi.cpp instantiates double and a counting type).
@@ -253,11 +253,11 @@ template <class R> class Solver {
   // ------------------------------------------------------------ diagnostics, maxima over the physical cells
   // out[0] max T (freeze-out test "T < T_f everywhere", program-flow step 8, :494);  out[1] max |u.u - 1| (:489);
   // out[2] max |g_{mu nu} pi^{mu nu}|/(e+p), out[3] max_lambda |pi^{lambda mu} u_mu|/(e+p) (Eqs. 47-51, :318-331; the lambda = eta
-  // entry times tau);  out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826);
+  // entry times tau);  out[8], out[9]: second-order inverse Reynolds numbers of Eq. 90 (see cell_diagnostics);  out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826);
   // out[6] max Kn_{theta pi} = tau_pi |theta|, out[7] max Kn_{theta Pi} = tau_Pi |theta| (:830) with theta of A.11 discretised as in the
   // sources (backward difference in time, central in space, :424) and the relaxation times the solver uses (R14); a cell whose
   // quotient is not finite (1/tau = 0) does not count; 0 when the sector is switched off
-  void cell_diagnostics(size_t s, double v[8]) const {      // the eight quantities at one cell (see diagnostics())
+  void cell_diagnostics(size_t s, double v[10]) {      // the ten quantities at one cell (see diagnostics())
     const size_t stride[3] = {1, (size_t)NX, (size_t)NX * NY};
     const double dr[3] = {P.dx, P.dy, P.dz};
     const double t = (double)tau, t2 = (double)tau2(tau);
@@ -290,22 +290,27 @@ template <class R> class Solver {
     const double kp = std::fabs(theta) / tc.inv_tau_pi, kP = std::fabs(theta) / tc.inv_tau_Pi;
     v[6] = ((P.physics & 1) && std::isfinite(kp)) ? kp : 0.0;
     v[7] = ((P.physics & 2) && std::isfinite(kP)) ? kP : 0.0;
+    // second-order inverse Reynolds numbers (Eq. 90, :831) from the terms of the source routine; 0 where 0/0 or the sector is off
+    R J[NQ], second[2];
+    sources(q, e, p, u, up, s, tau, J, second);
+    v[8] = std::isfinite((double)second[0]) ? (double)second[0] : 0.0;
+    v[9] = std::isfinite((double)second[1]) ? (double)second[1] : 0.0;
   }
-  void diagnostics(double out[8]) const {
-    for (int i = 0; i < 8; ++i) out[i] = 0.0;
+  void diagnostics(double out[10]) {
+    for (int i = 0; i < 10; ++i) out[i] = 0.0;
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i) {
-      double v[8];
+      double v[10];
       cell_diagnostics(idx(i, j, k), v);
-      for (int m = 0; m < 8; ++m) out[m] = std::fmax(out[m], v[m]);
+      for (int m = 0; m < 10; ++m) out[m] = std::fmax(out[m], v[m]);
     }
   }
-  // the same eight quantities cell by cell (Figs. 15-17 of the paper are such maps): maps8[m * np + c], physical cells, x fastest
-  void diagnostic_maps(double* maps8, size_t np, size_t offset) const {
+  // the same ten quantities cell by cell (Figs. 15-17 of the paper are such maps): maps[m * np + c], physical cells, x fastest
+  void diagnostic_maps(double* maps, size_t np, size_t offset) {
     size_t c = offset;
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i, ++c) {
-      double v[8];
+      double v[10];
       cell_diagnostics(idx(i, j, k), v);
-      for (int m = 0; m < 8; ++m) maps8[m * np + c] = v[m];
+      for (int m = 0; m < 10; ++m) maps[m * np + c] = v[m];
     }
   }
 
@@ -373,7 +378,7 @@ template <class R> class Solver {
 
   // ------------------------------------------------------------ sources J = S + G  (App. B; Eqs. 39-46; App. A index forms)
   void sources(const std::vector<R>* qi, const std::vector<R>& ei, const std::vector<R>& pi_, const std::vector<R>* ui,
-               const std::vector<R>* uprev, size_t s, R t, R J[NQ]) {
+               const std::vector<R>* uprev, size_t s, R t, R J[NQ], R* second = nullptr) {
     const size_t stride[3] = {1, (size_t)NX, (size_t)NX * NY};
     const R dr[3] = {R(P.dx), R(P.dy), R(P.dz)};
     const bool mil = milne();
@@ -412,6 +417,7 @@ template <class R> class Solver {
       J[2] -= qi[2][s] / t;
       J[3] -= R(3) * qi[3][s] / t;
     }
+    if (second) second[0] = second[1] = R(0);
     if ((P.physics & 3) == 0) return;     // ideal mode: pi, Pi stay zero
 
     // ---- velocity gradients: backward difference in time, central in space (:424)
@@ -466,6 +472,7 @@ template <class R> class Solver {
     R pisig = R(0);                        // pi^{mu nu} sigma_{mu nu}
     for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) pisig += g[m] * g[n] * pic[m][n] * sig[m][n];
 
+    R JJ = R(0), sigsig = R(0);            // J^{mu nu} J_{mu nu} / tau_pi^2 and sigma^{mu nu} sigma_{mu nu}  (Eq. 90)
     if (P.physics & 1) {
       for (int m = 0; m < 4; ++m) for (int n = m; n < 4; ++n) {
         R I1 = R(0), I3 = R(0), I4 = R(0);
@@ -478,6 +485,10 @@ template <class R> class Solver {
         I4 -= Delta[m][n] * pisig / R(3);
         R I2 = theta * pic[m][n];                                                                 // Eq. 44
         R Ipi = I1 + R(P.delta_pipi) * I2 - I3 + R(P.tau_pipi) * I4 - R(P.lambda_piPi) * Pic * sig[m][n];   // Eq. 42
+        // Eq. 5 with n^mu = 0: J^{mu nu}/tau_pi = -(Ipi - I1)  (I1 belongs to the projected time derivative, not to J)
+        const R w = g[m] * g[n] * ((m == n) ? R(1) : R(2));
+        JJ += w * (Ipi - I1) * (Ipi - I1);
+        sigsig += w * sig[m][n] * sig[m][n];
         R Gpi = R(0);                                                                             // :300, R1, R2
         for (int c = 0; c < nG; ++c) {
           if (G3[c].l == m) Gpi += uc[G3[c].a] * G3[c].v * pic[G3[c].b][n];
@@ -490,7 +501,9 @@ template <class R> class Solver {
     if (P.physics & 2) {
       R IPi = R(P.delta_PiPi) * Pic * theta - tc.lambda_Pipi_over_tau_Pi * pisig;                 // Eq. 41
       J[14] = (-tc.zeta_over_tau_Pi * theta - Pic * tc.inv_tau_Pi - IPi) / uc[0] + Pic * divv;    // B.10
+      if (second) second[1] = absr(IPi) / (tc.zeta_over_tau_Pi * absr(theta));                   // Eq. 90: |J|/(zeta |theta|), J/tau_Pi = -IPi
     }
+    if (second && (P.physics & 1)) second[0] = sqrt(absr(JJ)) / (R(2) * tc.eta_over_tau_pi * sqrt(absr(sigsig)));   // Eq. 90
   }
 
   // ------------------------------------------------------------ forward Euler step E[w] = w + dtau C[w]  (Eq. 59, :413)

@@ -148,12 +148,12 @@ class Oracle:
         return {"tau": tau.value, "n_steps": a.value, "n_inversion_failures": b.value, "n_nonfinite": c.value, "min_reg_factor": mr.value}
 
     def diagnostics(self):
-        out = np.empty(8)
+        out = np.empty(10)
         self.L.vho_diagnostics(self.h, _dp(out))
         return dict(zip(DIAG_NAMES, out))
 
     def diagnostic_maps(self):
-        out = np.empty((8,) + self.shape)
+        out = np.empty((10,) + self.shape)
         self.L.vho_diagnostic_maps(self.h, _dp(out))
         return out
 
@@ -215,7 +215,7 @@ def invert(params: dict, E, M2, Pi, guess):
 
 
 DIAG_NAMES = ("max_T", "max_norm_violation", "max_trace_violation", "max_transversality_violation", "max_inv_reynolds_shear", "max_inv_reynolds_bulk",
-              "max_knudsen_shear", "max_knudsen_bulk")
+              "max_knudsen_shear", "max_knudsen_bulk", "max_inv_reynolds2_shear", "max_inv_reynolds2_bulk")
 OP_CLASSES = ("add", "mul", "div", "cmp", "sqrt", "exp", "pow", "tanh")
 # flop weights of SURVEY.md 8(d): add/mul/compare 1, div 10, sqrt 15, exp 25, tanh 40; pow(x, 1/4) = two sqrt
 OP_WEIGHTS = dict(add=1, mul=1, div=10, cmp=1, sqrt=15, exp=25, pow=30, tanh=40)

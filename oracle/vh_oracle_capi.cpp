@@ -71,15 +71,15 @@ int vho_get_status(vho_handle* h, double* tau, long long* n_steps, long long* n_
 }
 
 // maxima over all events of Solver::diagnostics (double instantiation only)
-void vho_diagnostics(vho_handle* h, double* out8) {
-  for (int i = 0; i < 8; ++i) out8[i] = 0.0;
-  for (Sol* s : h->ev) { double o[8]; s->diagnostics(o); for (int i = 0; i < 8; ++i) if (o[i] > out8[i]) out8[i] = o[i]; }
+void vho_diagnostics(vho_handle* h, double* out10) {
+  for (int i = 0; i < 10; ++i) out10[i] = 0.0;
+  for (Sol* s : h->ev) { double o[10]; s->diagnostics(o); for (int i = 0; i < 10; ++i) if (o[i] > out10[i]) out10[i] = o[i]; }
 }
-// per-cell maps of the eight diagnostics: maps8[m * np + c], np = all physical cells of all events
-void vho_diagnostic_maps(vho_handle* h, double* maps8) {
+// per-cell maps of the ten diagnostics: maps[m * np + c], np = all physical cells of all events
+void vho_diagnostic_maps(vho_handle* h, double* maps) {
   const vho::Params& P = h->ev[0]->P;
   const size_t ne = (size_t)P.nx * P.ny * P.nz, np = ne * h->ev.size();
-  for (size_t b = 0; b < h->ev.size(); ++b) h->ev[b]->diagnostic_maps(maps8, np, b * ne);
+  for (size_t b = 0; b < h->ev.size(); ++b) h->ev[b]->diagnostic_maps(maps, np, b * ne);
 }
 void vho_last_failure(vho_handle* h, int ev, double* out4) { for (int i = 0; i < 4; ++i) out4[i] = h->ev[ev]->last_fail[i]; }
 

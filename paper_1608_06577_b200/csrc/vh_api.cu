@@ -461,40 +461,40 @@ int vh_eos_table(double* nodes4, double* x0, double* h) {
   return VH_OK;
 }
 
-int vh_get_diagnostics(vh_handle* h, double* out8) {
+int vh_get_diagnostics(vh_handle* h, double* out10) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostics before vh_set_initial");
-  if (!out8) return fail(h, VH_ERR_ARG, "out8 is NULL");
-  if (!h->diag && cudaMalloc((void**)&h->diag, 8 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
-  CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 8 * sizeof(unsigned long long), h->stream));
+  if (!out10) return fail(h, VH_ERR_ARG, "out10 is NULL");
+  if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
+  CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 10 * sizeof(unsigned long long), h->stream));
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
   if (h->prm.eos == 2) launch_diag<2>(h, t, nullptr); else if (h->prm.eos == 1) launch_diag<1>(h, t, nullptr); else launch_diag<0>(h, t, nullptr);
   CUDA_TRY(h, cudaGetLastError());
-  unsigned long long bits[8];
+  unsigned long long bits[10];
   CUDA_TRY(h, cudaMemcpyAsync(bits, h->diag, sizeof(bits), cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-  std::memcpy(out8, bits, sizeof(bits));
+  std::memcpy(out10, bits, sizeof(bits));
   return VH_OK;
 }
 
-int vh_get_diagnostic_maps(vh_handle* h, double* maps8, int mem_space) {
+int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
-  if (!maps8) return fail(h, VH_ERR_ARG, "maps8 is NULL");
+  if (!maps10) return fail(h, VH_ERR_ARG, "maps10 is NULL");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostic_maps before vh_set_initial");
-  if (!h->diag && cudaMalloc((void**)&h->diag, 8 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
-  const size_t bytes = (size_t)8 * h->P.nx * h->P.ny * h->P.nz * h->P.n_batch * sizeof(double);
-  double* dev = maps8;
+  if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
+  const size_t bytes = (size_t)10 * h->P.nx * h->P.ny * h->P.nz * h->P.n_batch * sizeof(double);
+  double* dev = maps10;
   if (mem_space == 0) {
     if (cudaMalloc(&dev, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, VH_ERR_ALLOC, "device allocation for the maps failed"); }
   }
-  cudaError_t ce = cudaMemsetAsync(h->diag, 0, 8 * sizeof(unsigned long long), h->stream);
+  cudaError_t ce = cudaMemsetAsync(h->diag, 0, 10 * sizeof(unsigned long long), h->stream);
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
   if (ce == cudaSuccess) {
     if (h->prm.eos == 2) launch_diag<2>(h, t, dev); else if (h->prm.eos == 1) launch_diag<1>(h, t, dev); else launch_diag<0>(h, t, dev);
     ce = cudaGetLastError();
   }
-  if (ce == cudaSuccess && mem_space == 0) ce = cudaMemcpyAsync(maps8, dev, bytes, cudaMemcpyDeviceToHost, h->stream);
+  if (ce == cudaSuccess && mem_space == 0) ce = cudaMemcpyAsync(maps10, dev, bytes, cudaMemcpyDeviceToHost, h->stream);
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
   if (mem_space == 0) cudaFree(dev);
   if (ce != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string("vh_get_diagnostic_maps: ") + cudaGetErrorString(ce));
@@ -506,7 +506,7 @@ int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long 
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_run_until before vh_set_initial");
   if (max_steps < 0 || check_every < 1 || !(T_f >= 0.0)) return fail(h, VH_ERR_ARG, "max_steps >= 0, check_every >= 1, T_f >= 0 required");
   long long done = 0;
-  double d[8];
+  double d[10];
   while (done < max_steps) {
     int rc = vh_get_diagnostics(h, d);
     if (rc) return rc;

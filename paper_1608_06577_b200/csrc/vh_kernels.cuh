@@ -402,6 +402,61 @@ __global__ void __launch_bounds__(256) pressure_kernel(const __grid_constant__ D
 // times tau); out[4] max R_pi^-1 = sqrt(pi^{mu nu} pi_{mu nu})/P0, out[5] max R_Pi^-1 = |Pi|/P0 (Eq. 89, :826); out[6], out[7] max Knudsen
 // numbers tau_pi |theta|, tau_Pi |theta| (:830): theta of A.11 with the differences of the sources (:424) and the solver's relaxation
 // times (R14); cells with a non-finite quotient do not count, a switched-off sector gives 0.
+// Second-order inverse Reynolds numbers (Eq. 90, :831): sqrt(J^{mu nu} J_{mu nu})/(2 eta sqrt(sigma^{mu nu} sigma_{mu nu})) and |J|/(zeta |theta|) with
+// J^{mu nu}, J of Eq. 5 at n^mu = 0.  In the notation of Eqs. 41-46: J^{mu nu}/tau_pi = -(delta_pipi I2 - I3 + tau_pipi I4 - lambda_piPi Pi sigma^{mu nu}),
+// J/tau_Pi = -(delta_PiPi Pi theta - lambda_Pipi pi^{mu nu} sigma_{mu nu}); eta/tau_pi and zeta/tau_Pi are the ratios the solver uses.
+template <int EOS>
+__device__ __forceinline__ void second_order_reynolds(const DevParams& P, double t, const double u[4], const Kin& K, const double pi[10], double Pi,
+                                                      double e, double& r2_shear, double& r2_bulk) {
+  const double t2 = t * t, it = 1.0 / t;
+  const double g[4] = {1.0, -1.0, -1.0, -t2};
+  const double gi[4] = {1.0, -1.0, -1.0, -it * it};
+  double p0, cs2;
+  eos_p_cs2<EOS>(P, e, p0, cs2);
+  const double T = eos_temperature<EOS>(P, e);
+  const double eotp = (e + p0) * P.inv_ctaupi;
+  const double zs = zeta_over_s(P, T), b = (1.0 / 3.0) - cs2;
+  const double itP = fmin((zs > 0.0) ? T * b * b * P.inv_ctauPi / zs : CUDART_INF, P.relax_clamp);
+  const double zotP = (zs > 0.0) ? zs * ((e + p0) / T) * itP : 0.0;
+  double S[4][4], W[4][4], Pm[4][4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = 0; n < 4; ++n) { S[m][n] = K.sig[sym(m, n)]; Pm[m][n] = pi[sym(m, n)]; }
+  W[0][0] = W[1][1] = W[2][2] = W[3][3] = 0.0;
+  W[0][1] = K.W[0]; W[0][2] = K.W[1]; W[0][3] = K.W[2]; W[1][2] = K.W[3]; W[1][3] = K.W[4]; W[2][3] = K.W[5];
+  W[1][0] = -K.W[0]; W[2][0] = -K.W[1]; W[3][0] = -K.W[2]; W[2][1] = -K.W[3]; W[3][1] = -K.W[4]; W[3][2] = -K.W[5];
+  double B[4][4], C[4][4];      // B^{mu nu} = pi^{mu l} g_l W^{l nu};  C^{mu nu} = g_l pi^{mu l} sigma^{nu l}
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = 0; n < 4; ++n) {
+      double bb = 0.0, cc = 0.0;
+#pragma unroll
+      for (int l = 0; l < 4; ++l) { bb += Pm[m][l] * g[l] * W[l][n]; cc += g[l] * Pm[m][l] * S[n][l]; }
+      B[m][n] = bb; C[m][n] = cc;
+    }
+  const double pisig = g[0] * C[0][0] + g[1] * C[1][1] + g[2] * C[2][2] + g[3] * C[3][3];
+  double JJ = 0.0, ss = 0.0;
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = m; n < 4; ++n) {
+      const int s = sym(m, n);
+      const double Dmn = ((m == n) ? gi[m] : 0.0) - u[m] * u[n];
+      const double I2 = K.theta * pi[s];
+      const double I3 = kVorticitySign * (B[m][n] + B[n][m]);
+      const double I4 = 0.5 * (C[m][n] + C[n][m]) - (1.0 / 3.0) * Dmn * pisig;
+      const double Jh = P.delta_pipi * I2 - I3 + P.tau_pipi * I4 - P.lambda_piPi * Pi * K.sig[s];
+      const double w = g[m] * g[n] * ((m == n) ? 1.0 : 2.0);
+      JJ += w * Jh * Jh;
+      ss += w * K.sig[s] * K.sig[s];
+    }
+  const double IPi = P.delta_PiPi * Pi * K.theta - P.lambda_Pipi_coef * b * pisig;
+  r2_shear = sqrt(fabs(JJ)) / (2.0 * eotp * sqrt(fabs(ss)));
+  r2_bulk = fabs(IPi) / (zotP * fabs(K.theta));
+}
+
 template <int EOS, bool MILNE>
 __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant__ DevParams P, const double* __restrict__ q, const double* __restrict__ e,
                                                           const double* __restrict__ p, const double* __restrict__ u, const double* __restrict__ u_prev,
@@ -409,7 +464,7 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const long long fs = P.fstride;
   const double t2 = MILNE ? t * t : 1.0;
-  double m[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  double m[10] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < np; n += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(n % P.nx);
     const int j = (int)((n / P.nx) % P.ny);
@@ -431,7 +486,7 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     const double c2 = pi[2] * ut - pi[5] * ux - pi[7] * uy - t2 * pi[8] * un;
     const double c3 = (pi[3] * ut - pi[6] * ux - pi[8] * uy - t2 * pi[9] * un) * (MILNE ? t : 1.0);
     const double iw = 1.0 / (ee + pp), ip = 1.0 / pp;
-    double v[8];
+    double v[10];
     v[1] = fabs(norm - 1.0);
     v[2] = fabs(tr) * iw;
     v[3] = fmax(fmax(fabs(c0), fabs(c1)), fmax(fabs(c2), fabs(c3))) * iw;
@@ -441,6 +496,27 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     double theta = (MILNE ? ut / t : 0.0) + (ut - u_prev[c]) * P.inv_dtau;
     theta += (u[fs + c + 1] - u[fs + c - 1]) * (0.5 * P.inv_dx) + (u[2 * fs + c + P.NXp] - u[2 * fs + c - P.NXp]) * (0.5 * P.inv_dy);
     if (P.NZp > 1) theta += (u[3 * fs + c + P.plane] - u[3 * fs + c - P.plane]) * (0.5 * P.inv_dz);
+    v[8] = 0.0; v[9] = 0.0;
+    if constexpr (MILNE) {
+      if (P.shear || P.bulk) {       // Eq. 90: velocity gradients as in the source terms (:424), kinematics of App. A
+        const double uc[4] = {ut, ux, uy, un};
+        double dt[4], dx[4], dy[4], dn[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+          const double* ua = u + a * fs + c;
+          dt[a] = (ua[0] - u_prev[a * fs + c]) * P.inv_dtau;
+          dx[a] = (ua[1] - ua[-1]) * (0.5 * P.inv_dx);
+          dy[a] = (ua[P.NXp] - ua[-P.NXp]) * (0.5 * P.inv_dy);
+          dn[a] = (P.NZp > 1) ? (ua[P.plane] - ua[-P.plane]) * (0.5 * P.inv_dz) : 0.0;
+        }
+        Kin K;
+        kinematics(uc, dt, dx, dy, dn, t, K);
+        double r2s, r2b;
+        second_order_reynolds<EOS>(P, t, uc, K, pi, Pi, ee, r2s, r2b);
+        v[8] = (P.shear && isfinite(r2s)) ? r2s : 0.0;
+        v[9] = (P.bulk && isfinite(r2b)) ? r2b : 0.0;
+      }
+    }
     const double T = eos_temperature<EOS>(P, ee);
     v[0] = T;
     double p0, cs2;
@@ -452,14 +528,14 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     v[6] = (P.shear && isfinite(kp)) ? kp : 0.0;
     v[7] = (P.bulk && isfinite(kP)) ? kP : 0.0;
 #pragma unroll
-    for (int s = 0; s < 8; ++s) m[s] = fmax(m[s], v[s]);
+    for (int s = 0; s < 10; ++s) m[s] = fmax(m[s], v[s]);
     if (maps) {                      // the same quantities cell by cell: maps[s * np + n], physical cells, x fastest
 #pragma unroll
-      for (int s = 0; s < 8; ++s) maps[s * np + n] = v[s];
+      for (int s = 0; s < 10; ++s) maps[s * np + n] = v[s];
     }
   }
 #pragma unroll
-  for (int s = 0; s < 8; ++s) {
+  for (int s = 0; s < 10; ++s) {
     double v = m[s];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));

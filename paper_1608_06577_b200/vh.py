@@ -208,18 +208,18 @@ class Solver:
         return {"tau": tau.value, "n_steps": a.value, "n_inversion_failures": b.value, "n_nonfinite": c.value, "min_reg_factor": mr.value}
 
     DIAG_NAMES = ("max_T", "max_norm_violation", "max_trace_violation", "max_transversality_violation", "max_inv_reynolds_shear",
-                  "max_inv_reynolds_bulk", "max_knudsen_shear", "max_knudsen_bulk")
+                  "max_inv_reynolds_bulk", "max_knudsen_shear", "max_knudsen_bulk", "max_inv_reynolds2_shear", "max_inv_reynolds2_bulk")
 
     def diagnostics(self):
-        out = (C.c_double * 8)()
+        out = (C.c_double * 10)()
         self._check(self.L.vh_get_diagnostics(self.h, out), "vh_get_diagnostics")
         return dict(zip(self.DIAG_NAMES, list(out)))
 
     def diagnostic_maps(self, device=None):
-        """The eight quantities of diagnostics() cell by cell: tensor [8, n_batch, nz, ny, nx] (order of DIAG_NAMES, without 'max_')."""
+        """The ten quantities of diagnostics() cell by cell: tensor [10, n_batch, nz, ny, nx] (order of DIAG_NAMES, without 'max_')."""
         torch = self.torch
         dev = self.device if device is None else torch.device(device)
-        out = torch.empty((8,) + self.shape, dtype=torch.float64, device=dev)
+        out = torch.empty((10,) + self.shape, dtype=torch.float64, device=dev)
         self._check(self.L.vh_get_diagnostic_maps(self.h, _ptr(out), self._space([out])), "vh_get_diagnostic_maps")
         return out
 

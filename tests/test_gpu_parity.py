@@ -410,7 +410,7 @@ def test_full_size_config5_sampled_subboxes(vh, vo):
 
 
 def test_diagnostics_and_freeze_out_termination(vh, vo):
-    # vh_get_diagnostics against the oracle's maxima; vh_run_until stops at the step at which T < T_f everywhere
+    # vh_get_diagnostics (incl. the second-order inverse Reynolds numbers of Eq. 90) against the oracle's maxima; vh_run_until stops at the step at which T < T_f everywhere
     # (program-flow step 8, :494) - the same step the oracle finds by testing after every step
     import torch
     for over in (dict(), dict(eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC)):
@@ -421,17 +421,21 @@ def test_diagnostics_and_freeze_out_termination(vh, vo):
         s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
         o.step(6); s.step(6)
         do, dg = o.diagnostics(), s.diagnostics()
-        for k in do:
-            if k == "max_norm_violation":
-                assert dg[k] < 1e-14 and do[k] < 1e-14
-            else:
-                assert dg[k] == pytest.approx(do[k], rel=1e-9), k
+        assert len(do) == 10 and list(do) == list(dg)
+        assert do["max_inv_reynolds2_shear"] > 0.1 and do["max_inv_reynolds2_bulk"] > 0.1      # Eq. 90: not small here (:834)
         # the same quantities cell by cell (vh_get_diagnostic_maps), to a device and to a host destination
         mo = o.diagnostic_maps()
         # 1/tau_Pi carries (1/3 - c_s^2)^2 (Eq. 18): where the EOS is conformal to within 1e-9 the rounding of c_s^2 is amplified
         # by (1/3)/|1/3 - c_s^2| in the bulk Knudsen number - a per-cell allowance of 16 ulp of c_s^2 times that factor
         bb = np.abs(1.0 / 3.0 - np.vectorize(lambda ee: vo.eos(prm, ee)["cs2"])(o.get_fields()["e"]))
-        slack = {"max_knudsen_bulk": 16 * np.finfo(float).eps / 3.0 / np.maximum(bb, 1e-300) * mo[7]}
+        amp = 16 * np.finfo(float).eps / 3.0 / np.maximum(bb, 1e-300)
+        slack = {"max_knudsen_bulk": amp * mo[7], "max_inv_reynolds2_bulk": amp * mo[9]}      # zeta/tau_Pi carries the same factor
+        for i, k in enumerate(do):
+            if k == "max_norm_violation":
+                assert dg[k] < 1e-14 and do[k] < 1e-14
+            else:
+                worst = slack[k].flat[np.argmax(mo[i])] if k in slack else 0.0
+                assert abs(dg[k] - do[k]) <= 1e-9 * do[k] + worst, k
         for dev in ("cuda:0", "cpu"):
             mg = s.diagnostic_maps(device=dev).cpu().numpy()
             for k, name in enumerate(do):
@@ -449,3 +453,26 @@ def test_diagnostics_and_freeze_out_termination(vh, vo):
         assert s.diagnostics()["max_T"] < T_f and s.status()["n_steps"] == 6 + n_g
         assert s.run_until(T_f, 5, check_every=2) == 0          # already frozen out: no step taken
         s.close()
+
+
+def test_second_order_reynolds_maps_generic_state(vh, vo):
+    # Eq. 90 (:831) on a state with vorticity, u^eta != 0, all pi components and Pi non-zero and u^{n-1} != u^n: every term of
+    # J^{mu nu} and J of Eq. 5 contributes; cell by cell against the oracle, directly on the supplied state and after 4 steps
+    import torch
+    prm = inputs.base_params(nx=36, ny=20, nz=10, dx=0.12, dy=0.1, dz=0.15, tau0=0.8, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=23)
+    up = st["u"] * 1.0
+    up[1:] *= 0.97
+    up[0] = np.sqrt(1 + up[1] ** 2 + up[2] ** 2 + prm["tau0"] ** 2 * up[3] ** 2)
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], st["pi"], st["Pi"]); o.set_uprev(up)
+    s = vh.Solver(prm)
+    t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
+    s.set_initial(t(st["e"]), t(st["u"]), t(st["pi"]), t(st["Pi"])); s.set_uprev(t(up))
+    for n_steps in (0, 4):
+        o.step(n_steps); s.step(n_steps)
+        mo, mg = o.diagnostic_maps(), s.diagnostic_maps().cpu().numpy()
+        assert mo[8].min() > 0 and mo[9].min() > 0
+        for k in (4, 5, 6, 7, 8, 9):
+            assert np.all(np.abs(mg[k] - mo[k]) <= 1e-9 * np.abs(mo[k]) + 1e-12 * mo[k].max()), (n_steps, k)
+    s.close()

@@ -278,3 +278,33 @@ def test_diagnostics_against_their_definitions(vo):
         np.testing.assert_allclose(m[k], r[0], rtol=1e-11, atol=1e-13 * max(np.max(r), 1e-3), err_msg=str(k))
         assert np.max(m[k]) == list(d.values())[k]
     assert d["max_norm_violation"] < 1e-14 and 0 < d["max_trace_violation"] < 0.05      # u.u = 1 after inversion (:489); constraints drift slowly (:333)
+
+
+def test_second_order_reynolds_numbers_in_bjorken_flow(vo):
+    # Eq. 90 (:831) with J, J^{mu nu} of Eq. 5 at n^mu = 0.  Closed form for a uniform fluid at rest in Milne coordinates (Bjorken flow):
+    # theta = 1/tau, sigma^{mu nu} = (2/(3 tau)) d^{mu nu}, pi^{mu nu} = pi d^{mu nu} with d = diag(0, 1/2, 1/2, -1/tau^2); no vorticity;
+    # pi^{lambda<mu} sigma^{nu>}_lambda = (pi/(3 tau)) d^{mu nu}; pi^{mu nu} sigma_{mu nu} = pi/tau.  Hence
+    #   (R_pi^(2))^-1 = |-(delta_pipi + tau_pipi/3) pi + (2/3) lambda_piPi Pi| / ((4/3) eta/tau_pi)     (coefficients in units of tau_pi)
+    #   (R_Pi^(2))^-1 = |-delta_PiPi Pi + (lambda_Pipi/tau_Pi) pi| / (zeta/tau_Pi)
+    tau0, e0, pi0, Pi0 = 0.7, 9.0, 0.31, -0.12
+    prm = inputs.base_params(nx=6, ny=5, nz=4, tau0=tau0, dtau=0.01, eos=1, zeta_model=1)
+    shape = (1, 4, 5, 6)
+    e = np.full(shape, e0)
+    pi = np.zeros((10,) + shape)
+    pi[4], pi[7], pi[9] = 0.5 * pi0, 0.5 * pi0, -pi0 / tau0 ** 2
+    o = vo.Oracle(prm)
+    o.set_initial(e, inputs.rest_velocity(shape), pi, np.full(shape, Pi0))
+    d, m, tc = o.diagnostics(), o.diagnostic_maps(), vo.transport(prm, e0)
+    r2s = abs(-(prm["delta_pipi"] + prm["tau_pipi"] / 3) * pi0 + (2.0 / 3.0) * prm["lambda_piPi"] * Pi0) / ((4.0 / 3.0) * tc["eta_over_tau_pi"])
+    r2b = abs(-prm["delta_PiPi"] * Pi0 + tc["lambda_Pipi_over_tau_Pi"] * pi0) / tc["zeta_over_tau_Pi"]
+    assert tc["zeta_over_tau_Pi"] > 0 and r2s > 0.01 and r2b > 0.01
+    assert d["max_inv_reynolds2_shear"] == pytest.approx(r2s, rel=1e-12)
+    assert d["max_inv_reynolds2_bulk"] == pytest.approx(r2b, rel=1e-12)
+    np.testing.assert_allclose(m[8], r2s, rtol=1e-12)
+    np.testing.assert_allclose(m[9], r2b, rtol=1e-12)
+    assert d["max_knudsen_shear"] == pytest.approx(1.0 / tau0 / tc["inv_tau_pi"], rel=1e-12)
+    # a state without gradients and without tau-expansion (Cartesian geometry is ideal-only, so: sectors off -> zeros)
+    o2 = vo.Oracle(dict(prm, physics=0))
+    o2.set_initial(e, inputs.rest_velocity(shape))
+    d2 = o2.diagnostics()
+    assert d2["max_inv_reynolds2_shear"] == 0.0 and d2["max_inv_reynolds2_bulk"] == 0.0
