@@ -486,9 +486,11 @@ template <class R> class Solver {
         R I2 = theta * pic[m][n];                                                                 // Eq. 44
         R Ipi = I1 + R(P.delta_pipi) * I2 - I3 + R(P.tau_pipi) * I4 - R(P.lambda_piPi) * Pic * sig[m][n];   // Eq. 42
         // Eq. 5 with n^mu = 0: J^{mu nu}/tau_pi = -(Ipi - I1)  (I1 belongs to the projected time derivative, not to J)
-        const R w = g[m] * g[n] * ((m == n) ? R(1) : R(2));
-        JJ += w * (Ipi - I1) * (Ipi - I1);
-        sigsig += w * sig[m][n] * sig[m][n];
+        if (second) {                      // diagnostics only: never part of a time step (nor of its operation count)
+          const R w = g[m] * g[n] * ((m == n) ? R(1) : R(2));
+          JJ += w * (Ipi - I1) * (Ipi - I1);
+          sigsig += w * sig[m][n] * sig[m][n];
+        }
         R Gpi = R(0);                                                                             // :300, R1, R2
         for (int c = 0; c < nG; ++c) {
           if (G3[c].l == m) Gpi += uc[G3[c].a] * G3[c].v * pic[G3[c].b][n];
