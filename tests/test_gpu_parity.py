@@ -476,3 +476,30 @@ def test_second_order_reynolds_maps_generic_state(vh, vo):
         for k in (4, 5, 6, 7, 8, 9):
             assert np.all(np.abs(mg[k] - mo[k]) <= 1e-9 * np.abs(mo[k]) + 1e-12 * mo[k].max()), (n_steps, k)
     s.close()
+
+
+def test_diagnostic_maps_batched_2plus1d(vh, vo):
+    # the per-cell maps in the batched 2+1d mode (extent 1 in eta: no eta differences; events laid out one after the other)
+    import torch
+    prm, init, _ = inputs.config_batched2d(n_batch=3, n=45, n_hot=5, seed=inputs.BASE_SEED + 5, radius=1.8)
+    o = vo.Oracle(prm)
+    o.set_initial(init["e"], init["u"])
+    s = vh.Solver(prm)
+    s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+    o.step(5); s.step(5)
+    mo, mg = o.diagnostic_maps(), s.diagnostic_maps().cpu().numpy()
+    assert mo.shape == mg.shape == (10, 3, 1, 45, 45)
+    bb = np.abs(1.0 / 3.0 - np.vectorize(lambda ee: vo.eos(prm, ee)["cs2"])(o.get_fields()["e"]))
+    amp = 16 * np.finfo(float).eps / 3.0 / np.maximum(bb, 1e-300)      # see test_diagnostics_and_freeze_out_termination
+    for k in range(10):
+        if k == 1:
+            assert mg[k].max() < 1e-14
+            continue
+        slack = amp * mo[k] if k in (7, 9) else 0.0
+        assert mo[k].max() > 0
+        assert np.all(np.abs(mg[k] - mo[k]) <= 1e-9 * mo[k].max() + slack), k
+    for b in range(3):      # events differ, and each event's maps sit in its own block
+        assert np.max(np.abs(mo[4, b] - mo[4, (b + 1) % 3])) > 1e-3
+    d = s.diagnostics()
+    assert list(d.values())[4] == mg[4].max() and list(d.values())[8] == mg[8].max()
+    s.close()
