@@ -8,7 +8,8 @@ fully generic covariant evaluation of the governing relaxation equations, PAPER.
   * flow field analytic and exactly normalised, derivatives analytic (sympy).
 
 The oracle gets the same flow sampled on a tiny grid (central differences, spacing 1e-4; backward time difference 1e-7), so
-the two agree to truncation error ~1e-7.  The vorticity term enters with the sign of Eq. 8 (reading R4)."""
+the two agree to truncation error ~1e-7.  The vorticity term enters with the sign of Eq. 8 (reading R4).
+The same evaluation pins the second-order inverse Reynolds numbers of Eq. 90 (J^{mu nu}, J of Eq. 5 written out with the projector)."""
 import numpy as np
 import pytest
 import sympy as sp
@@ -69,7 +70,13 @@ def generic_rhs(prm, point, coeffs, pi_seed, Pi):
     pisig = np.einsum("mn,ma,nb,ab->", pi, gl, gl, sig)
     DPi = -zotP * theta - Pi * itP - prm["delta_PiPi"] * Pi * theta + lPp * pisig      # Eq. 8 first line / tau_Pi
     J_Pi = DPi / u[0] + Pi * divv
-    return dict(u=u, ufun=ufun, pi=pi, J_pi=J_pi, J_Pi=J_Pi, theta=theta, sig=sig, om=om)
+    # Eq. 90 (:831) with J^{mu nu}, J of Eq. 5 (:116-120) at n^mu = 0, both divided by their relaxation time
+    J2 = 2 * t_om - prm["delta_pipi"] * pi * theta - prm["tau_pipi"] * t_ps + prm["lambda_piPi"] * Pi * sig
+    J0 = -prm["delta_PiPi"] * Pi * theta + lPp * pisig
+    con = lambda T: np.einsum("mn,ma,nb,ab->", T, gl, gl, T)
+    r2_shear = np.sqrt(abs(con(J2))) / (2 * eotp * np.sqrt(abs(con(sig))))
+    r2_bulk = abs(J0) / (zotP * abs(theta))
+    return dict(u=u, ufun=ufun, pi=pi, J_pi=J_pi, J_Pi=J_Pi, theta=theta, sig=sig, om=om, r2_shear=r2_shear, r2_bulk=r2_bulk, t_om=t_om)
 
 
 @pytest.mark.parametrize("pi_seed", [1, 2])
@@ -107,5 +114,10 @@ def test_dissipative_sources_against_generic_covariant_evaluation(vo, pi_seed):
         for n in range(m, 4):
             assert J[slot[m][n]] == pytest.approx(ref["J_pi"][m, n], abs=3e-6 * scale), (m, n)
     assert J[14] == pytest.approx(ref["J_Pi"], rel=3e-6)
+    # second-order inverse Reynolds numbers of Eq. 90 (reading R21) at the same cell, vorticity term included
+    m10 = o.diagnostic_maps()[:, 0, 0, 0, 0]
+    assert m10[8] == pytest.approx(ref["r2_shear"], rel=3e-6) and m10[9] == pytest.approx(ref["r2_bulk"], rel=3e-6)
+    assert m10[6] == pytest.approx(abs(ref["theta"]) / tc["inv_tau_pi"], rel=3e-6)
+    assert np.max(np.abs(ref["t_om"])) > 0.02 * np.max(np.abs(ref["pi"])) and ref["r2_shear"] > 0.05 and ref["r2_bulk"] > 0.05
     # the terms being pinned are all present at a comparable size (a vanishing term would pin nothing)
     assert np.max(np.abs(ref["om"])) > 0.05 and np.max(np.abs(ref["sig"])) > 0.05 and abs(ref["theta"]) > 0.05
