@@ -119,6 +119,15 @@ int vh_get_diagnostics(vh_handle* h, double* out10);
  * through a temporary device buffer of that size).  One kernel; synchronises the stream.                                  */
 int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space);
 
+/* Map of the regularisation strength (the paper's Fig. 17, :820): when enabled, the last stage of every time step also stores, per
+ * cell, the factor tanh(rho)/rho of Eqs. 73-74 it applied to pi^{mu nu} and Pi (one extra 8-byte store per cell and step; one
+ * more padded array of device memory).  Off by default.  vh_enable_regulation_map(h, 1) allocates the array and sets it to 1
+ * (as does every later vh_set_initial); (h, 0) frees it.  vh_get_regulation_map copies it out: map[c] of n_batch*nz*ny*nx
+ * doubles in the layout of vh_get_fields, mem_space 0 host / 1 device; VH_ERR_STATE if the map is not enabled.  In ideal mode
+ * nothing is regularised and the map stays 1.                                                                             */
+int vh_enable_regulation_map(vh_handle* h, int on);
+int vh_get_regulation_map(vh_handle* h, double* map, int mem_space);
+
 /* Program-flow steps 6-8 (:492-494): advance until T < T_f (fm^-1) everywhere or max_steps steps have been taken, testing the
  * temperature every check_every steps (>= 1) with the reduction of vh_get_diagnostics.  *steps_done (may be NULL) receives the
  * number of steps taken by this call; returns VH_OK in both cases (compare vh_get_diagnostics()[0] with T_f to tell them apart). */

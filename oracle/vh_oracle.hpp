@@ -184,6 +184,7 @@ template <class R> class Solver {
     tau = P.tau0;
     for (int n = 0; n < NQ; ++n) { q[n].assign(N, R(0)); qS[n].assign(N, R(0)); Q[n].assign(N, R(0)); }
     for (int m = 0; m < 4; ++m) { u[m].assign(N, R(0)); up[m].assign(N, R(0)); uS[m].assign(N, R(0)); }
+    reg_factor.assign(N, 1.0);
     e.assign(N, R(0)); p.assign(N, R(0));
   }
 
@@ -193,6 +194,7 @@ template <class R> class Solver {
   double tau;
   long long n_steps = 0, n_fail = 0, n_nonfinite = 0;
   double min_reg_factor = 1.0;
+  std::vector<double> reg_factor;         // tanh(rho)/rho that the most recent regularisation applied at each cell (Fig. 17); 1 before the first
   double last_fail[4] = {0, 0, 0, 0};     // E, M2, Pi, guess of the most recent failed inversion (diagnostics)
   std::vector<R> q[NQ], qS[NQ], Q[NQ];   // :470  q, qS, Q
   std::vector<R> u[4], up[4], uS[4];     // :470  u, up, uS
@@ -226,6 +228,7 @@ template <class R> class Solver {
     }
     ghost(q, e, p, u);
     tau = P.tau0; n_steps = 0; n_fail = 0; n_nonfinite = 0; min_reg_factor = 1.0;
+    reg_factor.assign((size_t)NX * NY * NZ, 1.0);
   }
 
   // optional: overwrite u^{n-1} (bit-exact restart)
@@ -303,6 +306,11 @@ template <class R> class Solver {
       cell_diagnostics(idx(i, j, k), v);
       for (int m = 0; m < 10; ++m) out[m] = std::fmax(out[m], v[m]);
     }
+  }
+  // the factor of Eqs. 73-74 that the last regularisation (program-flow step 8 of the last time step) applied, physical cells, x fastest
+  void regulation_map(double* out) const {
+    size_t c = 0;
+    for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i, ++c) out[c] = reg_factor[idx(i, j, k)];
   }
   // the same ten quantities cell by cell (Figs. 15-17 of the paper are such maps): maps[m * np + c], physical cells, x fastest
   void diagnostic_maps(double* maps, size_t np, size_t offset) {
@@ -589,6 +597,7 @@ template <class R> class Solver {
       if (P.physics & 3) {                                              // step 3 (:511), after the inversion (R8)
         R fac = regulate_cell(qq, s, ee, th.p, uu, t);
         if ((double)fac < min_reg_factor) min_reg_factor = (double)fac;
+        reg_factor[s] = (double)fac;
       }
     }
     ghost(qq, e, p, uo);                                                // step 4 (:512)

@@ -65,6 +65,7 @@ def lib():
         L.vho_last_failure.argtypes = [C.c_void_p, C.c_int, dp]
         L.vho_diagnostics.argtypes = [C.c_void_p, dp]
         L.vho_diagnostic_maps.argtypes = [C.c_void_p, dp]
+        L.vho_regulation_map.argtypes = [C.c_void_p, dp]
         L.vho_raw.restype = dp
         L.vho_raw.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.vho_set_tau.argtypes = [C.c_void_p, C.c_double]
@@ -155,6 +156,11 @@ class Oracle:
     def diagnostic_maps(self):
         out = np.empty((10,) + self.shape)
         self.L.vho_diagnostic_maps(self.h, _dp(out))
+        return out
+
+    def regulation_map(self):
+        out = np.empty(self.shape)
+        self.L.vho_regulation_map(self.h, _dp(out))
         return out
 
     def last_failure(self, ev=0):

@@ -109,6 +109,11 @@ void vho_flux_at(vho_handle* h, int ev, int i, int j, int k, int r, int upper, d
   for (int d = 0; d < 5; ++d) { size_t sn = c0 + d * stride[r] - 2 * stride[r]; for (int n = 0; n < 15; ++n) I[n][d] = s->q[n][sn]; eI[d] = s->e[sn]; }
   s->flux(I, eI, upper ? 2 : 1, r, dr[r], tau, false, H15);
 }
+void vho_regulation_map(vho_handle* h, double* out) {
+  const vho::Params& P = h->ev[0]->P;
+  const size_t ne = (size_t)P.nx * P.ny * P.nz;
+  for (size_t b = 0; b < h->ev.size(); ++b) h->ev[b]->regulation_map(out + b * ne);
+}
 void vho_post(vho_handle* h, int ev, double tau) { Sol* s = h->ev[ev]; s->post(s->q, s->u, tau); }
 void vho_ghost(vho_handle* h, int ev) { Sol* s = h->ev[ev]; s->ghost(s->q, s->e, s->p, s->u); }
 

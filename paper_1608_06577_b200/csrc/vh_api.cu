@@ -151,6 +151,13 @@ static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, d
   return debug_sync(h, "ghost kernel");
 }
 
+static cudaError_t reset_regulation_map(vh_handle* h) {
+  if (!h->regfac) return cudaSuccess;
+  fill_kernel<<<1024, 256, 0, h->stream>>>(h->regfac, h->P.fstride, 1.0);
+  h->launches++;
+  return cudaGetLastError();
+}
+
 template <int EOS>
 static void launch_diag(vh_handle* h, double t, double* maps) {
   const DevParams& P = h->P;
@@ -223,6 +230,7 @@ void vh_destroy(vh_handle* h) {
   cudaFree(h->cnt);
   cudaFree(h->eos_tab);
   cudaFree(h->diag);
+  cudaFree(h->regfac);
   cudaFree(h->stage_in);
   cudaFree(h->stage_out);
   delete h;
@@ -284,6 +292,7 @@ int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double
   h->n_steps = 0;
   int rc = reset_counters(h);
   if (rc) return rc;
+  CUDA_TRY(h, reset_regulation_map(h));
   h->initialised = true;
   return VH_OK;
 }
@@ -352,6 +361,7 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   // steps 1-4: q* = E[q^n; e,p,u^n,u^{n-1}] at tau^n, then (e*,p*,u*) at tau^n + dtau, regulate, ghosts
   A.q_in = h->q[0]; A.e_in = h->e[0]; A.p_in = h->p[0]; A.u_in = h->u[0]; A.u_prev = h->u[1]; A.q_n = nullptr;
   A.q_out = h->q[1]; A.e_out = h->e[1]; A.p_out = h->p[1]; A.u_out = h->u[2]; A.cnt = h->cnt; A.t = t; A.t_post = t1;
+  A.regfac = nullptr;      // the map is that of the step's last regularisation (stage 2)
   // variants 0, 2: (velocity kernel, stage kernel) per stage, ghost replicas written by the stage kernel;
   // variant 1: (cell kernel, ghost kernel) per stage.  ev[0..4] bracket the four launches of the step.
   const bool split = (h->variant != 1);
@@ -368,6 +378,7 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   // u^{n+1} overwrites the buffer of u^{n-1}, e^{n+1}/p^{n+1} the buffers of e^n/p^n (neither is read by stage 2).
   A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
   A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1]; A.t = t1; A.t_post = t1;
+  A.regfac = h->regfac;
   if (split) {
     CUDA_TRY(h, launch_stage_any(h, 2, A, ev ? ev[3] : nullptr));
   } else {
@@ -498,6 +509,46 @@ int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
   if (mem_space == 0) cudaFree(dev);
   if (ce != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string("vh_get_diagnostic_maps: ") + cudaGetErrorString(ce));
+  return VH_OK;
+}
+
+int vh_enable_regulation_map(vh_handle* h, int on) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!on) {
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    cudaFree(h->regfac);
+    h->regfac = nullptr;
+    return VH_OK;
+  }
+  if (!h->regfac) {
+    if (cudaMalloc((void**)&h->regfac, (size_t)h->P.fstride * sizeof(double)) != cudaSuccess) {
+      cudaGetLastError();
+      h->regfac = nullptr;
+      return fail(h, VH_ERR_ALLOC, "cudaMalloc(regulation map) failed");
+    }
+    CUDA_TRY(h, reset_regulation_map(h));
+  }
+  return VH_OK;
+}
+
+int vh_get_regulation_map(vh_handle* h, double* map, int mem_space) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if (!map) return fail(h, VH_ERR_ARG, "map is NULL");
+  if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
+  if (!h->regfac) return fail(h, VH_ERR_STATE, "vh_get_regulation_map without vh_enable_regulation_map(h, 1)");
+  const DevParams& P = h->P;
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  double* target = map;
+  if (mem_space == 0) {
+    int rc = ensure_stage(h, &h->stage_out, &h->stage_out_bytes, (size_t)np * sizeof(double));
+    if (rc) return rc;
+    target = h->stage_out;
+  }
+  pack_kernel<true><<<(unsigned)((np + 255) / 256), 256, 0, h->stream>>>(P, h->regfac, target, 1);
+  h->launches++;
+  CUDA_TRY(h, cudaGetLastError());
+  if (mem_space == 0) CUDA_TRY(h, cudaMemcpyAsync(map, h->stage_out, (size_t)np * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   return VH_OK;
 }
 

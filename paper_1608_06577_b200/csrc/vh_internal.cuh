@@ -24,8 +24,9 @@ struct vh_handle {
   double* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
   double* vR = nullptr;              // [3] ... high face
   vh::Counters* cnt = nullptr;
-  unsigned long long* diag = nullptr;   // [6] maxima of vh_get_diagnostics (bit patterns)
+  unsigned long long* diag = nullptr;   // [10] maxima of vh_get_diagnostics (bit patterns)
   double* eos_tab = nullptr;         // EOS 2: the lattice table (vh_eos_lattice.hpp) in global memory
+  double* regfac = nullptr;          // one padded array: tanh(rho)/rho applied by the last step's final regularisation (vh_enable_regulation_map), else null
   double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
   double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
   long long n_steps = 0;

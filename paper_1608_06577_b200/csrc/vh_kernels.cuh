@@ -19,6 +19,7 @@ struct StageArgs {
   Counters* cnt;
   double t;            // tau at which C[q] is evaluated (R7)
   double t_post;       // tau used by the inversion / regularisation of the result
+  double* regfac;      // padded array receiving tanh(rho)/rho of every cell (Fig. 17), or nullptr (the default: nothing is stored)
 };
 
 // ------------------------------------------------------------------------------------------------ flux part, variant 1
@@ -212,6 +213,7 @@ __device__ __forceinline__ void post_cell(const DevParams& P, const StageArgs& A
   if (VISC) {
     double fac = regulation_factor<MILNE>(P, q, e, p0, u, t);
     minfac = fmin(minfac, fac);
+    if (A.regfac && valid) A.regfac[c] = fac;
 #pragma unroll
     for (int n = PTT; n < NQ; ++n) q[n] *= fac;
   }
@@ -541,6 +543,10 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     if ((threadIdx.x & 31) == 0 && v > 0.0) atomicMax(out + s, (unsigned long long)__double_as_longlong(v));
   }
+}
+
+static __global__ void __launch_bounds__(256) fill_kernel(double* __restrict__ a, long long n, double v) {
+  for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < n; w += (long long)gridDim.x * blockDim.x) a[w] = v;
 }
 
 // ------------------------------------------------------------------------------------------------ peak microbenchmarks

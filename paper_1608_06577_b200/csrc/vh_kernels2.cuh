@@ -29,6 +29,7 @@ struct Stage2Args {
   double* q_out; double* e_out; double* p_out; double* u_out;
   Counters* cnt;
   double t, t_post;
+  double* regfac;      // see StageArgs
 };
 
 template <int BX, int BY, int BZ>
@@ -388,6 +389,7 @@ __global__ void __launch_bounds__(BX* BY* BZ, MINB) stage_kernel(const __grid_co
     for (int n = PTT; n < NQ; ++n) qo[n] = park[n][tid];
     fac = regulation_factor<MILNE>(P, qo, e, p0, u, tp);
     minfac = fmin(minfac, fac);
+    if (A.regfac && valid) A.regfac[c] = fac;
   }
 
   if (valid) {

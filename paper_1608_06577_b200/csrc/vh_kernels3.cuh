@@ -49,6 +49,7 @@ struct TileArgs {
   Counters* cnt;
   double t, t_post;
   int a_q, a_u, a_p;      // index of q_in / u_in / p_in in the pool of padded arrays (outermost tensor-map coordinate)
+  double* regfac;         // see StageArgs
 };
 
 // ------------------------------------------------------------------------------------------------ PTX: mbarrier + TMA
@@ -268,7 +269,7 @@ __device__ __forceinline__ double regulation_factor_fast(const DevParams& P, con
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel
-template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE, bool REGMAP = false>
 __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     stage_tile_kernel(const __grid_constant__ DevParams P, const __grid_constant__ TileArgs A, const __grid_constant__ CUtensorMap mapA,
                       const __grid_constant__ CUtensorMap mapZ, const __grid_constant__ CUtensorMap mapC) {
@@ -536,6 +537,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   if (VISC) {
     const double fac = regulation_factor_fast<MILNE>(P, qv, e, p0, u, tp);
     minfac = fmin(minfac, fac);
+    if constexpr (REGMAP) { if (valid) A.regfac[c] = fac; }      // Fig. 17 map (vh_enable_regulation_map): its own instantiation, the default kernel pays nothing
 #pragma unroll
     for (int n = PTT; n < NQ; ++n) qv[n] *= fac;
   }

@@ -37,7 +37,7 @@ static cudaError_t launch_split_t(vh_handle* h, int stage, const StageArgs& S, c
   cudaError_t e = debug_sync(h, "velocity kernel");
   if (e != cudaSuccess) return e;
   if (mid) cudaEventRecord(mid, h->stream);
-  Stage2Args A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post};
+  Stage2Args A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post, S.regfac};
   if (stage == 1) stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1, BX, BY, BZ, VH_STAGE_MINB><<<grid, block, 0, h->stream>>>(P, A);
   else stage_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2, BX, BY, BZ, VH_STAGE_MINB><<<grid, block, 0, h->stream>>>(P, A);
   h->launches++;
@@ -51,11 +51,14 @@ static cudaError_t launch_split_d(vh_handle* h, int stage, const StageArgs& A, c
 }
 
 // ---- tile pipeline (variant 0): velocity kernel + TMA tile kernel (vh_kernels3.cuh)
-template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE>
+template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE, bool REGMAP = false>
 static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
   using T = Tile<TWO_D>;
   constexpr size_t smem = tile_smem_bytes<TWO_D, VISC>();
-  auto kern = stage_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE>;
+  if constexpr (VISC && STAGE == 2 && !REGMAP) {      // the map of Fig. 17 is stored by an instantiation of its own
+    if (A.regfac) return launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE, true>(h, A);
+  }
+  auto kern = stage_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE, REGMAP>;
   static bool configured = false;      // one attribute call per instantiation (single device per process)
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -91,7 +94,7 @@ static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cu
   }
   if (mid) cudaEventRecord(mid, h->stream);
   TileArgs A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post,
-             (int)((S.q_in - h->pool) / fs), (int)((S.u_in - h->pool) / fs), (int)((S.p_in - h->pool) / fs)};
+             (int)((S.q_in - h->pool) / fs), (int)((S.u_in - h->pool) / fs), (int)((S.p_in - h->pool) / fs), S.regfac};
   return (stage == 1) ? launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1>(h, A) : launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2>(h, A);
 }
 template <int EOS, bool VISC, bool MILNE>

@@ -30,7 +30,7 @@ class vh_params(C.Structure):
 
 
 # every symbol include/vh.h declares
-EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_run_until", "vh_eos_table", "vh_launch_count",
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_enable_regulation_map", "vh_get_regulation_map", "vh_run_until", "vh_eos_table", "vh_launch_count",
            "vh_set_kernel_variant", "vh_measure_peaks", "vh_last_error", "vh_destroy"]
 
 _lib = None
@@ -57,6 +57,8 @@ def load_library():
     L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     L.vh_get_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
     L.vh_get_diagnostic_maps.argtypes = [vp, vp, C.c_int]
+    L.vh_enable_regulation_map.argtypes = [vp, C.c_int]
+    L.vh_get_regulation_map.argtypes = [vp, vp, C.c_int]
     L.vh_run_until.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
     L.vh_eos_table.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.vh_launch_count.argtypes = [vp]
@@ -221,6 +223,17 @@ class Solver:
         dev = self.device if device is None else torch.device(device)
         out = torch.empty((10,) + self.shape, dtype=torch.float64, device=dev)
         self._check(self.L.vh_get_diagnostic_maps(self.h, _ptr(out), self._space([out])), "vh_get_diagnostic_maps")
+        return out
+
+    def enable_regulation_map(self, on=True):
+        self._check(self.L.vh_enable_regulation_map(self.h, 1 if on else 0), "vh_enable_regulation_map")
+
+    def regulation_map(self, device=None):
+        """tanh(rho)/rho applied by the last step's final regularisation, per cell (Fig. 17): tensor [n_batch, nz, ny, nx]."""
+        torch = self.torch
+        dev = self.device if device is None else torch.device(device)
+        out = torch.empty(self.shape, dtype=torch.float64, device=dev)
+        self._check(self.L.vh_get_regulation_map(self.h, _ptr(out), self._space([out])), "vh_get_regulation_map")
         return out
 
     def run_until(self, T_f, max_steps, check_every=10):

@@ -503,3 +503,35 @@ def test_diagnostic_maps_batched_2plus1d(vh, vo):
     d = s.diagnostics()
     assert list(d.values())[4] == mg[4].max() and list(d.values())[8] == mg[8].max()
     s.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_regulation_map(vh, vo, variant):
+    # Fig. 17 (:820): the per-cell factor tanh(rho)/rho of the step's last regularisation, stored by the stage kernel when enabled;
+    # a state with large dissipative currents so that the factor spans (0, 1); all three kernel variants; host and device destination
+    import torch
+    prm = inputs.base_params(nx=40, ny=12, nz=6, tau0=0.9, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=11)
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], 6.0 * st["pi"], 6.0 * st["Pi"])
+    s = vh.Solver(prm)
+    s.set_kernel_variant(variant)
+    with pytest.raises(vh.VHError):
+        s.regulation_map()                      # not enabled: VH_ERR_STATE
+    s.enable_regulation_map()
+    t = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
+    s.set_initial(t(st["e"]), t(st["u"]), t(6.0 * st["pi"]), t(6.0 * st["Pi"]))
+    assert torch.all(s.regulation_map() == 1.0)
+    o.step(3); s.step(3)
+    mo = o.regulation_map()
+    assert mo.min() < 0.5 and mo.max() > 0.9
+    for dev in ("cuda:0", "cpu"):
+        mg = s.regulation_map(device=dev).cpu().numpy()
+        assert np.max(np.abs(mg - mo) / mo) <= 1e-9
+    fo, fg = o.get_fields(with_uprev=True), {k: v.cpu().numpy() for k, v in s.get_fields(with_uprev=True).items()}
+    assert_parity(fo, o.status(), fg, s.status())       # storing the map changes nothing else
+    s.set_initial(t(st["e"]), t(st["u"]))
+    assert torch.all(s.regulation_map() == 1.0)         # reset by vh_set_initial
+    s.enable_regulation_map(False)
+    s.step(1)
+    s.close()

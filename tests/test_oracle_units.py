@@ -308,3 +308,23 @@ def test_second_order_reynolds_numbers_in_bjorken_flow(vo):
     o2.set_initial(e, inputs.rest_velocity(shape))
     d2 = o2.diagnostics()
     assert d2["max_inv_reynolds2_shear"] == 0.0 and d2["max_inv_reynolds2_bulk"] == 0.0
+
+
+def test_regulation_map_records_the_applied_factor(vo):
+    # Fig. 17 (:820): the map of tanh(rho)/rho.  The recorded factor must be the one by which the regularisation scaled pi^{mu nu} and
+    # Pi at that cell (Eq. 73): ratio of the exported fields after / before program-flow step 3, cell by cell
+    prm = inputs.base_params(nx=9, ny=7, nz=5, tau0=0.9, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=11)
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], 6.0 * st["pi"], 6.0 * st["Pi"])
+    assert np.all(o.regulation_map() == 1.0)
+    before = o.get_fields()["q"].copy()
+    o.post(0.9)
+    after, m = o.get_fields()["q"], o.regulation_map()
+    assert m.shape == (1, 5, 7, 9) and 0.0 < m.min() < 0.9 and m.max() <= 1.0 and np.ptp(m) > 0.05
+    for n in range(4, 15):
+        np.testing.assert_allclose(after[n], m * before[n], rtol=1e-14, atol=0)
+    np.testing.assert_allclose(after[:4], before[:4], rtol=0, atol=0)
+    # after a full step the map is that of the step's last regularisation: never below the run's minimum
+    o.step(2)
+    assert o.regulation_map().min() >= o.status()["min_reg_factor"]
