@@ -116,7 +116,7 @@ int vh_get_diagnostics(vh_handle* h, double* out10);
 /* The same ten quantities cell by cell (the maps of the paper's Figs. 15-16, :826-834, are slices of [4]..[9]):
  * maps10[m * np + c], m = 0..9 as in vh_get_diagnostics, np = n_batch*nz*ny*nx, c = ((b*nz + k)*ny + j)*nx + i (physical cells,
  * the layout of vh_get_fields).  maps10 holds 10*np doubles in mem_space (0 host, 1 device; a host destination goes
- * through a temporary device buffer of that size).  One kernel; synchronises the stream.                                  */
+ * through the library's device staging buffer, grown to that size).  One kernel; synchronises the stream.            */
 int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space);
 
 /* Map of the regularisation strength (the paper's Fig. 17, :820): when enabled, the last stage of every time step also stores, per

@@ -19,7 +19,7 @@
 //     (Eqs. 73-74, reading R9) is pinned only through hand-computed values of rho for simple states
 //     (tests/test_oracle_units.py): "parity unpinned" beyond that - no printed solution exercises rho >~ 1; applied literally it makes
 //     the discrete Gubser run ill-conditioned ("config 2").  The lattice EOS (eos = 2, vh_oracle_lattice.hpp,
-//     readings R19, R20) is pinned by tests/test_oracle_lattice.py, zeta/s of Eq. 17 and diagnostics() (incl. Eq. 90, reading R21) by tests/test_oracle_units.py.
+//     readings R19, R20) is pinned by tests/test_oracle_lattice.py, zeta/s of Eq. 17, diagnostics() (incl. Eq. 90, reading R21, also tests/test_oracle_covariant.py) and regulation_map() by tests/test_oracle_units.py.
 //
 // The scalar type is a template parameter so that an operation-counting type can be
 // substituted (oracle/vh_oracle_capi.cpp instantiates double and a counting type).

@@ -496,19 +496,17 @@ int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
   if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
   const size_t bytes = (size_t)10 * h->P.nx * h->P.ny * h->P.nz * h->P.n_batch * sizeof(double);
   double* dev = maps10;
-  if (mem_space == 0) {
-    if (cudaMalloc(&dev, bytes) != cudaSuccess) { cudaGetLastError(); return fail(h, VH_ERR_ALLOC, "device allocation for the maps failed"); }
+  if (mem_space == 0) {      // host destination: through the staging buffer of vh_get_fields
+    int rc = ensure_stage(h, &h->stage_out, &h->stage_out_bytes, bytes);
+    if (rc) return rc;
+    dev = h->stage_out;
   }
-  cudaError_t ce = cudaMemsetAsync(h->diag, 0, 10 * sizeof(unsigned long long), h->stream);
+  CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 10 * sizeof(unsigned long long), h->stream));
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
-  if (ce == cudaSuccess) {
-    if (h->prm.eos == 2) launch_diag<2>(h, t, dev); else if (h->prm.eos == 1) launch_diag<1>(h, t, dev); else launch_diag<0>(h, t, dev);
-    ce = cudaGetLastError();
-  }
-  if (ce == cudaSuccess && mem_space == 0) ce = cudaMemcpyAsync(maps10, dev, bytes, cudaMemcpyDeviceToHost, h->stream);
-  if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);
-  if (mem_space == 0) cudaFree(dev);
-  if (ce != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string("vh_get_diagnostic_maps: ") + cudaGetErrorString(ce));
+  if (h->prm.eos == 2) launch_diag<2>(h, t, dev); else if (h->prm.eos == 1) launch_diag<1>(h, t, dev); else launch_diag<0>(h, t, dev);
+  CUDA_TRY(h, cudaGetLastError());
+  if (mem_space == 0) CUDA_TRY(h, cudaMemcpyAsync(maps10, dev, bytes, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   return VH_OK;
 }
 
