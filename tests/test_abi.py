@@ -119,3 +119,13 @@ def test_lattice_eos_table_of_the_product_matches_the_oracle(vo):
         assert r["T"] == pytest.approx(nodes[k, 2], rel=1e-10)
         assert r["cs2"] == pytest.approx(nodes[k, 1] / h / (4 * xk**3), rel=1e-8)
     assert nodes[0, 2] * inputs.HBARC == pytest.approx(0.03, rel=1e-12) and nodes[-1, 2] * inputs.HBARC == pytest.approx(2.0, rel=1e-12)
+
+
+def test_diagnostic_names_agree_with_the_header_and_the_oracle(vo):
+    # the binding, the header and the test oracle describe the same ten diagnostics in the same order
+    from paper_1608_06577_b200 import vh
+
+    src = open(os.path.join(ROOT, "include", "vh.h")).read()
+    n = int(re.search(r"#define\s+VH_N_DIAGNOSTICS\s+(\d+)", src).group(1))
+    assert n == len(vh.Solver.DIAG_NAMES) == len(vo.DIAG_NAMES) == 10
+    assert tuple(vh.Solver.DIAG_NAMES) == tuple(vo.DIAG_NAMES)
