@@ -63,8 +63,9 @@ typedef struct {
 } vh_params;
 
 /* Create a solver for the grid / physics in *p on the current CUDA device.  cuda_stream: a cudaStream_t (may be NULL =
- * default stream).  Allocates 61 padded SoA arrays (3 x 15 q, 3 x 4 u, 2 x e, 2 x p; :470-476 plus the ping-pong copy of
- * e, p needed because inversion is fused into the stage kernel).  *out is set only on success.                         */
+ * default stream).  Allocates 67 padded SoA arrays (3 x 15 q, 3 x 4 u, 2 x e, 2 x p; :470-476 plus the ping-pong copy of
+ * e, p needed because inversion is fused into the stage kernel; and the 6 state-velocity arrays the velocity kernel hands
+ * to the stage kernel).  The handle belongs to that device: every later call switches to it.  *out is set only on success. */
 int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out);
 
 /* Program-flow steps 3-5 (:489-491): build q^0 from (e, u^mu, pi^{mu nu}, Pi) by Eqs. 32-33 (:267-269), p = P0(e),

@@ -370,8 +370,10 @@ template <class R> class Solver {
     R th = R(P.minmod_theta);
     for (int n = 0; n < NQ; ++n) {
       // Eq. 67 slopes of cell c and of cell c+1
+      VHO_COUNTING_SECTION(3);
       R sc = minmod3(th * (I[n][c] - I[n][c - 1]) / dr, (I[n][c + 1] - I[n][c - 1]) / (R(2) * dr), th * (I[n][c + 1] - I[n][c]) / dr);
       R sn = minmod3(th * (I[n][c + 1] - I[n][c]) / dr, (I[n][c + 2] - I[n][c]) / (R(2) * dr), th * (I[n][c + 2] - I[n][c + 1]) / dr);
+      VHO_COUNTING_SECTION(1);
       qm[n] = I[n][c] + (dr / R(2)) * sc;         // q^-: Eq. 64 / 66
       qp[n] = I[n][c + 1] - (dr / R(2)) * sn;     // q^+: Eq. 63 / 65
     }

@@ -223,34 +223,40 @@ def invert(params: dict, E, M2, Pi, guess):
 DIAG_NAMES = ("max_T", "max_norm_violation", "max_trace_violation", "max_transversality_violation", "max_inv_reynolds_shear", "max_inv_reynolds_bulk",
               "max_knudsen_shear", "max_knudsen_bulk", "max_inv_reynolds2_shear", "max_inv_reynolds2_bulk")
 OP_CLASSES = ("add", "mul", "div", "cmp", "sqrt", "exp", "pow", "tanh")
-# flop weights of SURVEY.md 8(d): add/mul/compare 1, div 10, sqrt 15, exp 25, tanh 40; pow(x, 1/4) = two sqrt
-OP_WEIGHTS = dict(add=1, mul=1, div=10, cmp=1, sqrt=15, exp=25, pow=30, tanh=40)
+# flop weights of SURVEY.md 8(d): add/mul 1, div 10, sqrt 15, exp 25, tanh 40; pow(x, 1/4) = two sqrt.  Compares carry NO flop weight
+# (a select is not floating-point work; they are reported as their own class).
+OP_WEIGHTS = dict(add=1, mul=1, div=10, cmp=0, sqrt=15, exp=25, pow=30, tanh=40)
+SECTIONS = ("other", "flux", "invert", "slopes")
+# how often the oracle evaluates the same thing: each interface from both adjacent cells (Alg. 2), each limited slope four times
+# (as the slope of "this" cell and of "the next" cell, for the upper and the lower interface)
+REPEATS = dict(other=1, flux=2, invert=2, slopes=4)
 
 
 def count_ops(params: dict, e, u4, pi10=None, Pi=None, warm=1, n=1):
-    """Operation counts of n RK2 steps with the counting scalar (after `warm` uncounted steps).
-    Returns dict(other=..., flux=..., invert=...) of {class: count} summed over all cells: `flux` is the reconstruction and
-    Eq. 61 inside flux(), `invert` the interface-state inversions inside flux() (both evaluated twice per interface)."""
+    """Operation counts of n RK2 steps with the counting scalar (after `warm` uncounted steps), summed over all cells, per section
+    of the oracle: `slopes` = Eq. 67 inside flux(), `flux` = half-cell extrapolation and Eq. 61, `invert` = the interface-state
+    inversions inside flux(), `other` = sources, stage update, cell inversion, regularisation."""
     P = make_params(params)
     shape = (P.n_batch, P.nz, P.ny, P.nx)
     e = np.ascontiguousarray(e, dtype=np.float64).reshape(shape)
     u4 = np.ascontiguousarray(u4, dtype=np.float64).reshape((4,) + shape)
     pi10 = None if pi10 is None else np.ascontiguousarray(pi10, dtype=np.float64).reshape((10,) + shape)
     Pi = None if Pi is None else np.ascontiguousarray(Pi, dtype=np.float64).reshape(shape)
-    out = (C.c_longlong * 24)()
+    out = (C.c_longlong * 32)()
     rc = lib().vho_count_ops(C.byref(P), _dp(e), _dp(u4), _dp(pi10), _dp(Pi), int(warm), int(n), out)
     if rc < 0:
         raise ValueError("vho_count_ops needs n_batch == 1")
     vals = list(out)
-    return dict(other=dict(zip(OP_CLASSES, vals[:8])), flux=dict(zip(OP_CLASSES, vals[8:16])), invert=dict(zip(OP_CLASSES, vals[16:24])))
+    return {sec: dict(zip(OP_CLASSES, vals[8 * i:8 * i + 8])) for i, sec in enumerate(SECTIONS)}
 
 
 def algorithmic_flops_per_cell_update(params: dict, e, u4, pi10=None, Pi=None):
-    """Weighted flops per cell per RK2 step with every interface charged once (flux section / 2), and the raw counts."""
+    """MINIMAL algorithmic flops per cell per RK2 step: every section divided by the number of times the oracle repeats it
+    (REPEATS), compares excluded, exact 0 / +-1 constants not counted.  Returns (flops, per-class counts incl. 'cmp',
+    flops per section)."""
     c = count_ops(params, e, u4, pi10, Pi, warm=1, n=1)
     ncell = params["nx"] * params["ny"] * params["nz"]
-    per = {k: (c["other"][k] + 0.5 * c["flux"][k] + 0.5 * c["invert"][k]) / ncell for k in OP_CLASSES}
-    flops = sum(OP_WEIGHTS[k] * per[k] for k in OP_CLASSES)
-    plain = per["add"] + per["mul"] + per["div"] + per["sqrt"] + per["cmp"]
-    per["flops_interface_inversions"] = sum(OP_WEIGHTS[k] * 0.5 * c["invert"][k] / ncell for k in OP_CLASSES)
-    return flops, plain, per
+    per = {k: sum(c[sec][k] / REPEATS[sec] for sec in SECTIONS) / ncell for k in OP_CLASSES}
+    by_section = {sec: sum(OP_WEIGHTS[k] * c[sec][k] for k in OP_CLASSES) / REPEATS[sec] / ncell for sec in SECTIONS}
+    flops = sum(by_section.values())
+    return flops, per, by_section

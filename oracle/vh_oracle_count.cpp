@@ -1,15 +1,17 @@
 // TEST INFRASTRUCTURE ONLY (see vh_oracle.hpp).  Instantiates the oracle with an operation-counting scalar to measure
 // the ALGORITHMIC floating-point work of one KT/RK2 step ("replace the estimate by a measured count").
-// Operations whose operands are all compile-time / per-run constants are not counted (a compiler hoists them).
-// Interface fluxes are counted separately so that each interface can be charged once (the oracle, like PAPER.md Alg. 2,
-// evaluates every interface from both adjacent cells).
+// Operations whose operands are all compile-time / per-run constants are not counted (a compiler hoists them), and neither is
+// an addition of an exact constant 0 or a multiplication / division by an exact constant 0 or +-1 (the index-form loops of the
+// oracle multiply by Kronecker deltas and metric signs; that is notation, not work the method needs).  Compares are their own
+// class and carry no flop weight.  Work the oracle repeats is counted in sections of its own so that it can be charged once:
+// every interface is evaluated from both adjacent cells (Alg. 2), and every limited slope (Eq. 67) four times.
 #include <cmath>
 #include <cstring>
 
 namespace vho_cnt {
 enum { ADD = 0, MUL, DIV, CMP, SQRT, EXP, POW, TANH, NCLASS };
-static long long g_counts[3][NCLASS];
-static int g_section = 0;     // 0: everything else, 1: inside flux() (reconstruction + Eq. 61), 2: the interface-state inversions inside flux()
+static long long g_counts[4][NCLASS];
+static int g_section = 0;     // 0: everything else, 1: inside flux(): half-cell extrapolation + Eq. 61, 2: the interface-state inversions inside flux(), 3: the limited slopes inside flux()
 static bool g_on = false;
 inline void tick(int cls, bool live) { if (g_on && live) ++g_counts[g_section][cls]; }
 
@@ -22,10 +24,22 @@ struct Cnt {
   Cnt(double x, bool kk) : v(x), k(kk) {}
   explicit operator double() const { return v; }
 };
-inline Cnt operator+(Cnt a, Cnt b) { bool k = a.k && b.k; tick(ADD, !k); return Cnt(a.v + b.v, k); }
-inline Cnt operator-(Cnt a, Cnt b) { bool k = a.k && b.k; tick(ADD, !k); return Cnt(a.v - b.v, k); }
-inline Cnt operator*(Cnt a, Cnt b) { bool k = a.k && b.k; tick(MUL, !k); return Cnt(a.v * b.v, k); }
-inline Cnt operator/(Cnt a, Cnt b) { bool k = a.k && b.k; tick(b.k ? MUL : DIV, !k); return Cnt(a.v / b.v, k); }   // x / const = x * (1/const)
+inline bool zero(Cnt a) { return a.k && a.v == 0.0; }
+inline bool unit(Cnt a) { return a.k && (a.v == 1.0 || a.v == -1.0); }
+inline Cnt operator+(Cnt a, Cnt b) { bool k = a.k && b.k; tick(ADD, !k && !zero(a) && !zero(b)); return Cnt(a.v + b.v, k); }
+inline Cnt operator-(Cnt a, Cnt b) { bool k = a.k && b.k; tick(ADD, !k && !zero(a) && !zero(b)); return Cnt(a.v - b.v, k); }
+inline Cnt operator*(Cnt a, Cnt b) {
+  bool k = a.k && b.k;
+  if (!k && (zero(a) || zero(b))) return Cnt(a.v * b.v, true);      // x * 0 is the constant 0: nothing downstream of it is work either
+  tick(MUL, !k && !unit(a) && !unit(b));
+  return Cnt(a.v * b.v, k);
+}
+inline Cnt operator/(Cnt a, Cnt b) {      // x / const = x * (1/const)
+  bool k = a.k && b.k;
+  if (!k && zero(a)) return Cnt(a.v / b.v, true);
+  tick(b.k ? MUL : DIV, !k && !unit(b));
+  return Cnt(a.v / b.v, k);
+}
 inline Cnt operator-(Cnt a) { return Cnt(-a.v, a.k); }
 inline Cnt& operator+=(Cnt& a, Cnt b) { a = a + b; return a; }
 inline Cnt& operator-=(Cnt& a, Cnt b) { a = a - b; return a; }
@@ -46,7 +60,7 @@ namespace vho { using vho_cnt::sqrt; using vho_cnt::exp; using vho_cnt::tanh; us
 
 extern "C" {
 // Runs `warm` uncounted steps (so that no array holds constant-flagged data), then counts `n` steps.
-// counts: [3][8] = {other, flux, interface inversions} x {add, mul, div, cmp, sqrt, exp, pow, tanh}; totals over all cells and steps.
+// counts: [4][8] = {other, flux, interface inversions, slopes} x {add, mul, div, cmp, sqrt, exp, pow, tanh}; totals over all cells and steps.
 int vho_count_ops(const vho::Params* P, const double* e, const double* u4, const double* pi10, const double* Pi, int warm, int n,
                   long long* counts) {
   if (P->n_batch != 1) return -1;

@@ -26,6 +26,20 @@ static int fail(vh_handle* h, int code, const std::string& msg) {
     if (_e != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e)); \
   } while (0)
 
+// every entry point that touches the device runs on the handle's device, whatever the caller's current device is
+static int enter(vh_handle* h) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) {
+    cudaError_t e = cudaSetDevice(h->device);
+    if (e != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+  }
+  return VH_OK;
+}
+#define VH_ENTER(h)                         \
+  do {                                      \
+    if (int _rc = enter(h)) return _rc;     \
+  } while (0)
+
 static long long round_up(long long a, long long m) { return (a + m - 1) / m * m; }
 
 static int fill_dev_params(const vh_params& p, DevParams& P) {
@@ -54,7 +68,6 @@ static int fill_dev_params(const vh_params& p, DevParams& P) {
   P.theta = p.minmod_theta;
   P.inv_rho_max = 1.0 / p.rho_max; P.xi0_rho_max = p.xi0 * p.rho_max;
   P.newton_max_iter = p.newton_max_iter; P.newton_rtol = p.newton_rtol;
-  P.debug = getenv("VH_DEBUG_FLAGS") ? atoi(getenv("VH_DEBUG_FLAGS")) : 0;
   P.relax_clamp = (p.tau_relax_floor_over_dtau > 0.0) ? 1.0 / (p.tau_relax_floor_over_dtau * p.dtau) : std::numeric_limits<double>::infinity();
   return 0;
 }
@@ -168,6 +181,16 @@ static void launch_diag(vh_handle* h, double t, double* maps) {
   h->launches++;
 }
 
+static int reset_counters(vh_handle* h) {
+  Counters c;
+  c.n_fail = 0; c.n_nonfinite = 0;
+  double one = 1.0;
+  std::memcpy(&c.min_reg_bits, &one, sizeof(double));
+  CUDA_TRY(h, cudaMemcpyAsync(h->cnt, &c, sizeof(c), cudaMemcpyHostToDevice, h->stream));
+  CUDA_TRY(h, cudaStreamSynchronize(h->stream));    // c lives on this stack frame
+  return VH_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ C ABI
 extern "C" {
 
@@ -184,12 +207,13 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   fill_dev_params(*p, h->P);
   h->two_d = (p->nz == 1);
   h->stream = (cudaStream_t)cuda_stream;
+  cudaGetDevice(&h->device);
   const long long fs = h->P.fstride;
   const size_t bytes = (size_t)67 * fs * sizeof(double);
   ce = cudaMalloc((void**)&h->pool, bytes);
-  if (ce != cudaSuccess) { delete h; return fail(nullptr, VH_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes: " + cudaGetErrorString(ce)); }
+  if (ce != cudaSuccess) { cudaGetLastError(); delete h; return fail(nullptr, VH_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes: " + cudaGetErrorString(ce)); }
   ce = cudaMalloc((void**)&h->cnt, sizeof(Counters));
-  if (ce != cudaSuccess) { cudaFree(h->pool); delete h; return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc(counters) failed"); }
+  if (ce != cudaSuccess) { cudaGetLastError(); cudaFree(h->pool); delete h; return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc(counters) failed"); }
   double* w = h->pool;
   for (int i = 0; i < 3; ++i) { h->q[i] = w; w += 15 * fs; }
   for (int i = 0; i < 3; ++i) { h->u[i] = w; w += 4 * fs; }
@@ -210,7 +234,7 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
     ce = cudaMalloc((void**)&h->eos_tab, tb);
     if (ce == cudaSuccess) ce = cudaMemcpyAsync(h->eos_tab, tab.node.data(), tb, cudaMemcpyHostToDevice, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);      // tab lives on this stack frame
-    if (ce != cudaSuccess) { cudaFree(h->eos_tab); cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_ALLOC, "EOS table upload failed"); }
+    if (ce != cudaSuccess) { cudaGetLastError(); cudaFree(h->eos_tab); cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_ALLOC, "EOS table upload failed"); }
     const int n = vh_eos::VH_EOS_N;
     const double* nd = tab.node.data();
     const double e0 = std::pow(tab.x0, 4), eN = std::pow(tab.xN, 4);
@@ -219,12 +243,18 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
     h->P.eos_lo_slope = nd[0] / e0; h->P.eos_pN = nd[4 * n]; h->P.eos_eN = eN;
     h->P.eos_T0_over_x0 = nd[2] / tab.x0; h->P.eos_TN_over_xN = nd[4 * n + 2] / tab.xN;
   }
+  if (reset_counters(h) != VH_OK) {      // vh_get_status before vh_set_initial reads zeros, not uninitialised memory
+    std::string msg = h->err;
+    cudaFree(h->eos_tab); cudaFree(h->pool); cudaFree(h->cnt); delete h;
+    return fail(nullptr, VH_ERR_CUDA, msg);
+  }
   *out = h;
   return VH_OK;
 }
 
 void vh_destroy(vh_handle* h) {
   if (!h) return;
+  enter(h);
   cudaStreamSynchronize(h->stream);
   cudaFree(h->pool);
   cudaFree(h->cnt);
@@ -250,23 +280,14 @@ static int ensure_stage(vh_handle* h, double** buf, size_t* have, size_t need) {
   if (*have >= need) return VH_OK;
   cudaFree(*buf);
   *buf = nullptr; *have = 0;
-  if (cudaMalloc((void**)buf, need) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(staging) failed");
+  if (cudaMalloc((void**)buf, need) != cudaSuccess) { cudaGetLastError(); *buf = nullptr; return fail(h, VH_ERR_ALLOC, "cudaMalloc(staging) failed"); }
   *have = need;
-  return VH_OK;
-}
-
-static int reset_counters(vh_handle* h) {
-  Counters c;
-  c.n_fail = 0; c.n_nonfinite = 0;
-  double one = 1.0;
-  std::memcpy(&c.min_reg_bits, &one, sizeof(double));
-  CUDA_TRY(h, cudaMemcpyAsync(h->cnt, &c, sizeof(c), cudaMemcpyHostToDevice, h->stream));
-  CUDA_TRY(h, cudaStreamSynchronize(h->stream));    // c lives on this stack frame
   return VH_OK;
 }
 
 int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double* pi10, const double* Pi, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!e || !u4) return fail(h, VH_ERR_ARG, "e and u4 are required");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   const DevParams& P = h->P;
@@ -300,6 +321,7 @@ int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double
 int vh_set_state(vh_handle* h, const double* q15, const double* e, const double* u4, const double* u4_prev, long long n_steps_done,
                  int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!q15 || !e || !u4 || !u4_prev || n_steps_done < 0) return fail(h, VH_ERR_ARG, "q15, e, u4, u4_prev are required; n_steps_done >= 0");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   const DevParams& P = h->P;
@@ -330,12 +352,14 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
   h->n_steps = n_steps_done;
   int rc = reset_counters(h);
   if (rc) return rc;
+  CUDA_TRY(h, reset_regulation_map(h));
   h->initialised = true;
   return VH_OK;
 }
 
 int vh_set_uprev(vh_handle* h, const double* u4_prev, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_set_uprev before vh_set_initial");
   if (!u4_prev || (mem_space != 0 && mem_space != 1)) return fail(h, VH_ERR_ARG, "bad argument");
   const DevParams& P = h->P;
@@ -396,6 +420,7 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
 
 int vh_step(vh_handle* h, int n_steps) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_step before vh_set_initial");
   if (n_steps < 0) return fail(h, VH_ERR_ARG, "n_steps must be >= 0");
   for (int it = 0; it < n_steps; ++it) {
@@ -407,9 +432,11 @@ int vh_step(vh_handle* h, int n_steps) {
 
 int vh_step_profile(vh_handle* h, int n_steps, double* ms4) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_step_profile before vh_set_initial");
   if (n_steps < 1 || !ms4) return fail(h, VH_ERR_ARG, "n_steps >= 1 and ms4 != NULL required");
-  cudaEvent_t ev[5];
+  cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  struct Guard { cudaEvent_t* e; ~Guard() { for (int i = 0; i < 5; ++i) if (e[i]) cudaEventDestroy(e[i]); } } guard{ev};      // also on every early return
   for (int i = 0; i < 5; ++i) CUDA_TRY(h, cudaEventCreate(&ev[i]));
   double acc[4] = {0, 0, 0, 0};
   for (int it = 0; it < n_steps; ++it) {
@@ -418,13 +445,13 @@ int vh_step_profile(vh_handle* h, int n_steps, double* ms4) {
     CUDA_TRY(h, cudaEventSynchronize(ev[4]));
     for (int i = 0; i < 4; ++i) { float ms = 0; CUDA_TRY(h, cudaEventElapsedTime(&ms, ev[i], ev[i + 1])); acc[i] += ms; }
   }
-  for (int i = 0; i < 5; ++i) cudaEventDestroy(ev[i]);
   for (int i = 0; i < 4; ++i) ms4[i] = acc[i] / n_steps;
   return VH_OK;
 }
 
 int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, double* u4_prev, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_fields before vh_set_initial");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   const DevParams& P = h->P;
@@ -451,6 +478,7 @@ int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, d
 int vh_get_status(vh_handle* h, double* tau, long long* n_steps_done, long long* n_inversion_failures, long long* n_nonfinite,
                   double* min_reg_factor) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   Counters c;
   CUDA_TRY(h, cudaMemcpyAsync(&c, h->cnt, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(h, cudaStreamSynchronize(h->stream));
@@ -474,9 +502,10 @@ int vh_eos_table(double* nodes4, double* x0, double* h) {
 
 int vh_get_diagnostics(vh_handle* h, double* out10) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostics before vh_set_initial");
   if (!out10) return fail(h, VH_ERR_ARG, "out10 is NULL");
-  if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
+  if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); h->diag = nullptr; return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed"); }
   CUDA_TRY(h, cudaMemsetAsync(h->diag, 0, 10 * sizeof(unsigned long long), h->stream));
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
   if (h->prm.eos == 2) launch_diag<2>(h, t, nullptr); else if (h->prm.eos == 1) launch_diag<1>(h, t, nullptr); else launch_diag<0>(h, t, nullptr);
@@ -490,10 +519,11 @@ int vh_get_diagnostics(vh_handle* h, double* out10) {
 
 int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!maps10) return fail(h, VH_ERR_ARG, "maps10 is NULL");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostic_maps before vh_set_initial");
-  if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed");
+  if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); h->diag = nullptr; return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed"); }
   const size_t bytes = (size_t)10 * h->P.nx * h->P.ny * h->P.nz * h->P.n_batch * sizeof(double);
   double* dev = maps10;
   if (mem_space == 0) {      // host destination: through the staging buffer of vh_get_fields
@@ -512,6 +542,7 @@ int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
 
 int vh_enable_regulation_map(vh_handle* h, int on) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!on) {
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     cudaFree(h->regfac);
@@ -531,6 +562,7 @@ int vh_enable_regulation_map(vh_handle* h, int on) {
 
 int vh_get_regulation_map(vh_handle* h, double* map, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!map) return fail(h, VH_ERR_ARG, "map is NULL");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   if (!h->regfac) return fail(h, VH_ERR_STATE, "vh_get_regulation_map without vh_enable_regulation_map(h, 1)");
@@ -552,6 +584,7 @@ int vh_get_regulation_map(vh_handle* h, double* map, int mem_space) {
 
 int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long long* steps_done) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_run_until before vh_set_initial");
   if (max_steps < 0 || check_every < 1 || !(T_f >= 0.0)) return fail(h, VH_ERR_ARG, "max_steps >= 0, check_every >= 1, T_f >= 0 required");
   long long done = 0;

@@ -34,7 +34,6 @@ struct DevParams {
   double inv_rho_max, xi0_rho_max;
   int newton_max_iter; double newton_rtol;
   double relax_clamp;           // 1/(c*dtau) or +inf
-  int debug;                    // VH_DEBUG_FLAGS (development only)
 };
 
 // ---------------------------------------------------------------- branch-free reciprocal / square roots on the MUFU seeds
@@ -183,7 +182,7 @@ template <int EOS> __device__ __forceinline__ double invert_energy(const DevPara
     }
   }
   fail = bad || !conv || !(e > 0.0) || !isfinite(e);
-  if (fail) e = fmax(E, 1e-300);
+  if (fail) e = (1e-300 > E) ? 1e-300 : E;      // max(E, tiny) that keeps a NaN E visible to n_nonfinite
   return e;
 }
 

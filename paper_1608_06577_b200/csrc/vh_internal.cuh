@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <string>
+#include <vector>
 
 #ifndef VH_STAGE_MINB
 #define VH_STAGE_MINB 2      // resident blocks per SM the stage kernel is compiled for (register cap 65536/(256*MINB))
@@ -16,6 +17,8 @@ struct vh_handle {
   vh_params prm;
   vh::DevParams P;
   cudaStream_t stream = nullptr;
+  int device = 0;                    // the device the handle was created on (its buffers, tensor maps and kernel attributes belong to it)
+  std::vector<const void*> smem_opted_in;   // kernels whose dynamic shared-memory limit was raised on `device` for this handle
   double* pool = nullptr;            // 67 padded arrays
   double* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
   double* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
@@ -48,6 +51,15 @@ inline cudaError_t vh_debug_sync(vh_handle* h, const char* what) {
     e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) fprintf(stderr, "[vh] %s faulted at step %lld: %s\n", what, h->n_steps, cudaGetErrorString(e));
   }
+  return e;
+}
+
+// Raise a kernel's dynamic shared-memory limit once per handle.  The attribute is per device, and a handle belongs to one device, so
+// nothing process-wide is cached.
+inline cudaError_t vh_opt_in_smem(vh_handle* h, const void* kern, size_t smem) {
+  for (const void* k : h->smem_opted_in) if (k == kern) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) h->smem_opted_in.push_back(kern);
   return e;
 }
 

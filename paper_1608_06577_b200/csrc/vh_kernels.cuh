@@ -272,10 +272,10 @@ __global__ void __launch_bounds__(256) stage_cell_kernel(const __grid_constant__
 #pragma unroll
   for (int n = 0; n < 4; ++n) uc[n] = A.u_in[n * fs + c];
 
-  if (!(P.debug & 8)) flux_dir_cell<EOS, VISC, MILNE>(P, A.q_in, A.e_in, c, 1, 0, P.inv_dx, t2, P.nx > 1, P.nx > 1 && i == 0, C, nfail);
-  if (!(P.debug & 16)) flux_dir_cell<EOS, VISC, MILNE>(P, A.q_in, A.e_in, c, P.NXp, 1, P.inv_dy, t2, P.ny > 1, P.ny > 1 && j == 0, C, nfail);
-  if (!TWO_D && !(P.debug & 32)) flux_dir_cell<EOS, VISC, MILNE>(P, A.q_in, A.e_in, c, P.plane, 2, P.inv_dz, t2, P.nz > 1, P.nz > 1 && k == 0, C, nfail);
-  if (!(P.debug & 4)) sources_cell<EOS, VISC, MILNE, TWO_D>(P, A, c, t, qc, ec, pc, uc, C);
+  flux_dir_cell<EOS, VISC, MILNE>(P, A.q_in, A.e_in, c, 1, 0, P.inv_dx, t2, P.nx > 1, P.nx > 1 && i == 0, C, nfail);
+  flux_dir_cell<EOS, VISC, MILNE>(P, A.q_in, A.e_in, c, P.NXp, 1, P.inv_dy, t2, P.ny > 1, P.ny > 1 && j == 0, C, nfail);
+  if (!TWO_D) flux_dir_cell<EOS, VISC, MILNE>(P, A.q_in, A.e_in, c, P.plane, 2, P.inv_dz, t2, P.nz > 1, P.nz > 1 && k == 0, C, nfail);
+  sources_cell<EOS, VISC, MILNE, TWO_D>(P, A, c, t, qc, ec, pc, uc, C);
 
   double qo[NQ];
 #pragma unroll
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(256) stage_cell_kernel(const __grid_constant__
     qo[n] = v;
   }
   post_cell<EOS, VISC, MILNE>(P, A, c, qo, ec, valid, nfail, nnonf, minfac);
-  if (!(P.debug & 1)) flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0, *(volatile unsigned long long*)&A.cnt->min_reg_bits);
+  flush_counters(A.cnt, valid ? nfail : 0ull, valid ? nnonf : 0ull, valid ? minfac : 1.0, *(volatile unsigned long long*)&A.cnt->min_reg_bits);
 }
 
 // ------------------------------------------------------------------------------------------------ ghost cells (Eqs. 75-76)

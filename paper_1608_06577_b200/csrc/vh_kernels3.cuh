@@ -522,10 +522,11 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
   if (fail) ++nfail;
   const double p0 = eos_p<EOS>(P, e);
   const double Pt = p0 + Pi;
-  const double ut = sqrt_fast((E + Pt) * rcp_fast(e + Pt));      // Eq. 53
+  bool ut_ok;
+  const double ut = u_tau_checked(E + Pt, e + Pt, ut_ok);        // Eq. 53
   const double inv = rcp_fast((e + Pt) * ut);                    // Eq. 54
   const double u[4] = {ut, Mx * inv, My * inv, Mn * inv};
-  if (!(isfinite(e) && isfinite(ut))) ++nnonf;
+  if (!(isfinite(e) && ut_ok)) ++nnonf;
   if (valid) {      // results that the regularisation does not touch go out first: their stores drain while rho is being computed
 #pragma unroll
     for (int n = 0; n < 4; ++n) A.q_out[n * fs + c] = qv[n];

@@ -59,12 +59,7 @@ static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
     if (A.regfac) return launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE, true>(h, A);
   }
   auto kern = stage_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, STAGE, REGMAP>;
-  static bool configured = false;      // one attribute call per instantiation (single device per process)
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  if (cudaError_t e = vh_opt_in_smem(h, (const void*)kern, smem); e != cudaSuccess) return e;
   const DevParams& P = h->P;
   dim3 grid((P.nx + T::TX - 1) / T::TX, (P.ny + T::TY - 1) / T::TY, ((P.nz + T::TZ - 1) / T::TZ) * P.n_batch);
   kern<<<grid, T::NT, smem, h->stream>>>(P, A, h->mapA, h->mapZ, h->mapC);
@@ -79,12 +74,7 @@ static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cu
     using V = VTile<TWO_D>;
     constexpr size_t vsmem = vtile_smem_bytes<TWO_D, VISC>();
     auto vkern = velocity_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1>;
-    static bool configured = false;      // one attribute call per instantiation (single device per process)
-    if (!configured) {
-      cudaError_t e = cudaFuncSetAttribute(vkern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vsmem);
-      if (e != cudaSuccess) return e;
-      configured = true;
-    }
+    if (cudaError_t e = vh_opt_in_smem(h, (const void*)vkern, vsmem); e != cudaSuccess) return e;
     dim3 grid((P.nx + V::VX - 1) / V::VX, (P.ny + V::VY - 1) / V::VY, ((P.nz + V::VZ - 1) / V::VZ) * P.n_batch);
     VelTileArgs VA{S.e_in, h->vL, h->vR, S.cnt, S.t, (int)((S.q_in - h->pool) / fs)};
     vkern<<<grid, V::NT, vsmem, h->stream>>>(P, VA, h->mapVA, h->mapVZ);

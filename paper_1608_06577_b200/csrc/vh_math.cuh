@@ -97,8 +97,16 @@ __device__ __forceinline__ double newton_single(const DevParams& P, double E, do
     if (fabs(d) <= P.newton_rtol * fabs(en)) { conv = true; done = true; }
   }
   fail = bad || !conv || !(e > 0.0) || !isfinite(e);
-  if (fail) e = fmax(E, 1e-300);
+  if (fail) e = (1e-300 > E) ? 1e-300 : E;      // max(E, tiny) that keeps a NaN E (fmax would drop it and hide the cell from n_nonfinite)
   return e;
+}
+
+// u^tau = sqrt((E + P)/(e + P)) of Eq. 53 and whether it is a number: the IEEE square root of a negative, infinite or NaN quotient is
+// not finite, which sqrt_fast() alone would hide (it returns 0 there); such a cell is counted in n_nonfinite and carries NaN
+__device__ __forceinline__ double u_tau_checked(double E_plus_P, double e_plus_P, bool& finite) {
+  const double x = E_plus_P * rcp_fast(e_plus_P);
+  finite = (x >= 0.0) && (x < CUDART_INF);
+  return finite ? sqrt_fast(x) : CUDART_NAN;
 }
 
 // clip of a failed state's velocity (R6)

@@ -1,0 +1,146 @@
+"""GPU <-> oracle parity, second file: the stated configurations at their stated sizes (BASELINE.json north_star: "the full viscous
+128^3 KT step matches the oracle within 1e-9 after 10 steps"; configs[1] as written, 201 x 201), all kernel variants on the generic
+state, and forced inversion failures / non-finite cells with the status counters compared exactly.  Same norm and helpers as
+tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_1608_06577_b200 import inputs
+from test_gpu_parity import NOISE, TOL, _subbox_worst, assert_parity, field_errors, vh  # noqa: F401  (vh is the module fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def _t(a):
+    import torch
+    return None if a is None else torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_kernel_variants_generic_state(vh, vo, variant):
+    # the two retained A/B pipelines (variant 1: one-thread-per-cell kernel + ghost kernel; variant 2: velocity kernel + stage kernel
+    # through L1) on the input that exercises every term: vorticity, u^eta != 0, all ten pi components, Pi, u^{n-1} != u^n, ragged tiles
+    prm = inputs.base_params(nx=36, ny=20, nz=10, dx=0.12, dy=0.1, dz=0.15, tau0=0.8, dtau=0.02)
+    st = inputs.smooth_random_state(prm, seed=21)
+    up = st["u"] * 1.0
+    up[1:] *= 0.97
+    up[0] = np.sqrt(1 + up[1] ** 2 + up[2] ** 2 + prm["tau0"] ** 2 * up[3] ** 2)
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], st["pi"], st["Pi"])
+    o.set_uprev(up)
+    o.step(10)
+    s = vh.Solver(prm)
+    s.set_kernel_variant(variant)
+    s.set_initial(_t(st["e"]), _t(st["u"]), _t(st["pi"]), _t(st["Pi"]))
+    s.set_uprev(_t(up))
+    s.step(10)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields(with_uprev=True).items()}
+    sg = s.status()
+    s.close()
+    assert_parity(o.get_fields(with_uprev=True), o.status(), fg, sg)
+
+
+def _state_with_bad_cell(vh, vo, prm, st, cell, T_tt, Pi_val):
+    """Both sides start from the same (q, e, u, u_prev) in which one cell's T^{tau tau} (and Pi) was overwritten."""
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], st.get("pi"), st.get("Pi"))
+    f0 = o.get_fields(with_uprev=True)
+    k, j, i = cell
+    o.raw("q", 0)[k + 2, j + 2, i + 2] = T_tt
+    if Pi_val is not None:
+        o.raw("q", 14)[k + 2, j + 2, i + 2] = Pi_val
+    o.ghost()
+    q = f0["q"].copy()
+    q[0][0, k, j, i] = T_tt
+    if Pi_val is not None:
+        q[14][0, k, j, i] = Pi_val
+    s = vh.Solver(prm)
+    return o, s, q, f0
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_forced_failure_single_cell_counts_nonfinite(vh, vo, variant):
+    # one cell (all neighbours are its ghost copies) with E = T^{tau tau} - pi^{tau tau} < 0: the cell inversion of stage 1 fails
+    # (R6: e = tiny), (E + P)/(e + P) < 0 makes u^tau of Eq. 53 not a number, stage 2 then sees NaN: 2 failures, 2 non-finite cells
+    # (shear only: with bulk on, Pi* < 0 from the relaxation makes the quotient of Eq. 53 positive again)
+    prm = inputs.base_params(nx=1, ny=1, nz=1, tau0=0.7, dtau=0.02, physics=1)
+    shp = (1, 1, 1, 1)
+    st = {"e": np.full(shp, 12.0), "u": inputs.rest_velocity(shp)}
+    o, s, q, f0 = _state_with_bad_cell(vh, vo, prm, st, (0, 0, 0), -1.0, None)
+    s.set_kernel_variant(variant)
+    s.set_state(_t(q), _t(f0["e"]), _t(f0["u"]), _t(f0["up"]))
+    o.step(1)
+    s.step(1)
+    so, sg = o.status(), s.status()
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields().items()}
+    s.close()
+    assert so["n_inversion_failures"] == 2 and so["n_nonfinite"] == 2
+    assert sg["n_inversion_failures"] == so["n_inversion_failures"]
+    assert sg["n_nonfinite"] == so["n_nonfinite"]
+    assert not np.isfinite(fg["u"][0]).all() and not np.isfinite(o.get_fields()["u"][0]).all()      # the blow-up is visible in the fields
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_forced_failures_in_a_grid_counters_and_fields(vh, vo, variant):
+    # a cell with E < 0 but E + Pi > 0: every inversion of that cell and of the states extrapolated from it fails (R6: e = max(E, tiny),
+    # velocity from M/(E + P) clipped), yet everything stays finite - failure counters must agree exactly and the fields to 1e-9
+    prm = inputs.base_params(nx=36, ny=8, nz=6, tau0=0.7, dtau=0.01)
+    st = inputs.smooth_random_state(prm, seed=17)
+    cell = (3, 4, 20)
+    o, s, q, f0 = _state_with_bad_cell(vh, vo, prm, st, cell, None, None)
+    k, j, i = cell
+    E_bad = -0.05 * f0["e"][0, k, j, i]
+    T_tt = E_bad + f0["q"][4][0, k, j, i]
+    Pi_val = 0.5 * f0["e"][0, k, j, i]
+    o, s, q, f0 = _state_with_bad_cell(vh, vo, prm, st, cell, T_tt, Pi_val)
+    s.set_kernel_variant(variant)
+    s.set_state(_t(q), _t(f0["e"]), _t(f0["u"]), _t(f0["up"]))
+    o.step(1)
+    s.step(1)
+    so, sg = o.status(), s.status()
+    fo = o.get_fields(with_uprev=True)
+    fg = {k_: v.cpu().numpy() for k_, v in s.get_fields(with_uprev=True).items()}
+    s.close()
+    assert so["n_inversion_failures"] >= 6 and so["n_nonfinite"] == 0
+    assert np.isfinite(fo["q"]).all() and np.isfinite(fg["q"]).all()
+    assert_parity(fo, so, fg, sg)
+
+
+def test_north_star_128cubed_ten_steps(vh, vo):
+    """BASELINE.json north_star at its stated size: configs[2] (128^3 viscous, the launch configuration bench.py times) for TEN
+    steps.  One RK2 step has a domain of dependence of +-4 cells (two stages of the +-2 stencil), so the oracle is run on 88^3
+    sub-boxes cut out of the same initial data and compared on the cells 40 away from every cut face (all the way to a face that is
+    the domain boundary): one box in a domain corner, one centred on the hottest cell."""
+    prm, init, _ = inputs.config_3d()
+    s = vh.Solver(prm)
+    s.set_initial(_t(init["e"]), _t(init["u"]))
+    s.step(10)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields().items()}
+    sg = s.status()
+    s.close()
+    assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
+    B, H = 88, 40
+    kz, ky, kx = np.unravel_index(np.argmax(init["e"][0]), init["e"][0].shape)
+    clamp = lambda c: int(min(max(c - B // 2, 0), 128 - B))
+    boxes = [(0, 0, 0), (clamp(kx), clamp(ky), clamp(kz))]
+    worst = _subbox_worst(vo, prm, init, fg, boxes, B, H, 10)
+    assert worst <= TOL, worst
+
+
+@pytest.mark.parametrize("n_steps,tol", [(10, 1e-9), (50, 1e-8)])
+def test_config2_gubser_as_written(vh, vo, n_steps, tol):
+    # BASELINE configs[1] as written: 201 x 201, dx = 0.05, dtau = 0.0125, theta = 1.8, Eq. 74 applied literally (DESIGN.md section 7
+    # explains why parity beyond ~100 steps of this configuration is ill-conditioned for ANY two implementations)
+    prm, init, _, _ = inputs.config_gubser()
+    assert prm["nx"] == 201 and prm["ny"] == 201
+    o = vo.Oracle(prm)
+    o.set_initial(init["e"], init["u"], init.get("pi"), init.get("Pi"))
+    o.step(n_steps)
+    s = vh.Solver(prm)
+    s.set_initial(_t(init["e"]), _t(init["u"]), _t(init.get("pi")), _t(init.get("Pi")))
+    s.step(n_steps)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields(with_uprev=True).items()}
+    sg = s.status()
+    s.close()
+    assert o.status()["n_inversion_failures"] == 0
+    assert_parity(o.get_fields(with_uprev=True), o.status(), fg, sg, tol=tol)
