@@ -29,9 +29,56 @@ METRIC = "cell-updates/s (full RK2 KT step, FP64) at 128^3 viscous"
 UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_UPDATE = 856.0      # 107 doubles per cell-update, each state array read/written once per stage
 ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the stage kernel at 128^3 from the committed ncu --set full
-# capture (profiles/r01c_ncu_summary.md); valid for the default workload (128^3) only
-NCU_TRAFFIC_BYTES = {"stage1": 629327104 + 353338112, "stage2": 932169216 + 358881024}      # profiles/r01c_ncu_summary.md
+# Raw `ncu --csv` metric page of one RK2 step of THIS workload (four launches, in launch order), committed with the build it was taken
+# from; the command is in profiles/r02_metrics.md.  bench.py reads DRAM traffic, executed DFMA/DADD/DMUL and FP64-pipe utilisation per
+# launch from it (they are properties of the build, not of a run: ncu replays kernels and cannot be on while timing).
+NCU_METRICS_CSV = os.path.join(ROOT, "profiles", "r02_metrics.csv")
+LAUNCH_KEYS = ("velocity1", "stage1", "velocity2", "stage2")
+
+
+def ncu_metrics(path=NCU_METRICS_CSV):
+    """{launch key: {metric: value}} from the committed raw ncu CSV (rows: one per launch and metric), or {} if it is absent or does
+    not hold exactly one step of the default pipeline (velocity, stage, velocity, stage)."""
+    import csv
+    if not os.path.exists(path):
+        return {}
+    rows = list(csv.reader(l for l in open(path) if l.startswith('"')))
+    if not rows:
+        return {}
+    h = rows[0]
+    try:
+        ki, mi, vi, ii = h.index("Kernel Name"), h.index("Metric Name"), h.index("Metric Value"), h.index("ID")
+    except ValueError:
+        return {}
+    per, order = {}, []
+    for r in rows[1:]:
+        if r[ii] not in per:
+            per[r[ii]] = {"kernel": r[ki]}
+            order.append(r[ii])
+        try:
+            per[r[ii]][r[mi]] = float(r[vi].replace(",", ""))
+        except ValueError:
+            pass
+    if len(order) != 4:
+        return {}
+    out = {}
+    for key, lid in zip(LAUNCH_KEYS, order):
+        if ("velocity" in key) != ("velocity" in per[lid]["kernel"]):
+            return {}
+        out[key] = per[lid]
+    return out
+
+
+def host_cpu():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return model, os.cpu_count()
 
 
 def workload(rank=0, physics="config3"):
@@ -173,18 +220,19 @@ def time_oracle(prm, init, dims, steps, warmup=0):
         o.step(warmup)
     dt = o.time_steps(steps)
     ncell = dims[0] * dims[1] * dims[2]
-    return ncell * steps / dt, dt, "central %dx%dx%d cut-out of the 128^3 initial data, %d RK2 step(s), serial C++ oracle -O2" % (dims[0], dims[1], dims[2], steps)
+    what = "the full %dx%dx%d workload" % dims if dims == (prm["nx"], prm["ny"], prm["nz"]) else "central %dx%dx%d cut-out of the 128^3 initial data" % dims
+    return ncell * steps / dt, dt, "%s, %d RK2 step(s), serial C++ oracle -O2, 1 core" % (what, steps)
 
 
 def algorithmic_flops(prm, init):
-    """Measured algorithmic flop count per cell-update (oracle with an operation-counting scalar on a 16^3 cut-out, every
-    interface charged once; weights of SURVEY.md 8(d)).  Test infrastructure used for the report only."""
+    """MINIMAL algorithmic flop count per cell-update: the oracle with an operation-counting scalar on a 16^3 cut-out; every interface
+    charged once, every limited slope once, compares excluded, exact 0 / +-1 constants not counted; weights of SURVEY.md 8(d).
+    Returns (flops, per-class op counts, flops per oracle section).  Test infrastructure used for the report only."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import vh_oracle
 
     sub, e, u = oracle_sample(prm, init, 16, 16, 16)
-    flops, plain, per = vh_oracle.algorithmic_flops_per_cell_update(sub, e, u)
-    return flops, plain, per
+    return vh_oracle.algorithmic_flops_per_cell_update(sub, e, u)
 
 
 def run_reference(args):
@@ -193,13 +241,14 @@ def run_reference(args):
         return 0
     prm, init = workload(0, args.physics)
     dims = (64, 64, 32)
-    warm = min(args.warmup, 1)
+    warm = args.warmup
     value, dt, sample = time_oracle(prm, init, dims, args.steps, warmup=warm)
+    model, ncores = host_cpu()
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": warm,
         "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": "configs[2]: 128^3 3+1d viscous non-conformal, seeded hotspots; bounded sample " + sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "host_cpu": model, "host_cores_total": ncores},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -216,6 +265,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0, help="stage-kernel variant (vh_set_kernel_variant), 0 = default")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-paper-physics", action="store_true", help="skip the second, labelled measurement with the lattice EOS and Eq. 17 zeta/s")
     ap.add_argument("--physics", default="config3", choices=["config3", "paper"], help="paper: lattice EOS + Eq. 17 zeta/s on the config-3 grid")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -304,6 +354,25 @@ def main():
     copy_gbs, fp64_gflops = vh.measure_peaks(n_bytes=1 << 30, repeats=10)
     s.close()
 
+    # ---------------- second, labelled workload: the paper's own physics (lattice EOS, Eq. 17 zeta/s) on the same grid
+    paper_line = None
+    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics:
+        prm2, init2 = workload(rank, "paper")
+        s2 = vh.Solver(prm2, device=dev)
+        s2.set_initial(torch.as_tensor(init2["e"], device=dev), torch.as_tensor(init2["u"], device=dev))
+        s2.step(W)
+        torch.cuda.synchronize()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(); s2.step(K); a1.record()
+        torch.cuda.synchronize()
+        ms2 = a0.elapsed_time(a1)
+        st2 = s2.status()
+        prof2 = s2.step_profile(min(K, 10))
+        s2.close()
+        paper_line = {"workload": "configs[2] grid and hotspots with the paper's own physics: lattice EOS (Eqs. 19-20), zeta/s of Eq. 17 (T_c = 200 MeV)",
+                      "ms_per_step": ms2 / K, "value": ncell * K / (ms2 * 1e-3), "unit": UNIT, "per_kernel_ms": prof2,
+                      "n_inversion_failures": st2["n_inversion_failures"], "n_nonfinite": st2["n_nonfinite"]}
+
     if rank == 0:
         peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
         hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
@@ -312,19 +381,35 @@ def main():
                 hbm_peak, hbm_src = float(json.load(open(peaks_file))["hbm_gbs"]), "MEASURED_PEAKS.json"
             except Exception:
                 pass
-        flops_cu, plain_cu, mix = algorithmic_flops(prm, init)
-        flops_inv_cu = mix.pop("flops_interface_inversions")
+        flops_cu, mix, by_section = algorithmic_flops(prm, init)
+        flops_inv_cu = by_section["invert"]
+        variant1 = (args.variant == 1)
+        default_pipeline = (args.variant == 0)
         # Kernel shares of the algorithmic work: the velocity kernel does the interface-state inversions
         # (Eq. 72 at every reconstructed state), the stage kernel everything else; one stage = half of a cell-update.
-        variant1 = (args.variant == 1)
-        stage_keys = ("stage1", "stage2")
-        dom = max(stage_keys, key=lambda k: prof[k])            # dominant kernel: the longer of the two stage-kernel launches
+        alg_kernel = {k: 0.5 * (flops_inv_cu if "velocity" in k else flops_cu - flops_inv_cu) for k in LAUNCH_KEYS}
+        if variant1:
+            alg_kernel = {"stage1": 0.5 * flops_cu, "stage2": 0.5 * flops_cu}
+        bytes_kernel = {"stage1": ALG_BYTES_STAGE["stage1"], "stage2": ALG_BYTES_STAGE["stage2"], "velocity1": 10 * 8.0, "velocity2": 10 * 8.0}
+        ncu = ncu_metrics() if (ncell == 128 ** 3 and default_pipeline and args.physics == "config3") else {}
+        ex_kernel, pipe_kernel, traffic_kernel = {}, {}, {}
+        for k, m in ncu.items():
+            try:
+                ex_kernel[k] = (2.0 * m["smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"] + m["smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"]
+                                + m["smsp__sass_thread_inst_executed_op_dmul_pred_on.sum"]) / ncell
+                pipe_kernel[k] = m["sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"] / 100.0
+                traffic_kernel[k] = m["dram__bytes_read.sum"] + m["dram__bytes_write.sum"]
+            except KeyError:
+                pass
+        # dominant kernel: the longest of the step's launches, velocity kernels included
+        cand = [k for k in prof if k in alg_kernel]
+        dom = max(cand, key=lambda k: prof[k])
         dur = prof[dom] * 1e-3
-        flops_stage = 0.5 * (flops_cu if variant1 else flops_cu - flops_inv_cu)
-        flops_launch = flops_stage * ncell
-        # algorithmic bytes of the stage kernel: the state arrays of SURVEY 8(d) (each read / written once per stage) plus,
-        # in the split pipeline, the six state velocities it reads back (they are a by-product, not state: not counted)
-        bytes_launch = ALG_BYTES_STAGE[dom] * ncell
+        # Useful flops of a launch: the minimal algorithmic count, but never more than the kernel executes (2 DFMA + DADD + DMUL, ncu):
+        # where the kernel gets by with fewer flops than the count, the count still holds work the method does not need.
+        useful = {k: min(alg_kernel[k], ex_kernel.get(k, alg_kernel[k])) for k in cand}
+        flops_launch = useful[dom] * ncell
+        bytes_launch = bytes_kernel[dom] * ncell
         t_alu = flops_launch / (fp64_gflops * 1e9)
         t_hbm = bytes_launch / (hbm_peak * 1e9)
         if t_alu >= t_hbm:
@@ -332,20 +417,31 @@ def main():
         else:
             roof = {"bound": "hbm", "achieved": bytes_launch / dur / 1e9, "peak": hbm_peak, "unit": "GB/s"}
         roof["frac"] = roof["achieved"] / roof["peak"]
-        step_roof_s = max(flops_cu * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9))
+        useful_step = sum(useful.values())
+        step_roof_s = max(useful_step * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9))
+        kname = ("velocity_tile_kernel" if "velocity" in dom else "stage_tile_kernel") if default_pipeline else ("stage_cell_kernel" if variant1 else "stage_kernel")
         roof.update({
-            "traffic": NCU_TRAFFIC_BYTES.get(dom) if (ncell == 128 ** 3 and not args.variant and args.physics == "config3") else None, "kernel": "stage_tile_kernel (%s)" % dom if not variant1 else "stage_cell_kernel (%s)" % dom,
-            "launch_ms": prof[dom],
+            "traffic": traffic_kernel.get(dom), "traffic_source": os.path.relpath(NCU_METRICS_CSV, ROOT) if dom in traffic_kernel else None,
+            "kernel": "%s (%s)" % (kname, dom), "launch_ms": prof[dom],
             "peak_source": "FP64 FMA microbenchmark, same run (vh_measure_peaks)" if roof["bound"] == "alu" else hbm_src,
-            "alg_flops_per_cell_update": flops_cu, "alg_flops_interface_inversions_per_cell_update": flops_inv_cu,
-            "alg_flops_this_kernel_per_cell": flops_stage, "alg_bytes_per_cell_update": ALG_BYTES_PER_CELL_UPDATE,
-            "alg_bytes_this_kernel_per_cell": ALG_BYTES_STAGE[dom],
-            "flop_weights": "add/mul/cmp 1, div 10, sqrt 15, exp 25, pow 30, tanh 40 (SURVEY 8(d)); counted on the oracle, each interface once",
+            "numerator": "min(minimal algorithmic flops, executed flops) of this kernel per cell x cells per launch",
+            "alg_flops_this_kernel_per_cell": alg_kernel[dom], "executed_flops_per_cell": ex_kernel.get(dom),
+            "alg_over_executed": (alg_kernel[dom] / ex_kernel[dom]) if dom in ex_kernel else None,
+            "fp64_pipe_util": pipe_kernel.get(dom),
+            "frac_on_minimal_count": alg_kernel[dom] * ncell / dur / (fp64_gflops * 1e9),
+            "alg_flops_per_cell_update": flops_cu, "alg_flops_by_section_per_cell_update": {k: round(v, 1) for k, v in by_section.items()},
+            "executed_flops_per_cell_update": sum(ex_kernel.values()) if len(ex_kernel) == 4 else None,
+            "alg_bytes_per_cell_update": ALG_BYTES_PER_CELL_UPDATE, "alg_bytes_this_kernel_per_cell": bytes_kernel[dom],
+            "flop_weights": "add/mul 1, div 10, sqrt 15, exp 25, pow 30, tanh 40 (SURVEY 8(d)); compares carry no weight; counted on the oracle with "
+                            "each interface once, each limited slope once, exact 0/+-1 constants not counted",
             "op_mix_per_cell_update": {k: round(v, 1) for k, v in mix.items()},
             "hbm_view": {"achieved_gbs": bytes_launch / dur / 1e9, "peak_gbs": hbm_peak, "peak_source": hbm_src, "frac": bytes_launch / dur / 1e9 / hbm_peak,
                          "copy_gbs_same_run": copy_gbs},
             "step_roofline_ms": step_roof_s * 1e3, "step_frac": step_roof_s / (ms / K * 1e-3),
             "per_kernel_ms": prof,
+            "per_kernel": {k: {"ms": prof[k], "alg_flops_per_cell": alg_kernel[k], "executed_flops_per_cell": ex_kernel.get(k),
+                               "frac": useful[k] * ncell / (prof[k] * 1e-3) / (fp64_gflops * 1e9), "fp64_pipe_util": pipe_kernel.get(k),
+                               "traffic": traffic_kernel.get(k), "alg_bytes": bytes_kernel[k] * ncell} for k in cand},
         })
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
@@ -354,7 +450,7 @@ def main():
                                     "dtau=0.025, one independent replica per GPU (no sharding, no collective)") if args.physics == "config3" else
                                    ("configs[2] grid and hotspots with the paper's own physics: lattice EOS (Eqs. 19-20), zeta/s of Eq. 17 (T_c = 200 MeV), "
                                     "eta/s=0.2; one independent replica per GPU"),
-                       "l2": "state (61 arrays, 1.34 GB) exceeds the 126 MB L2; no flush needed", "kernel_variant": args.variant,
+                       "l2": "state (67 padded arrays, 1.34 GB) exceeds the 126 MB L2; no flush needed", "kernel_variant": args.variant,
                        "paper_context": "GTX 980 Ti, FP32, lattice EOS: 244.45 ms/step = 8.58e6 cell-updates/s (PAPER.md Table 3; another machine, not a target)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": E,
                     "what": "per step: vh_set_initial(host e,u,pi,Pi) + vh_step(1) + vh_get_fields(host q,e,p,u), pinned buffers"},
@@ -364,9 +460,14 @@ def main():
             "status": {"n_inversion_failures": st["n_inversion_failures"], "n_nonfinite": st["n_nonfinite"], "min_reg_factor": st["min_reg_factor"]},
             "measured_peaks_same_run": {"copy_gbs": copy_gbs, "fp64_fma_gflops": fp64_gflops},
         }
+        if paper_line is not None:
+            line["paper_physics"] = paper_line
         if world == 1 and not args.no_cpu_baseline:
-            v, dt, sample = time_oracle(prm, init, (96, 96, 64), 2)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "seconds": dt}
+            # SURVEY 8(d) "Oracle timing": the serial oracle on the FULL workload for 3 steps (about 40 s), 1 core, CPU model and core count stated
+            v, dt, sample = time_oracle(prm, init, (prm["nx"], prm["ny"], prm["nz"]), 3)
+            model, ncores = host_cpu()
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "seconds": dt, "host_cpu": model,
+                                    "host_cores_total": ncores}
         print(json.dumps(line))
     if dist is not None:
         dist.barrier()
