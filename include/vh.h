@@ -42,7 +42,7 @@ typedef struct {
   int nx, ny, nz, n_batch;          /* physical cells per event; nz == 1 -> 2+1d (:474); n_batch >= 1 independent events  */
   double dx, dy, dz;                /* fm, fm, rapidity units                                                           */
   double tau0, dtau;                /* fm                                                                               */
-  int geometry;                     /* 0 Milne (Eqs. 27-29); 1 Cartesian, ideal only: G terms off, tau^2 -> 1 (:684)      */
+  int geometry;                     /* 0 Milne (Eqs. 27-29); 1 Cartesian: G terms and Christoffel symbols off, tau^2 -> 1 (:684) */
   int physics;                      /* bit0 shear pi^{mu nu}, bit1 bulk Pi; 0 = ideal (pi, Pi stay 0)                     */
   int eos;                          /* 0: p = e/3;  1: p = (e/3)(1 - alpha exp(-e/e0));  T = (e/a)^{1/4} for both;         */
                                     /* 2: lattice EOS of Eqs. 19-20 (:200-215) with T(e), c_s^2 from its table (DESIGN R19, R20) */

@@ -47,7 +47,7 @@ struct Params {
   int nx, ny, nz, n_batch;     // physical cells; nz==1 -> 2+1d; n_batch independent events
   double dx, dy, dz;           // fm, fm, rapidity
   double tau0, dtau;           // fm
-  int geometry;                // 0 Milne, 1 Cartesian (ideal only, R12)
+  int geometry;                // 0 Milne, 1 Cartesian (R12: the paper uses it for its ideal tests; the viscous terms work too, pinned by tests/test_oracle_cartesian.py)
   int physics;                 // bit0 shear, bit1 bulk; 0 ideal
   int eos;                     // 0: p=e/3; 1: p=(e/3)(1-alpha*exp(-e/e0)), T=(e/a)^(1/4) for both; 2: lattice EOS (Eqs. 19-20), T(e) from its table
   double eos_a, eos_alpha, eos_e0;

@@ -15,7 +15,6 @@ struct vho_handle { vho::Params P; std::vector<Sol*> ev; };
 
 vho_handle* vho_create(const vho::Params* P) {
   if (!P || P->nx < 1 || P->ny < 1 || P->nz < 1 || P->n_batch < 1) return nullptr;
-  if (P->geometry == 1 && P->physics != 0) return nullptr;   // R12
   vho_handle* h = new vho_handle;
   h->P = *P;
   for (int b = 0; b < P->n_batch; ++b) h->ev.push_back(new Sol(*P));

@@ -2,7 +2,7 @@
 
     python -m paper_1608_06577_b200.build [--force] [--verbose]
 
-vh_api.cu and nine launch units (vh_launch.cu compiled with -DVH_COMBO=0..8, one per EOS / viscous / Milne combination) are
+vh_api.cu and twelve launch units (vh_launch.cu compiled with -DVH_COMBO=0..11, one per EOS / viscous / Milne combination) are
 compiled in parallel to objects under csrc/build/ and linked into libvh.so.  The built .so is git-ignored but travels with the
 source tree; nothing is JIT-compiled at import time."""
 import os
@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 SO = os.path.join(HERE, "libvh.so")
-N_COMBO = 9
+N_COMBO = 12
 HEADERS = ["vh_device.cuh", "vh_math.cuh", "vh_kernels.cuh", "vh_kernels2.cuh", "vh_kernels3.cuh", "vh_kernels4.cuh", "vh_internal.cuh", "vh_eos_lattice.hpp",
            os.path.join("..", "..", "include", "vh.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]

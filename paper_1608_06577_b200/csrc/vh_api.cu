@@ -77,7 +77,6 @@ static int check_params(const vh_params* p, std::string& why) {
   if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->n_batch < 1) { why = "grid extents and n_batch must be >= 1"; return -1; }
   if (!(p->dx > 0 && p->dy > 0 && p->dz > 0 && p->dtau > 0)) { why = "spacings and dtau must be > 0"; return -1; }
   if (p->geometry != 0 && p->geometry != 1) { why = "geometry must be 0 (Milne) or 1 (Cartesian)"; return -1; }
-  if (p->geometry == 1 && p->physics != 0) { why = "Cartesian geometry supports ideal physics only (PAPER.md:684)"; return -1; }
   if (p->geometry == 0 && !(p->tau0 > 0)) { why = "Milne geometry needs tau0 > 0"; return -1; }
   if (p->physics < 0 || p->physics > 3) { why = "physics must be a combination of bit0 (shear) and bit1 (bulk)"; return -1; }
   if (p->eos < 0 || p->eos > 2) { why = "eos must be 0, 1 or 2"; return -1; }
@@ -98,7 +97,7 @@ static int check_params(const vh_params* p, std::string& why) {
 #define debug_sync vh_debug_sync
 // one Euler stage with the handle's kernel variant: the launch units are compiled per (EOS, viscous, Milne) combination
 static cudaError_t launch_stage_any(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
-  const int phys = (h->prm.physics != 0) ? 0 : ((h->prm.geometry == 0) ? 1 : 2);
+  const int phys = (h->prm.physics != 0) ? ((h->prm.geometry == 0) ? 0 : 3) : ((h->prm.geometry == 0) ? 1 : 2);
   switch (h->prm.eos + 3 * phys) {
     case 0: return vh_launch_stage_combo0(h, stage, A, mid);
     case 1: return vh_launch_stage_combo1(h, stage, A, mid);
@@ -108,7 +107,10 @@ static cudaError_t launch_stage_any(vh_handle* h, int stage, const StageArgs& A,
     case 5: return vh_launch_stage_combo5(h, stage, A, mid);
     case 6: return vh_launch_stage_combo6(h, stage, A, mid);
     case 7: return vh_launch_stage_combo7(h, stage, A, mid);
-    default: return vh_launch_stage_combo8(h, stage, A, mid);
+    case 8: return vh_launch_stage_combo8(h, stage, A, mid);
+    case 9: return vh_launch_stage_combo9(h, stage, A, mid);
+    case 10: return vh_launch_stage_combo10(h, stage, A, mid);
+    default: return vh_launch_stage_combo11(h, stage, A, mid);
   }
 }
 

@@ -220,42 +220,46 @@ struct Kin {            // kinematic scalars / tensors at a cell (App. A)
   double W[6];          // W^{tx} W^{ty} W^{tn} W^{xy} W^{xn} W^{yn} (A.14-A.19)
 };
 
-// u = (ut,ux,uy,un); dt,dx,dy,dn = partial derivatives of the four components (:424)
+// u = (ut,ux,uy,un); dt,dx,dy,dn = partial derivatives of the four components (:424).
+// MILNE = false is the Cartesian mode (R12): metric factors tau^2 -> 1 (t2, g2i) and every Christoffel symbol -> 0 (ch = Gamma^eta_{eta tau}
+// = 1/tau, ct = Gamma^tau_{eta eta} = tau), kept apart so that each falls out at compile time.
+template <bool MILNE>
 __device__ __forceinline__ void kinematics(const double u[4], const double dt[4], const double dx[4], const double dy[4], const double dn[4],
                                            double t, Kin& K) {
   const double ut = u[0], ux = u[1], uy = u[2], un = u[3];
-  const double it = 1.0 / t, it2 = it * it, t2 = t * t;
+  const double t2 = MILNE ? t * t : 1.0, g2i = MILNE ? 1.0 / (t * t) : 1.0;
+  const double ch = MILNE ? 1.0 / t : 0.0, ct = MILNE ? t : 0.0;
   // convective derivatives (A.5-A.8)
   double dut = ut * dt[0] + ux * dx[0] + uy * dy[0] + un * dn[0];
   double dux = ut * dt[1] + ux * dx[1] + uy * dy[1] + un * dn[1];
   double duy = ut * dt[2] + ux * dx[2] + uy * dy[2] + un * dn[2];
   double dun = ut * dt[3] + ux * dx[3] + uy * dy[3] + un * dn[3];
-  double th = ut * it + dt[0] + dx[1] + dy[2] + dn[3];                 // A.11
+  double th = ut * ch + dt[0] + dx[1] + dy[2] + dn[3];                 // A.11
   double th3 = th * (1.0 / 3.0);
   K.theta = th;
-  K.Du[0] = dut + t * un * un;                                          // A.9
+  K.Du[0] = dut + ct * un * un;                                         // A.9
   K.Du[1] = -dux;
   K.Du[2] = -duy;
-  K.Du[3] = -t2 * dun - 2.0 * t * ut * un;                              // A.10
+  K.Du[3] = -t2 * (dun + 2.0 * ch * ut * un);                           // A.10
   double un2 = un * un;
   // A.12 (D(.) read as the convective derivative of the contravariant component, reading in DESIGN.md)
-  K.sig[0] = -t * ut * un2 + dt[0] - ut * dut + (ut * ut - 1.0) * th3;
-  K.sig[1] = -0.5 * t * un2 * ux + 0.5 * (dt[1] - dx[0]) - 0.5 * (ut * dux + ux * dut) + ut * ux * th3;
-  K.sig[2] = -0.5 * t * un2 * uy + 0.5 * (dt[2] - dy[0]) - 0.5 * (ut * duy + uy * dut) + ut * uy * th3;
-  K.sig[3] = -0.5 * un * it * (2.0 * ut * ut + t2 * un2) + 0.5 * (dt[3] - dn[0] * it2) - 0.5 * (ut * dun + un * dut) + ut * un * th3;
+  K.sig[0] = -ct * ut * un2 + dt[0] - ut * dut + (ut * ut - 1.0) * th3;
+  K.sig[1] = -0.5 * ct * un2 * ux + 0.5 * (dt[1] - dx[0]) - 0.5 * (ut * dux + ux * dut) + ut * ux * th3;
+  K.sig[2] = -0.5 * ct * un2 * uy + 0.5 * (dt[2] - dy[0]) - 0.5 * (ut * duy + uy * dut) + ut * uy * th3;
+  K.sig[3] = -0.5 * un * (2.0 * ch * ut * ut + ct * un2) + 0.5 * (dt[3] - dn[0] * g2i) - 0.5 * (ut * dun + un * dut) + ut * un * th3;
   K.sig[4] = -dx[1] - ux * dux + (1.0 + ux * ux) * th3;
   K.sig[5] = -0.5 * (dx[2] + dy[1]) - 0.5 * (ux * duy + uy * dux) + ux * uy * th3;
-  K.sig[6] = -ut * ux * un * it - 0.5 * (dx[3] + dn[1] * it2) - 0.5 * (ux * dun + un * dux) + ux * un * th3;
+  K.sig[6] = -ut * ux * un * ch - 0.5 * (dx[3] + dn[1] * g2i) - 0.5 * (ux * dun + un * dux) + ux * un * th3;
   K.sig[7] = -dy[2] - uy * duy + (1.0 + uy * uy) * th3;
-  K.sig[8] = -ut * uy * un * it - 0.5 * (dy[3] + dn[2] * it2) - 0.5 * (uy * dun + un * duy) + uy * un * th3;
-  K.sig[9] = -ut * it2 * it * (1.0 + 2.0 * un2 * t2) - dn[3] * it2 - un * dun + (it2 + un2) * th3;
+  K.sig[8] = -ut * uy * un * ch - 0.5 * (dy[3] + dn[2] * g2i) - 0.5 * (uy * dun + un * duy) + uy * un * th3;
+  K.sig[9] = -ut * g2i * ch * (1.0 + 2.0 * un2 * t2) - dn[3] * g2i - un * dun + (g2i + un2) * th3;
   // A.14-A.19 divided by the metric factors so that W^{mu nu} is the contravariant antisymmetric tensor of :122
-  K.W[0] = 0.5 * (dt[1] + dx[0]) + 0.5 * (ux * dut - ut * dux) + 0.5 * t * un2 * ux;
-  K.W[1] = 0.5 * (dt[2] + dy[0]) + 0.5 * (uy * dut - ut * duy) + 0.5 * t * un2 * uy;
-  K.W[2] = un * it + 0.5 * dt[3] + 0.5 * dn[0] * it2 + 0.5 * (un * dut - ut * dun) - ut * ut * un * it + 0.5 * t * un2 * un;
+  K.W[0] = 0.5 * (dt[1] + dx[0]) + 0.5 * (ux * dut - ut * dux) + 0.5 * ct * un2 * ux;
+  K.W[1] = 0.5 * (dt[2] + dy[0]) + 0.5 * (uy * dut - ut * duy) + 0.5 * ct * un2 * uy;
+  K.W[2] = un * ch + 0.5 * dt[3] + 0.5 * dn[0] * g2i + 0.5 * (un * dut - ut * dun) - ut * ut * un * ch + 0.5 * ct * un2 * un;
   K.W[3] = 0.5 * (dy[1] - dx[2]) + 0.5 * (uy * dux - ux * duy);
-  K.W[4] = 0.5 * dn[1] * it2 - 0.5 * dx[3] + 0.5 * (un * dux - ux * dun) - ux * ut * un * it;
-  K.W[5] = 0.5 * dn[2] * it2 - 0.5 * dy[3] + 0.5 * (un * duy - uy * dun) - uy * ut * un * it;
+  K.W[4] = 0.5 * dn[1] * g2i - 0.5 * dx[3] + 0.5 * (un * dux - ux * dun) - ux * ut * un * ch;
+  K.W[5] = 0.5 * dn[2] * g2i - 0.5 * dy[3] + 0.5 * (un * duy - uy * dun) - uy * ut * un * ch;
 }
 
 // symmetric-slot lookup for 4x4 symmetric tensors stored as 10 (tt tx ty tn xx xy xn yy yn nn)
@@ -267,10 +271,11 @@ __device__ __forceinline__ constexpr int sym(int m, int n) {
 
 // Dissipative source terms J = S + G for the 10 pi components and Pi (B.10-B.12, Eqs. 39-46).
 // pi[10] in slot order; returns Jpi[10], JPi.
-template <int EOS>
+template <int EOS, bool MILNE>
 __device__ __forceinline__ void dissipative_sources(const DevParams& P, double t, const double u[4], const Kin& K, const double pi[10], double Pi,
                                                     double e, double p, double cs2, double divv, double Jpi[10], double& JPi) {
-  const double t2 = t * t, it = 1.0 / t;
+  const double t2 = MILNE ? t * t : 1.0, g2i = MILNE ? 1.0 / (t * t) : 1.0;      // metric factors
+  const double it = MILNE ? 1.0 / t : 0.0, ct = MILNE ? t : 0.0;                  // Christoffel symbols (0 in the Cartesian mode, R12)
   const double g[4] = {1.0, -1.0, -1.0, -t2};
   // transport coefficients (Eqs. 10-16; R14)
   double T = eos_temperature<EOS>(P, e);
@@ -307,15 +312,15 @@ __device__ __forceinline__ void dissipative_sources(const DevParams& P, double t
     }
   }
   double pisig = g[0] * C[0][0] + g[1] * C[1][1] + g[2] * C[2][2] + g[3] * C[3][3];      // pi^{mu nu} sigma_{mu nu}
-  const double gi[4] = {1.0, -1.0, -1.0, -it * it};
+  const double gi[4] = {1.0, -1.0, -1.0, -g2i};
   const double iut = 1.0 / u[0];
   // G_pi = u^a Gamma^mu_{ab} pi^{b nu} + (mu<->nu)  (:300; R1, R2)
   double G[10];
   const double ut = u[0], un = u[3];
-  G[0] = 2.0 * t * un * pi[3];
-  G[1] = t * un * pi[6];
-  G[2] = t * un * pi[8];
-  G[3] = t * un * pi[9] + (ut * pi[3] + un * pi[0]) * it;
+  G[0] = 2.0 * ct * un * pi[3];
+  G[1] = ct * un * pi[6];
+  G[2] = ct * un * pi[8];
+  G[3] = ct * un * pi[9] + (ut * pi[3] + un * pi[0]) * it;
   G[4] = 0.0; G[5] = 0.0;
   G[6] = (ut * pi[6] + un * pi[1]) * it;
   G[7] = 0.0;

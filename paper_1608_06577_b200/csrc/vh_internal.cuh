@@ -64,8 +64,8 @@ inline cudaError_t vh_opt_in_smem(vh_handle* h, const void* kern, size_t smem) {
 }
 
 // One Euler stage (kernels of the handle's variant) for one combination of template parameters; defined in vh_launch.cu.
-// combo = eos + 3 * (0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian), eos = 0, 1, 2.  mid (optional) is recorded between the two launches.
+// combo = eos + 3 * (0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian, 3: viscous Cartesian), eos = 0, 1, 2.  mid (optional) is recorded between the two launches.
 #define VH_DECLARE_COMBO(K) cudaError_t vh_launch_stage_combo##K(vh_handle* h, int stage, const vh::StageArgs& A, cudaEvent_t mid);
 VH_DECLARE_COMBO(0) VH_DECLARE_COMBO(1) VH_DECLARE_COMBO(2) VH_DECLARE_COMBO(3) VH_DECLARE_COMBO(4) VH_DECLARE_COMBO(5)
-VH_DECLARE_COMBO(6) VH_DECLARE_COMBO(7) VH_DECLARE_COMBO(8)
+VH_DECLARE_COMBO(6) VH_DECLARE_COMBO(7) VH_DECLARE_COMBO(8) VH_DECLARE_COMBO(9) VH_DECLARE_COMBO(10) VH_DECLARE_COMBO(11)
 #undef VH_DECLARE_COMBO

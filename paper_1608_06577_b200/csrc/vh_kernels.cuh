@@ -176,11 +176,11 @@ __device__ __forceinline__ void sources_cell(const DevParams& P, const StageArgs
   }
   if (VISC) {
     Kin K;
-    kinematics(uc, du[0], du[1], du[2], du[3], t, K);
+    kinematics<MILNE>(uc, du[0], du[1], du[2], du[3], t, K);
     double p0, cs2;
     eos_p_cs2<EOS>(P, ec, p0, cs2);
     double Jpi[10], JPi;
-    dissipative_sources<EOS>(P, t, uc, K, qc + PTT, qc[BPI], ec, p0, cs2, divv, Jpi, JPi);
+    dissipative_sources<EOS, MILNE>(P, t, uc, K, qc + PTT, qc[BPI], ec, p0, cs2, divv, Jpi, JPi);
     if (P.shear) {
 #pragma unroll
       for (int n = 0; n < 10; ++n) C[PTT + n] += Jpi[n];
@@ -407,12 +407,12 @@ __global__ void __launch_bounds__(256) pressure_kernel(const __grid_constant__ D
 // Second-order inverse Reynolds numbers (Eq. 90, :831): sqrt(J^{mu nu} J_{mu nu})/(2 eta sqrt(sigma^{mu nu} sigma_{mu nu})) and |J|/(zeta |theta|) with
 // J^{mu nu}, J of Eq. 5 at n^mu = 0.  In the notation of Eqs. 41-46: J^{mu nu}/tau_pi = -(delta_pipi I2 - I3 + tau_pipi I4 - lambda_piPi Pi sigma^{mu nu}),
 // J/tau_Pi = -(delta_PiPi Pi theta - lambda_Pipi pi^{mu nu} sigma_{mu nu}); eta/tau_pi and zeta/tau_Pi are the ratios the solver uses.
-template <int EOS>
+template <int EOS, bool MILNE>
 __device__ __forceinline__ void second_order_reynolds(const DevParams& P, double t, const double u[4], const Kin& K, const double pi[10], double Pi,
                                                       double e, double& r2_shear, double& r2_bulk) {
-  const double t2 = t * t, it = 1.0 / t;
+  const double t2 = MILNE ? t * t : 1.0;
   const double g[4] = {1.0, -1.0, -1.0, -t2};
-  const double gi[4] = {1.0, -1.0, -1.0, -it * it};
+  const double gi[4] = {1.0, -1.0, -1.0, -1.0 / t2};
   double p0, cs2;
   eos_p_cs2<EOS>(P, e, p0, cs2);
   const double T = eos_temperature<EOS>(P, e);
@@ -499,7 +499,7 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
     theta += (u[fs + c + 1] - u[fs + c - 1]) * (0.5 * P.inv_dx) + (u[2 * fs + c + P.NXp] - u[2 * fs + c - P.NXp]) * (0.5 * P.inv_dy);
     if (P.NZp > 1) theta += (u[3 * fs + c + P.plane] - u[3 * fs + c - P.plane]) * (0.5 * P.inv_dz);
     v[8] = 0.0; v[9] = 0.0;
-    if constexpr (MILNE) {
+    {
       if (P.shear || P.bulk) {       // Eq. 90: velocity gradients as in the source terms (:424), kinematics of App. A
         const double uc[4] = {ut, ux, uy, un};
         double dt[4], dx[4], dy[4], dn[4];
@@ -512,9 +512,9 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
           dn[a] = (P.NZp > 1) ? (ua[P.plane] - ua[-P.plane]) * (0.5 * P.inv_dz) : 0.0;
         }
         Kin K;
-        kinematics(uc, dt, dx, dy, dn, t, K);
+        kinematics<MILNE>(uc, dt, dx, dy, dn, t, K);
         double r2s, r2b;
-        second_order_reynolds<EOS>(P, t, uc, K, pi, Pi, ee, r2s, r2b);
+        second_order_reynolds<EOS, MILNE>(P, t, uc, K, pi, Pi, ee, r2s, r2b);
         v[8] = (P.shear && isfinite(r2s)) ? r2s : 0.0;
         v[9] = (P.bulk && isfinite(r2b)) ? r2b : 0.0;
       }

@@ -229,10 +229,11 @@ __device__ __forceinline__ void conservation_sources2(const DevParams& P, const 
 
 // ------------------------------------------------------------------------------------------------ dissipative sources
 // J = S + G for pi^{mu nu} (10) and Pi (B.10-B.12, Eqs. 39-46), one component at a time: emit(slot, J).
-template <int EOS, class Emit>
+template <int EOS, bool MILNE, class Emit>
 __device__ __forceinline__ void dissipative_sources2(const DevParams& P, double t, const double u[4], const Kin& K, const double pi[10], double Pi,
                                                      double e, double divv, Emit emit) {
-  const double t2 = t * t, it = rcp_fast(t);
+  const double t2 = MILNE ? t * t : 1.0;                                       // metric factor
+  const double it = MILNE ? rcp_fast(t) : 0.0, ct = MILNE ? t : 0.0;           // Christoffel symbols (0 in the Cartesian mode, R12)
   // transport coefficients (Eqs. 10-16; R14)
   double p, cs2;
   eos_p_cs2<EOS>(P, e, p, cs2);
@@ -270,8 +271,7 @@ __device__ __forceinline__ void dissipative_sources2(const DevParams& P, double 
       gS[0][n] = S[sym(0, n)]; gS[1][n] = -S[sym(1, n)]; gS[2][n] = -S[sym(2, n)]; gS[3][n] = -t2 * S[sym(3, n)];
     }
   }
-  const double it2 = it * it;
-  const double gi[4] = {1.0, -1.0, -1.0, -it2};
+  const double gi[4] = {1.0, -1.0, -1.0, MILNE ? -it * it : -1.0};
   const double third_pisig = (1.0 / 3.0) * pisig;
 #pragma unroll
   for (int m = 0; m < 4; ++m)
@@ -293,10 +293,10 @@ __device__ __forceinline__ void dissipative_sources2(const DevParams& P, double 
       double Ipi = I1 + P.delta_pipi * K.theta * pi[s] - kVorticitySign * B + P.tau_pipi * I4 - P.lambda_piPi * Pi * S[s];
       // G_pi = u^a Gamma^mu_{ab} pi^{b nu} + (mu<->nu)  (:300; R1, R2)
       double G = 0.0;
-      if (s == 0) G = 2.0 * t * un * pi[3];
-      if (s == 1) G = t * un * pi[6];
-      if (s == 2) G = t * un * pi[8];
-      if (s == 3) G = t * un * pi[9] + (ut * pi[3] + un * pi[0]) * it;
+      if (s == 0) G = 2.0 * ct * un * pi[3];
+      if (s == 1) G = ct * un * pi[6];
+      if (s == 2) G = ct * un * pi[8];
+      if (s == 3) G = ct * un * pi[9] + (ut * pi[3] + un * pi[0]) * it;
       if (s == 6) G = (ut * pi[6] + un * pi[1]) * it;
       if (s == 8) G = (ut * pi[8] + un * pi[2]) * it;
       if (s == 9) G = 2.0 * (ut * pi[9] + un * pi[3]) * it;
@@ -350,13 +350,13 @@ __global__ void __launch_bounds__(BX* BY* BZ, MINB) stage_kernel(const __grid_co
     }
     if (VISC) {
       Kin K;
-      kinematics(uc, du[0], du[1], du[2], du[3], t, K);
+      kinematics<MILNE>(uc, du[0], du[1], du[2], du[3], t, K);
       double pi[10];
 #pragma unroll
       for (int n = 0; n < 10; ++n) pi[n] = A.q_in[(PTT + n) * fs + c];
       const double Pi = A.q_in[BPI * fs + c];
       const double ec = A.e_in[c];
-      dissipative_sources2<EOS>(P, t, uc, K, pi, Pi, ec, divv, [&](int slot, double J) {
+      dissipative_sources2<EOS, MILNE>(P, t, uc, K, pi, Pi, ec, divv, [&](int slot, double J) {
         const bool on = (slot == BPI) ? (P.bulk != 0) : (P.shear != 0);
         double v = fma(P.dtau, J, park[slot][tid]);
         if (STAGE == 2) v = 0.5 * (A.q_n[slot * fs + c] + v);      // Eq. 70

@@ -124,11 +124,12 @@ __device__ __forceinline__ void face_coefficients(double vm_lo, double vp_lo, do
 // c_pi pi^{mn} + c_S sigma^{mn} goes to the cell's park slot at once; (3) sigma, W are transformed IN PLACE into the 16
 // entries of Y^{ln} (pair (l,n), l < n: Y^{ln} = g_l (b sigma + a W), Y^{nl} = g_n (b sigma - a W)); (4) the contraction with
 // pi is added to the parked value.  pi(s) reads the cell's pi component from shared memory; ld/st access the park slot.
-template <int EOS, class PiGet, class ParkLd, class ParkSt>
+template <int EOS, bool MILNE, class PiGet, class ParkLd, class ParkSt>
 __device__ __forceinline__ void relaxation_sources4(const DevParams& P, double t, const double (&u)[4], const double (&du)[4][4], PiGet pi,
                                                     double Pi, double e, double divv, double dt, ParkLd ld, ParkSt st) {
   const double ut = u[0], ux = u[1], uy = u[2], un = u[3];
-  const double t2 = t * t, it = rcp_fast(t), it2 = it * it;
+  // Cartesian mode (R12): metric factors tau^2 -> 1 (t2, it2), Christoffel symbols -> 0 (it = Gamma^eta_{eta tau}, ct = Gamma^tau_{eta eta})
+  const double t2 = MILNE ? t * t : 1.0, it = MILNE ? rcp_fast(t) : 0.0, it2 = MILNE ? it * it : 1.0, ct = MILNE ? t : 0.0;
   const double* dT = du[0]; const double* dX = du[1]; const double* dY = du[2]; const double* dN = du[3];
   // convective derivatives (A.5-A.8), expansion rate (A.11), covariant acceleration (A.9-A.10)
   const double dut = ut * dT[0] + ux * dX[0] + uy * dY[0] + un * dN[0];
@@ -138,22 +139,22 @@ __device__ __forceinline__ void relaxation_sources4(const DevParams& P, double t
   const double th = ut * it + dT[0] + dX[1] + dY[2] + dN[3];
   const double th3 = th * (1.0 / 3.0);
   const double un2 = un * un;
-  const double Du0 = dut + t * un2, Du1 = -dux, Du2 = -duy, Du3 = -t2 * dun - 2.0 * t * ut * un;
+  const double Du0 = dut + ct * un2, Du1 = -dux, Du2 = -duy, Du3 = -t2 * (dun + 2.0 * it * ut * un);
   // Z[0..9] = sigma^{mu nu} (A.12; slot order tt tx ty tn xx xy xn yy yn nn), Z[10..15] = W^{tx} W^{ty} W^{tn} W^{xy} W^{xn} W^{yn}
   double Z[16];
-  Z[0] = -t * ut * un2 + dT[0] - ut * dut + (ut * ut - 1.0) * th3;
-  Z[1] = -0.5 * t * un2 * ux + 0.5 * (dT[1] - dX[0]) - 0.5 * (ut * dux + ux * dut) + ut * ux * th3;
-  Z[2] = -0.5 * t * un2 * uy + 0.5 * (dT[2] - dY[0]) - 0.5 * (ut * duy + uy * dut) + ut * uy * th3;
-  Z[3] = -0.5 * un * it * (2.0 * ut * ut + t2 * un2) + 0.5 * (dT[3] - dN[0] * it2) - 0.5 * (ut * dun + un * dut) + ut * un * th3;
+  Z[0] = -ct * ut * un2 + dT[0] - ut * dut + (ut * ut - 1.0) * th3;
+  Z[1] = -0.5 * ct * un2 * ux + 0.5 * (dT[1] - dX[0]) - 0.5 * (ut * dux + ux * dut) + ut * ux * th3;
+  Z[2] = -0.5 * ct * un2 * uy + 0.5 * (dT[2] - dY[0]) - 0.5 * (ut * duy + uy * dut) + ut * uy * th3;
+  Z[3] = -0.5 * un * (2.0 * it * ut * ut + ct * un2) + 0.5 * (dT[3] - dN[0] * it2) - 0.5 * (ut * dun + un * dut) + ut * un * th3;
   Z[4] = -dX[1] - ux * dux + (1.0 + ux * ux) * th3;
   Z[5] = -0.5 * (dX[2] + dY[1]) - 0.5 * (ux * duy + uy * dux) + ux * uy * th3;
   Z[6] = -ut * ux * un * it - 0.5 * (dX[3] + dN[1] * it2) - 0.5 * (ux * dun + un * dux) + ux * un * th3;
   Z[7] = -dY[2] - uy * duy + (1.0 + uy * uy) * th3;
   Z[8] = -ut * uy * un * it - 0.5 * (dY[3] + dN[2] * it2) - 0.5 * (uy * dun + un * duy) + uy * un * th3;
   Z[9] = -ut * it2 * it * (1.0 + 2.0 * un2 * t2) - dN[3] * it2 - un * dun + (it2 + un2) * th3;
-  Z[10] = 0.5 * (dT[1] + dX[0]) + 0.5 * (ux * dut - ut * dux) + 0.5 * t * un2 * ux;
-  Z[11] = 0.5 * (dT[2] + dY[0]) + 0.5 * (uy * dut - ut * duy) + 0.5 * t * un2 * uy;
-  Z[12] = un * it + 0.5 * dT[3] + 0.5 * dN[0] * it2 + 0.5 * (un * dut - ut * dun) - ut * ut * un * it + 0.5 * t * un2 * un;
+  Z[10] = 0.5 * (dT[1] + dX[0]) + 0.5 * (ux * dut - ut * dux) + 0.5 * ct * un2 * ux;
+  Z[11] = 0.5 * (dT[2] + dY[0]) + 0.5 * (uy * dut - ut * duy) + 0.5 * ct * un2 * uy;
+  Z[12] = un * it + 0.5 * dT[3] + 0.5 * dN[0] * it2 + 0.5 * (un * dut - ut * dun) - ut * ut * un * it + 0.5 * ct * un2 * un;
   Z[13] = 0.5 * (dY[1] - dX[2]) + 0.5 * (uy * dux - ux * duy);
   Z[14] = 0.5 * dN[1] * it2 - 0.5 * dX[3] + 0.5 * (un * dux - ux * dun) - ux * ut * un * it;
   Z[15] = 0.5 * dN[2] * it2 - 0.5 * dY[3] + 0.5 * (un * duy - uy * dun) - uy * ut * un * it;
@@ -213,7 +214,7 @@ __device__ __forceinline__ void relaxation_sources4(const DevParams& P, double t
   }
   const double k3 = 2.0 * w * beta;
   const double gi[4] = {1.0, -1.0, -1.0, -it2};
-  const double g1 = w * t * un, g2 = w * ut * it, g3 = w * un * it;      // Christoffel weights of G_pi (:300; R1, R2)
+  const double g1 = w * ct * un, g2 = w * ut * it, g3 = w * un * it;      // Christoffel weights of G_pi (:300; R1, R2)
 #pragma unroll
   for (int m = 0; m < 4; ++m)
 #pragma unroll
@@ -431,7 +432,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     mbar_wait(&full[NSTAGE], 0u);
     const double* mine = cen + tid;
     double* mypark = park + tid;
-    relaxation_sources4<EOS>(P, t, uc, du, [&](int s) { return mine[s * NT]; }, mine[10 * NT], ec, divv, dt,
+    relaxation_sources4<EOS, MILNE>(P, t, uc, du, [&](int s) { return mine[s * NT]; }, mine[10 * NT], ec, divv, dt,
                              [&](int slot) { return mypark[slot * NT]; }, [&](int slot, double J) { mypark[slot * NT] = J; });
   }
 

@@ -5,7 +5,7 @@
 using namespace vh;
 
 #ifndef VH_COMBO
-#error "compile with -DVH_COMBO=0..8"
+#error "compile with -DVH_COMBO=0..11"
 #endif
 #define debug_sync vh_debug_sync
 
@@ -98,7 +98,8 @@ static cudaError_t launch_tile_d(vh_handle* h, int stage, const StageArgs& A, cu
 #define VH_CAT(a, b) VH_CAT2(a, b)
 cudaError_t VH_CAT(vh_launch_stage_combo, VH_COMBO)(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
   constexpr int EOS = VH_COMBO % 3;
-  constexpr bool VISC = (VH_COMBO / 3) == 0, MILNE = (VH_COMBO / 3) != 2;
+  constexpr int G = VH_COMBO / 3;      // 0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian, 3: viscous Cartesian
+  constexpr bool VISC = (G == 0) || (G == 3), MILNE = (G < 2);
   if (h->variant == 0) return launch_tile_d<EOS, VISC, MILNE>(h, stage, A, mid);
   if (h->variant == 2) return launch_split_d<EOS, VISC, MILNE>(h, stage, A, mid);
   return launch_stage_d<EOS, VISC, MILNE>(h, stage, A);

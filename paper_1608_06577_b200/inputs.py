@@ -112,6 +112,33 @@ def config_shocktube(n=200, axis=0, theta=1.8, cfl=0.5, length=10.0, T_L=0.4, T_
     return prm, dict(e=e, u=rest_velocity(shp), pi=None, Pi=None), 100, x
 
 
+def config_diagonal_shocktube(n=101, d=0.1, cfl=0.25, theta=1.0, e_hi=0.0246, e_lo=0.0015):
+    """PAPER.md 5.2 (:696-704): the Sod membrane of section 5.1 placed along the main diagonal y = x of the transverse grid; energy
+    densities of :634 in GeV/fm^3, p = e/3, ideal, Cartesian.  High side: y > x.  Returns the coordinate x' = (x - y)/sqrt2 normal
+    to the membrane as the last item."""
+    prm = base_params(nx=n, ny=n, nz=1, dx=d, dy=d, dz=d, tau0=0.0, dtau=cfl * d, geometry=1, physics=0, eos=0, zeta_model=0,
+                      minmod_theta=theta, tau_relax_floor_over_dtau=0.0)
+    x = centred_axis(n, d)
+    X, Y = np.meshgrid(x, x, indexing="xy")            # [y, x]
+    xn = (X - Y) / math.sqrt(2.0)
+    shp = (1, 1, n, n)
+    e = np.where(xn < -1e-12, e_hi / HBARC, e_lo / HBARC).reshape(shp)
+    return prm, dict(e=e, u=rest_velocity(shp), pi=None, Pi=None), xn
+
+
+def config_blast(n=101, d=0.1, cfl=0.25, theta=1.0, radius=1.0, e_in=0.0246, e_out=0.0015):
+    """PAPER.md 5.3 (:706-718): cylindrical explosion - e = 0.0246 GeV/fm^3 inside r <= R = 1 fm, 0.0015 GeV/fm^3 outside, in a
+    10 x 10 fm^2 box, p = e/3, ideal, Cartesian.  Returns r(x, y) as the last item."""
+    prm = base_params(nx=n, ny=n, nz=1, dx=d, dy=d, dz=d, tau0=0.0, dtau=cfl * d, geometry=1, physics=0, eos=0, zeta_model=0,
+                      minmod_theta=theta, tau_relax_floor_over_dtau=0.0)
+    x = centred_axis(n, d)
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    r = np.sqrt(X * X + Y * Y)
+    shp = (1, 1, n, n)
+    e = np.where(r <= radius, e_in / HBARC, e_out / HBARC).reshape(shp)
+    return prm, dict(e=e, u=rest_velocity(shp), pi=None, Pi=None), r
+
+
 # ------------------------------------------------------------------ config 2: Gubser flow (PAPER.md :757-779)
 def gubser_ode(eta_over_s, c_tau_pi, T0hat=1.2, rho_lo=-12.0, rho_hi=6.0):
     """Conformal Israel-Stewart under Gubser symmetry (tau_pipi = 0), with pibar = pihat^eta_eta/(ehat+phat):

@@ -277,7 +277,7 @@ def test_error_codes_and_status(vh):
     with pytest.raises(vh.VHError):
         vh.Solver(bad)
     with pytest.raises(vh.VHError):
-        vh.Solver(inputs.base_params(nx=4, ny=4, nz=4, geometry=1, physics=3))
+        vh.Solver(inputs.base_params(nx=4, ny=4, nz=4, geometry=2))
     with pytest.raises(vh.VHError):
         vh.Solver(inputs.base_params(nx=4, ny=4, nz=4, minmod_theta=2.5))
     s = vh.Solver(inputs.base_params(nx=4, ny=4, nz=4))

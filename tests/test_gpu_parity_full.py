@@ -144,3 +144,55 @@ def test_config2_gubser_as_written(vh, vo, n_steps, tol):
     s.close()
     assert o.status()["n_inversion_failures"] == 0
     assert_parity(o.get_fields(with_uprev=True), o.status(), fg, sg, tol=tol)
+
+
+def _run_pair(vh, vo, prm, st, n_steps, variant=0, uprev=None):
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], st.get("pi"), st.get("Pi"))
+    if uprev is not None:
+        o.set_uprev(uprev)
+    o.step(n_steps)
+    s = vh.Solver(prm)
+    s.set_kernel_variant(variant)
+    s.set_initial(_t(st["e"]), _t(st["u"]), _t(st.get("pi")), _t(st.get("Pi")))
+    if uprev is not None:
+        s.set_uprev(_t(uprev))
+    s.step(n_steps)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields(with_uprev=True).items()}
+    sg = s.status()
+    s.close()
+    return o.get_fields(with_uprev=True), o.status(), fg, sg
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_viscous_cartesian_generic_state(vh, vo, variant):
+    # geometry = 1 with shear and bulk on (Christoffel symbols off, tau^2 -> 1; oracle pinned by the damped sound wave of
+    # tests/test_oracle_cartesian.py) on the all-terms state, 3+1d with ragged tiles, and in 2+1d
+    prm = inputs.base_params(nx=36, ny=12, nz=6, dx=0.12, dy=0.1, dz=0.15, tau0=0.8, dtau=0.02, geometry=1)
+    st = inputs.smooth_random_state(prm, seed=23)
+    up = st["u"] * 1.0
+    up[1:] *= 0.98
+    up[0] = np.sqrt(1 + up[1] ** 2 + up[2] ** 2 + up[3] ** 2)
+    fo, so, fg, sg = _run_pair(vh, vo, prm, st, 10, variant, uprev=up)
+    assert np.max(np.abs(fo["q"][13])) > 0 and np.max(np.abs(fo["q"][14])) > 0 and np.max(np.abs(fo["u"][3])) > 0
+    assert_parity(fo, so, fg, sg)
+    prm2 = inputs.base_params(nx=40, ny=20, nz=1, tau0=0.8, dtau=0.02, geometry=1, minmod_theta=1.5)
+    st2 = inputs.smooth_random_state(prm2, seed=29)
+    assert_parity(*_run_pair(vh, vo, prm2, st2, 10, variant))
+
+
+def test_diagonal_shock_tube_and_blast(vh, vo):
+    # PAPER.md 5.2-5.3 (:696-718): the 2+1d Cartesian ideal test problems, 10 steps to 1e-9 and the full runs (100 / 80 steps) to 1e-6;
+    # the GPU result keeps the mirror symmetries of the problems to rounding
+    prm, init, _ = inputs.config_diagonal_shocktube()
+    assert_parity(*_run_pair(vh, vo, prm, init, 10))
+    fo, so, fg, sg = _run_pair(vh, vo, prm, init, 100)
+    assert_parity(fo, so, fg, sg, tol=1e-6)
+    e = fg["e"][0, 0]
+    assert np.max(np.abs(e - e[::-1, ::-1].T)) <= 1e-11 * np.max(e)
+    prm, init, _ = inputs.config_blast()
+    assert_parity(*_run_pair(vh, vo, prm, init, 10))
+    fo, so, fg, sg = _run_pair(vh, vo, prm, init, 80)
+    assert_parity(fo, so, fg, sg, tol=1e-6)
+    e = fg["e"][0, 0]
+    assert np.max(np.abs(e - e.T)) <= 1e-11 * np.max(e) and np.max(np.abs(e - e[:, ::-1])) <= 1e-11 * np.max(e)
