@@ -55,6 +55,8 @@ def lib():
         L = C.CDLL(so)
         L.vho_create.restype = C.c_void_p
         L.vho_create.argtypes = [C.POINTER(Params)]
+        L.vho_create_f32.restype = C.c_void_p
+        L.vho_create_f32.argtypes = [C.POINTER(Params)]
         L.vho_destroy.argtypes = [C.c_void_p]
         dp = C.POINTER(C.c_double)
         L.vho_set_initial.argtypes = [C.c_void_p, dp, dp, dp, dp]
@@ -97,11 +99,13 @@ WHICH = {"q": 0, "qS": 1, "Q": 2, "u": 3, "up": 4, "uS": 5, "e": 6, "p": 7}
 class Oracle:
     """One oracle run.  Arrays: physical cells only, shape [..., n_batch, nz, ny, nx] (x fastest)."""
 
-    def __init__(self, params: dict):
+    def __init__(self, params: dict, precision="f64"):
+        """precision "f32": the same algorithm with a float scalar (set_initial / set_uprev / step / get_fields / status only)."""
         self.L = lib()
         self.d = dict(params)
         self.P = make_params(params)
-        self.h = self.L.vho_create(C.byref(self.P))
+        self.precision = precision
+        self.h = (self.L.vho_create_f32 if precision == "f32" else self.L.vho_create)(C.byref(self.P))
         if not self.h:
             raise ValueError("vho_create rejected the parameters")
         self.shape = (self.P.n_batch, self.P.nz, self.P.ny, self.P.nx)

@@ -5,13 +5,14 @@
 #include <cstring>
 
 using Sol = vho::Solver<double>;
+using SolF = vho::Solver<float>;      // the same algorithm in single precision: comparator of the FP32 build
 
 extern "C" {
 
 int vho_params_size() { return (int)sizeof(vho::Params); }
 
-// one Solver per event of the batch
-struct vho_handle { vho::Params P; std::vector<Sol*> ev; };
+// one Solver per event of the batch (ev: double precision; evf: single precision, created by vho_create_f32 - then ev is empty)
+struct vho_handle { vho::Params P; std::vector<Sol*> ev; std::vector<SolF*> evf; };
 
 vho_handle* vho_create(const vho::Params* P) {
   if (!P || P->nx < 1 || P->ny < 1 || P->nz < 1 || P->n_batch < 1) return nullptr;
@@ -20,52 +21,76 @@ vho_handle* vho_create(const vho::Params* P) {
   for (int b = 0; b < P->n_batch; ++b) h->ev.push_back(new Sol(*P));
   return h;
 }
-void vho_destroy(vho_handle* h) { if (!h) return; for (Sol* s : h->ev) delete s; delete h; }
+vho_handle* vho_create_f32(const vho::Params* P) {
+  if (!P || P->nx < 1 || P->ny < 1 || P->nz < 1 || P->n_batch < 1) return nullptr;
+  vho_handle* h = new vho_handle;
+  h->P = *P;
+  for (int b = 0; b < P->n_batch; ++b) h->evf.push_back(new SolF(*P));
+  return h;
+}
+void vho_destroy(vho_handle* h) { if (!h) return; for (Sol* s : h->ev) delete s; for (SolF* s : h->evf) delete s; delete h; }
 
-// arrays: physical cells only, x fastest, then y, eta, batch; component-major SoA per array (u4: [4][batch][cells])
-int vho_set_initial(vho_handle* h, const double* e, const double* u4, const double* pi10, const double* Pi) {
-  size_t np = (size_t)h->P.nx * h->P.ny * h->P.nz, nb = h->ev.size();
+}  // extern "C"
+
+// the calls both precisions support, written once over the vector of solvers
+template <class S> static void set_initial_t(const vho::Params& P, std::vector<S*>& ev, const double* e, const double* u4, const double* pi10, const double* Pi) {
+  size_t np = (size_t)P.nx * P.ny * P.nz, nb = ev.size();
   std::vector<double> ub(4 * np), pb(10 * np);
   for (size_t b = 0; b < nb; ++b) {
     for (int m = 0; m < 4; ++m) std::memcpy(&ub[m * np], u4 + (m * nb + b) * np, np * sizeof(double));
     if (pi10) for (int n = 0; n < 10; ++n) std::memcpy(&pb[n * np], pi10 + (n * nb + b) * np, np * sizeof(double));
-    h->ev[b]->set_initial(e + b * np, ub.data(), pi10 ? pb.data() : nullptr, Pi ? Pi + b * np : nullptr);
+    ev[b]->set_initial(e + b * np, ub.data(), pi10 ? pb.data() : nullptr, Pi ? Pi + b * np : nullptr);
   }
-  return 0;
 }
-int vho_set_uprev(vho_handle* h, const double* up4) {
-  size_t np = (size_t)h->P.nx * h->P.ny * h->P.nz, nb = h->ev.size();
+template <class S> static void set_uprev_t(const vho::Params& P, std::vector<S*>& ev, const double* up4) {
+  size_t np = (size_t)P.nx * P.ny * P.nz, nb = ev.size();
   std::vector<double> ub(4 * np);
   for (size_t b = 0; b < nb; ++b) {
     for (int m = 0; m < 4; ++m) std::memcpy(&ub[m * np], up4 + (m * nb + b) * np, np * sizeof(double));
-    h->ev[b]->set_uprev(ub.data());
+    ev[b]->set_uprev(ub.data());
   }
-  return 0;
 }
-int vho_step(vho_handle* h, int n) {
-  for (int it = 0; it < n; ++it) for (Sol* s : h->ev) s->step();
-  return 0;
-}
-int vho_get_fields(vho_handle* h, double* q15, double* e, double* p, double* u4, double* up4) {
-  size_t np = (size_t)h->P.nx * h->P.ny * h->P.nz, nb = h->ev.size();
+template <class S> static void get_fields_t(const vho::Params& P, std::vector<S*>& ev, double* q15, double* e, double* p, double* u4, double* up4) {
+  size_t np = (size_t)P.nx * P.ny * P.nz, nb = ev.size();
   std::vector<double> qb(15 * np), ub(4 * np), upb(4 * np);
   for (size_t b = 0; b < nb; ++b) {
-    h->ev[b]->get_fields(q15 ? qb.data() : nullptr, e ? e + b * np : nullptr, p ? p + b * np : nullptr,
-                         u4 ? ub.data() : nullptr, up4 ? upb.data() : nullptr);
+    ev[b]->get_fields(q15 ? qb.data() : nullptr, e ? e + b * np : nullptr, p ? p + b * np : nullptr,
+                      u4 ? ub.data() : nullptr, up4 ? upb.data() : nullptr);
     if (q15) for (int n = 0; n < 15; ++n) std::memcpy(q15 + (n * nb + b) * np, &qb[n * np], np * sizeof(double));
     if (u4) for (int m = 0; m < 4; ++m) std::memcpy(u4 + (m * nb + b) * np, &ub[m * np], np * sizeof(double));
     if (up4) for (int m = 0; m < 4; ++m) std::memcpy(up4 + (m * nb + b) * np, &upb[m * np], np * sizeof(double));
   }
-  return 0;
 }
-int vho_get_status(vho_handle* h, double* tau, long long* n_steps, long long* n_fail, long long* n_nonfinite, double* min_reg) {
+template <class S> static void get_status_t(std::vector<S*>& ev, double* tau, long long* n_steps, long long* n_fail, long long* n_nonfinite, double* min_reg) {
   long long f = 0, nf = 0; double mr = 1.0;
-  for (Sol* s : h->ev) { f += s->n_fail; nf += s->n_nonfinite; if (s->min_reg_factor < mr) mr = s->min_reg_factor; }
-  if (tau) *tau = h->ev[0]->tau;
-  if (n_steps) *n_steps = h->ev[0]->n_steps;
+  for (S* s : ev) { f += s->n_fail; nf += s->n_nonfinite; if (s->min_reg_factor < mr) mr = s->min_reg_factor; }
+  if (tau) *tau = ev[0]->tau;
+  if (n_steps) *n_steps = ev[0]->n_steps;
   if (n_fail) *n_fail = f;
   if (n_nonfinite) *n_nonfinite = nf;
   if (min_reg) *min_reg = mr;
+}
+
+extern "C" {
+// arrays: physical cells only, x fastest, then y, eta, batch; component-major SoA per array (u4: [4][batch][cells]); always double
+int vho_set_initial(vho_handle* h, const double* e, const double* u4, const double* pi10, const double* Pi) {
+  if (h->evf.empty()) set_initial_t(h->P, h->ev, e, u4, pi10, Pi); else set_initial_t(h->P, h->evf, e, u4, pi10, Pi);
+  return 0;
+}
+int vho_set_uprev(vho_handle* h, const double* up4) {
+  if (h->evf.empty()) set_uprev_t(h->P, h->ev, up4); else set_uprev_t(h->P, h->evf, up4);
+  return 0;
+}
+int vho_step(vho_handle* h, int n) {
+  for (int it = 0; it < n; ++it) { for (Sol* s : h->ev) s->step(); for (SolF* s : h->evf) s->step(); }
+  return 0;
+}
+int vho_get_fields(vho_handle* h, double* q15, double* e, double* p, double* u4, double* up4) {
+  if (h->evf.empty()) get_fields_t(h->P, h->ev, q15, e, p, u4, up4); else get_fields_t(h->P, h->evf, q15, e, p, u4, up4);
+  return 0;
+}
+int vho_get_status(vho_handle* h, double* tau, long long* n_steps, long long* n_fail, long long* n_nonfinite, double* min_reg) {
+  if (h->evf.empty()) get_status_t(h->ev, tau, n_steps, n_fail, n_nonfinite, min_reg); else get_status_t(h->evf, tau, n_steps, n_fail, n_nonfinite, min_reg);
   return 0;
 }
 

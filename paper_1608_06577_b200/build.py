@@ -3,7 +3,8 @@
     python -m paper_1608_06577_b200.build [--force] [--verbose]
 
 vh_api.cu and twelve launch units (vh_launch.cu compiled with -DVH_COMBO=0..11, one per EOS / viscous / Milne combination) are
-compiled in parallel to objects under csrc/build/ and linked into libvh.so.  The built .so is git-ignored but travels with the
+compiled in parallel to objects under csrc/build/<precision>/ and linked into libvh.so (real = double) and libvh_f32.so
+(real = float, -DVH_REAL=float; `--f64` / `--f32` build only one of them).  The built .so is git-ignored but travels with the
 source tree; nothing is JIT-compiled at import time."""
 import os
 import subprocess
@@ -14,8 +15,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 SO = os.path.join(HERE, "libvh.so")
+# real = double: libvh.so (the product, everything BASELINE.json measures); real = float: libvh_f32.so
+LIBS = {"f64": (SO, []), "f32": (os.path.join(HERE, "libvh_f32.so"), ["-DVH_REAL=float"])}
 N_COMBO = 12
-HEADERS = ["vh_device.cuh", "vh_math.cuh", "vh_kernels.cuh", "vh_kernels2.cuh", "vh_kernels3.cuh", "vh_kernels4.cuh", "vh_internal.cuh", "vh_eos_lattice.hpp",
+HEADERS = ["vh_real.cuh", "vh_peaks.cuh", "vh_device.cuh", "vh_math.cuh", "vh_kernels.cuh", "vh_kernels2.cuh", "vh_kernels3.cuh", "vh_kernels4.cuh", "vh_internal.cuh", "vh_eos_lattice.hpp",
            os.path.join("..", "..", "include", "vh.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
@@ -28,38 +31,45 @@ def units():
     return out
 
 
-def up_to_date() -> bool:
-    if not os.path.exists(SO):
+def up_to_date(so) -> bool:
+    if not os.path.exists(so):
         return False
-    t = os.path.getmtime(SO)
+    t = os.path.getmtime(so)
     deps = [os.path.join(CSRC, f) for f in ["vh_api.cu", "vh_launch.cu"] + HEADERS] + [os.path.abspath(__file__)]
     return all(os.path.getmtime(d) <= t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and up_to_date():
+def build(force: bool = False, verbose: bool = False, precisions=("f64", "f32")) -> str:
+    """Builds the library of every requested precision that is out of date; returns the path of libvh.so."""
+    todo = [p for p in precisions if force or not up_to_date(LIBS[p][0])]
+    if not todo:
         return SO
     nvcc = os.environ.get("NVCC", "nvcc")
-    os.makedirs(OBJ, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
+    jobs = []
+    for p in todo:
+        os.makedirs(os.path.join(OBJ, p), exist_ok=True)
+        for src, obj, flags in units():
+            jobs.append((p, src, os.path.join(OBJ, p, obj), flags + LIBS[p][1]))
 
-    def compile_one(u):
-        src, obj, flags = u
-        cmd = [nvcc] + NVCC_FLAGS + extra + flags + ["-c", "-o", os.path.join(OBJ, obj), os.path.join(CSRC, src)]
-        r = subprocess.run(cmd, capture_output=True, text=True)
-        return u, r
+    def compile_one(j):
+        p, src, obj, flags = j
+        cmd = [nvcc] + NVCC_FLAGS + extra + flags + ["-c", "-o", obj, os.path.join(CSRC, src)]
+        return j, subprocess.run(cmd, capture_output=True, text=True)
 
-    with ThreadPoolExecutor(max_workers=min(len(units()), os.cpu_count() or 1)) as ex:
-        results = list(ex.map(compile_one, units()))
-    for (src, obj, flags), r in results:
+    with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1)) as ex:
+        results = list(ex.map(compile_one, jobs))
+    for (p, src, obj, flags), r in results:
         if verbose or r.returncode != 0:
             sys.stderr.write("---- %s %s\n%s%s" % (src, " ".join(flags), r.stdout, r.stderr))
         if r.returncode != 0:
             raise RuntimeError("nvcc failed on %s %s" % (src, " ".join(flags)))
-    cmd = [nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", SO] + [os.path.join(OBJ, u[1]) for u in units()]
-    subprocess.check_call(cmd)
+    for p in todo:
+        objs = [os.path.join(OBJ, p, u[1]) for u in units()]
+        subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIBS[p][0]] + objs)
     return SO
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    only = [p for p in LIBS if "--" + p in sys.argv]
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, precisions=tuple(only) or tuple(LIBS)))

@@ -1,6 +1,7 @@
 // vh_api.cu -- C ABI (include/vh.h): handle, buffers, buffer rotation (PAPER.md program-flow steps 7, 9), kernel dispatch.
 #include "vh_internal.cuh"
 #include "vh_eos_lattice.hpp"
+#include "vh_peaks.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -10,6 +11,7 @@
 #include <limits>
 #include <new>
 #include <string>
+#include <vector>
 
 using namespace vh;
 
@@ -46,7 +48,7 @@ static int fill_dev_params(const vh_params& p, DevParams& P) {
   std::memset(&P, 0, sizeof(P));
   P.nx = p.nx; P.ny = p.ny; P.nz = p.nz; P.n_batch = p.n_batch;
   const bool two_d = (p.nz == 1);
-  P.NXp = (int)round_up(p.nx + 4, 16);
+  P.NXp = (int)round_up(p.nx + XOFF + 2, 16);      // XOFF cells before the first physical cell, two ghost cells after the last
   P.NYp = p.ny + 4;
   P.NZp = two_d ? 1 : p.nz + 4;
   P.zoff = two_d ? 0 : 2;
@@ -89,6 +91,7 @@ static int check_params(const vh_params* p, std::string& why) {
   if (!(p->minmod_theta >= 1.0 && p->minmod_theta <= 2.0)) { why = "minmod_theta must lie in [1,2] (Eq. 67)"; return -1; }
   if (!(p->rho_max > 0 && p->xi0 > 0)) { why = "xi0, rho_max must be > 0"; return -1; }
   if (p->newton_max_iter < 1 || !(p->newton_rtol > 0)) { why = "newton_max_iter >= 1 and newton_rtol > 0 required"; return -1; }
+  if (kF32 && p->newton_rtol < 1e-6) { why = "the single-precision library needs newton_rtol >= 1e-6 (a tighter stopping rule cannot be met in FP32)"; return -1; }
   if ((long long)p->nz * p->n_batch > 65535) { why = "nz*n_batch exceeds the grid z limit (65535)"; return -1; }
   return 0;
 }
@@ -126,36 +129,40 @@ static int make_tensor_maps(vh_handle* h, int n_arrays) {
   EncodeTiledFn encode = (EncodeTiledFn)fn;
   const DevParams& P = h->P;
   const cuuint64_t dims[5] = {(cuuint64_t)P.NXp, (cuuint64_t)P.NYp, (cuuint64_t)P.NZp, (cuuint64_t)P.n_batch, (cuuint64_t)n_arrays};
-  const cuuint64_t strides[4] = {(cuuint64_t)P.NXp * 8, (cuuint64_t)P.plane * 8, (cuuint64_t)P.bstride * 8, (cuuint64_t)P.fstride * 8};
+  const cuuint64_t R = sizeof(real);
+  const cuuint64_t strides[4] = {(cuuint64_t)P.NXp * R, (cuuint64_t)P.plane * R, (cuuint64_t)P.bstride * R, (cuuint64_t)P.fstride * R};
+  const CUtensorMapDataType dtype = kF32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+  // L2 promotion no wider than a box row (32 or 36 elements: 256 / 288 bytes in double, 128 / 144 bytes in single precision)
+  const CUtensorMapL2promotion promo = kF32 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
   const cuuint32_t ones[5] = {1, 1, 1, 1, 1};
   const bool td = h->two_d;
   const cuuint32_t boxA[5] = {(cuuint32_t)(td ? Tile<true>::AX : Tile<false>::AX), (cuuint32_t)(td ? Tile<true>::AY : Tile<false>::AY),
                               (cuuint32_t)(td ? Tile<true>::TZ : Tile<false>::TZ), 1, 1};
   const cuuint32_t boxZ[5] = {(cuuint32_t)Tile<false>::TX, (cuuint32_t)Tile<false>::TY, 2, 1, 1};
-  CUresult r = encode(&h->mapA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                      CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  CUresult r = encode(&h->mapA, dtype, 5, h->pool, dims, strides, boxA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                      CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box A) failed with CUresult " + std::to_string((int)r));
-  r = encode(&h->mapZ, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  r = encode(&h->mapZ, dtype, 5, h->pool, dims, strides, boxZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box Z) failed with CUresult " + std::to_string((int)r));
   const cuuint32_t boxC[5] = {(cuuint32_t)Tile<false>::TX, (cuuint32_t)(td ? Tile<true>::TY : Tile<false>::TY),
                               (cuuint32_t)(td ? Tile<true>::TZ : Tile<false>::TZ), 1, 1};
-  r = encode(&h->mapC, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxC, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  r = encode(&h->mapC, dtype, 5, h->pool, dims, strides, boxC, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box C) failed with CUresult " + std::to_string((int)r));
   const cuuint32_t boxVA[5] = {(cuuint32_t)(td ? VTile<true>::AX : VTile<false>::AX), (cuuint32_t)(td ? VTile<true>::AY : VTile<false>::AY),
                                (cuuint32_t)(td ? VTile<true>::VZ : VTile<false>::VZ), 1, 1};
-  r = encode(&h->mapVA, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxVA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  r = encode(&h->mapVA, dtype, 5, h->pool, dims, strides, boxVA, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box VA) failed with CUresult " + std::to_string((int)r));
   const cuuint32_t boxVZ[5] = {(cuuint32_t)VTile<false>::VX, (cuuint32_t)VTile<false>::VY, 1, 1, 1};
-  r = encode(&h->mapVZ, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, h->pool, dims, strides, boxVZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  r = encode(&h->mapVZ, dtype, 5, h->pool, dims, strides, boxVZ, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(h, VH_ERR_CUDA, "cuTensorMapEncodeTiled(box VZ) failed with CUresult " + std::to_string((int)r));
   return VH_OK;
 }
 
-static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, double* u) {
+static cudaError_t launch_ghost(vh_handle* h, real* q, real* e, real* p, real* u) {
   const DevParams& P = h->P;
   long long W = h->two_d ? (long long)P.ny + P.nx : (long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny;
   dim3 grid((unsigned)((W + 255) / 256), 21, P.n_batch);
@@ -168,13 +175,13 @@ static cudaError_t launch_ghost(vh_handle* h, double* q, double* e, double* p, d
 
 static cudaError_t reset_regulation_map(vh_handle* h) {
   if (!h->regfac) return cudaSuccess;
-  fill_kernel<<<1024, 256, 0, h->stream>>>(h->regfac, h->P.fstride, 1.0);
+  fill_kernel<<<1024, 256, 0, h->stream>>>(h->regfac, h->P.fstride, real(1.0));
   h->launches++;
   return cudaGetLastError();
 }
 
 template <int EOS>
-static void launch_diag(vh_handle* h, double t, double* maps) {
+static void launch_diag(vh_handle* h, real t, double* maps) {
   const DevParams& P = h->P;
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const unsigned nb = (unsigned)std::min<long long>((np + 255) / 256, 2048LL);      // grid-stride loop
@@ -211,12 +218,12 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   h->stream = (cudaStream_t)cuda_stream;
   cudaGetDevice(&h->device);
   const long long fs = h->P.fstride;
-  const size_t bytes = (size_t)67 * fs * sizeof(double);
+  const size_t bytes = (size_t)67 * fs * sizeof(real);
   ce = cudaMalloc((void**)&h->pool, bytes);
   if (ce != cudaSuccess) { cudaGetLastError(); delete h; return fail(nullptr, VH_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes: " + cudaGetErrorString(ce)); }
   ce = cudaMalloc((void**)&h->cnt, sizeof(Counters));
   if (ce != cudaSuccess) { cudaGetLastError(); cudaFree(h->pool); delete h; return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc(counters) failed"); }
-  double* w = h->pool;
+  real* w = h->pool;
   for (int i = 0; i < 3; ++i) { h->q[i] = w; w += 15 * fs; }
   for (int i = 0; i < 3; ++i) { h->u[i] = w; w += 4 * fs; }
   for (int i = 0; i < 2; ++i) { h->e[i] = w; w += fs; }
@@ -232,15 +239,16 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   }
   if (p->eos == 2) {      // lattice EOS: build the table on the host (milliseconds), keep it in global memory
     const vh_eos::LatticeTable tab = vh_eos::Builder().build();
-    const size_t tb = tab.node.size() * sizeof(double);
+    const std::vector<real> nodes(tab.node.begin(), tab.node.end());      // the table in the library's precision
+    const size_t tb = nodes.size() * sizeof(real);
     ce = cudaMalloc((void**)&h->eos_tab, tb);
-    if (ce == cudaSuccess) ce = cudaMemcpyAsync(h->eos_tab, tab.node.data(), tb, cudaMemcpyHostToDevice, h->stream);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(h->eos_tab, nodes.data(), tb, cudaMemcpyHostToDevice, h->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);      // tab lives on this stack frame
     if (ce != cudaSuccess) { cudaGetLastError(); cudaFree(h->eos_tab); cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_ALLOC, "EOS table upload failed"); }
     const int n = vh_eos::VH_EOS_N;
     const double* nd = tab.node.data();
     const double e0 = std::pow(tab.x0, 4), eN = std::pow(tab.xN, 4);
-    h->P.eos_tab = reinterpret_cast<const double2*>(h->eos_tab);
+    h->P.eos_tab = reinterpret_cast<const real2*>(h->eos_tab);
     h->P.eos_n = n; h->P.eos_x0 = tab.x0; h->P.eos_xN = tab.xN; h->P.eos_inv_h = 1.0 / tab.h;
     h->P.eos_lo_slope = nd[0] / e0; h->P.eos_pN = nd[4 * n]; h->P.eos_eN = eN;
     h->P.eos_T0_over_x0 = nd[2] / tab.x0; h->P.eos_TN_over_xN = nd[4 * n + 2] / tab.xN;
@@ -329,7 +337,7 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
   const DevParams& P = h->P;
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const unsigned nb = (unsigned)((np + 255) / 256);
-  struct Item { const double* src; double* dst; int nc; };
+  struct Item { const double* src; real* dst; int nc; };
   Item items[4] = {{q15, h->q[0], 15}, {e, h->e[0], 1}, {u4, h->u[0], 4}, {u4_prev, h->u[1], 4}};
   if (mem_space == 0) {
     int rc = ensure_stage(h, &h->stage_in, &h->stage_in_bytes, (size_t)16 * np * sizeof(double));
@@ -414,8 +422,8 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   }
   if (ev) CUDA_TRY(h, cudaEventRecord(ev[4], h->stream));
   // steps 7, 9: rotate.  u: (u^n, u^{n-1}, u*) <- (u^{n+1}, u^n, scratch); q: q^n <-> q^{n+1}
-  double* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;
-  double* qn = h->q[2]; h->q[2] = h->q[0]; h->q[0] = qn;
+  real* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;
+  real* qn = h->q[2]; h->q[2] = h->q[0]; h->q[0] = qn;
   h->n_steps++;
   return VH_OK;
 }
@@ -459,7 +467,7 @@ int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, d
   const DevParams& P = h->P;
   const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
   const unsigned nb = (unsigned)((np + 255) / 256);
-  struct Item { double* dst; double* src; int nc; };
+  struct Item { double* dst; real* src; int nc; };
   Item items[5] = {{q15, h->q[0], 15}, {e, h->e[0], 1}, {p, h->p[0], 1}, {u4, h->u[0], 4}, {u4_prev, h->u[1], 4}};
   if (mem_space == 0) {
     int rc = ensure_stage(h, &h->stage_out, &h->stage_out_bytes, (size_t)15 * np * sizeof(double));
@@ -552,7 +560,7 @@ int vh_enable_regulation_map(vh_handle* h, int on) {
     return VH_OK;
   }
   if (!h->regfac) {
-    if (cudaMalloc((void**)&h->regfac, (size_t)h->P.fstride * sizeof(double)) != cudaSuccess) {
+    if (cudaMalloc((void**)&h->regfac, (size_t)h->P.fstride * sizeof(real)) != cudaSuccess) {
       cudaGetLastError();
       h->regfac = nullptr;
       return fail(h, VH_ERR_ALLOC, "cudaMalloc(regulation map) failed");

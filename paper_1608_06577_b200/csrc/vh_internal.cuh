@@ -19,17 +19,17 @@ struct vh_handle {
   cudaStream_t stream = nullptr;
   int device = 0;                    // the device the handle was created on (its buffers, tensor maps and kernel attributes belong to it)
   std::vector<const void*> smem_opted_in;   // kernels whose dynamic shared-memory limit was raised on `device` for this handle
-  double* pool = nullptr;            // 67 padded arrays
-  double* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
-  double* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
-  double* e[2] = {nullptr, nullptr};            // e^n / e^{n+1}, e*
-  double* p[2] = {nullptr, nullptr};
-  double* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
-  double* vR = nullptr;              // [3] ... high face
+  vh::real* pool = nullptr;          // 67 padded arrays (real = the library's precision: double in libvh.so, float in libvh_f32.so)
+  vh::real* q[3] = {nullptr, nullptr, nullptr};   // q^n, q*, q^{n+1}   (:470 q, qS, Q)
+  vh::real* u[3] = {nullptr, nullptr, nullptr};   // u^n, u^{n-1}, u*   (:470 u, up, uS)
+  vh::real* e[2] = {nullptr, nullptr};            // e^n / e^{n+1}, e*
+  vh::real* p[2] = {nullptr, nullptr};
+  vh::real* vL = nullptr;              // [3] velocity of the reconstructed state at each cell's low face, per direction
+  vh::real* vR = nullptr;              // [3] ... high face
   vh::Counters* cnt = nullptr;
   unsigned long long* diag = nullptr;   // [10] maxima of vh_get_diagnostics (bit patterns)
-  double* eos_tab = nullptr;         // EOS 2: the lattice table (vh_eos_lattice.hpp) in global memory
-  double* regfac = nullptr;          // one padded array: tanh(rho)/rho applied by the last step's final regularisation (vh_enable_regulation_map), else null
+  vh::real* eos_tab = nullptr;         // EOS 2: the lattice table (vh_eos_lattice.hpp) in global memory
+  vh::real* regfac = nullptr;          // one padded array: tanh(rho)/rho applied by the last step's final regularisation (vh_enable_regulation_map), else null
   double* stage_in = nullptr;  size_t stage_in_bytes = 0;     // device staging for host-side set_initial
   double* stage_out = nullptr; size_t stage_out_bytes = 0;    // device staging for host-side get_fields
   long long n_steps = 0;

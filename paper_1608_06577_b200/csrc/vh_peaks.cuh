@@ -1,0 +1,26 @@
+// vh_peaks.cuh -- the two peak microbenchmarks behind vh_measure_peaks (always FP64: they measure the roofline denominators).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace vh {
+
+// ------------------------------------------------------------------------------------------------ peak microbenchmarks
+static __global__ void __launch_bounds__(256) copy_kernel(const double2* __restrict__ src, double2* __restrict__ dst, long long n2) {
+  long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < n2; w += stride) dst[w] = src[w];
+}
+
+static __global__ void __launch_bounds__(256) fma_kernel(double* out, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+  if (s == 123.456) out[0] = s;     // never true; keeps the chain alive
+}
+
+}  // namespace vh

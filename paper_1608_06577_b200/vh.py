@@ -7,6 +7,8 @@ import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(HERE, "libvh.so")
+# the same sources compiled with real = float (the paper ran single precision): same C ABI, caller arrays stay double
+LIBS = {"f64": SO, "f32": os.path.join(HERE, "libvh_f32.so")}
 
 VH_OK = 0
 
@@ -36,14 +38,17 @@ EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_st
 _lib = None
 
 
-def load_library():
-    """dlopen libvh.so and declare the prototypes.  Works without a GPU (no CUDA call is made)."""
+def load_library(precision="f64"):
+    """dlopen libvh.so (precision "f64") or libvh_f32.so ("f32") and declare the prototypes.  Works without a GPU (no CUDA call is made)."""
     global _lib
-    if _lib is not None:
-        return _lib
-    if not os.path.exists(SO):
-        raise RuntimeError("CUDA extension %s is missing: run `python -m paper_1608_06577_b200.build` (there is no CPU fallback)" % SO)
-    L = C.CDLL(SO)
+    if _lib is None:
+        _lib = {}
+    if precision in _lib:
+        return _lib[precision]
+    so = LIBS[precision]
+    if not os.path.exists(so):
+        raise RuntimeError("CUDA extension %s is missing: run `python -m paper_1608_06577_b200.build` (there is no CPU fallback)" % so)
+    L = C.CDLL(so)
     vp = C.c_void_p
     for name in EXPORTS:
         getattr(L, name).restype = C.c_int
@@ -69,7 +74,7 @@ def load_library():
     L.vh_last_error.restype = C.c_char_p
     L.vh_destroy.argtypes = [vp]
     L.vh_destroy.restype = None
-    _lib = L
+    _lib[precision] = L
     return L
 
 
@@ -98,11 +103,12 @@ class Solver:
     Arrays are torch tensors (float64) of shape [..., n_batch, nz, ny, nx]: CUDA tensors are passed as device pointers
     (mem_space 1), CPU tensors as host pointers (mem_space 0; the library does the copies on its stream)."""
 
-    def __init__(self, params: dict, device="cuda:0", stream=None):
+    def __init__(self, params: dict, device="cuda:0", stream=None, precision="f64"):
         import torch
 
         self.torch = torch
-        self.L = load_library()
+        self.precision = precision
+        self.L = load_library(precision)
         if not torch.cuda.is_available():
             raise VHError("no CUDA device available (there is no CPU fallback)")
         self.device = torch.device(device)
