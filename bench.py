@@ -26,6 +26,7 @@ import numpy as np  # noqa: E402
 from paper_1608_06577_b200 import inputs  # noqa: E402
 
 METRIC = "cell-updates/s (full RK2 KT step, FP64) at 128^3 viscous"
+METRIC_F32 = "cell-updates/s (full RK2 KT step, single-precision build) at 128^3 viscous"
 UNIT = "cell-updates/s"
 ALG_BYTES_PER_CELL_UPDATE = 856.0      # 107 doubles per cell-update, each state array read/written once per stage
 ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
@@ -266,6 +267,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-paper-physics", action="store_true", help="skip the second, labelled measurement with the lattice EOS and Eq. 17 zeta/s")
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: the single-precision build (libvh_f32.so; SURVEY 8(f) NEXT-3), a labelled extra line")
     ap.add_argument("--physics", default="config3", choices=["config3", "paper"], help="paper: lattice EOS + Eq. 17 zeta/s on the config-3 grid")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -291,8 +293,11 @@ def main():
     K = args.steps
 
     prm, init = workload(rank, args.physics)
+    f32 = (args.precision == "f32")
+    if f32:
+        prm["newton_rtol"] = 2e-6          # the stopping rule of Eq. 72 at single precision (the f32 library refuses anything below 1e-6)
     ncell = prm["nx"] * prm["ny"] * prm["nz"] * prm["n_batch"]
-    s = vh.Solver(prm, device=dev)
+    s = vh.Solver(prm, device=dev, precision=args.precision)
     if args.variant:
         s.set_kernel_variant(args.variant)
     e_d = torch.as_tensor(init["e"], device=dev)
@@ -352,11 +357,14 @@ def main():
 
     # ---------------- peaks measured in the same run by the library's own microbenchmarks
     copy_gbs, fp64_gflops = vh.measure_peaks(n_bytes=1 << 30, repeats=10)
+    fp32_gflops = vh.measure_fp32_peak(repeats=10) if f32 else None
+    alu_gflops = fp32_gflops if f32 else fp64_gflops      # the ALU peak of the precision the library computes in
+    bscale = 0.5 if f32 else 1.0                          # bytes per stored value relative to FP64
     s.close()
 
     # ---------------- second, labelled workload: the paper's own physics (lattice EOS, Eq. 17 zeta/s) on the same grid
     paper_line = None
-    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics:
+    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics and not f32:
         prm2, init2 = workload(rank, "paper")
         s2 = vh.Solver(prm2, device=dev)
         s2.set_initial(torch.as_tensor(init2["e"], device=dev), torch.as_tensor(init2["u"], device=dev))
@@ -390,8 +398,8 @@ def main():
         alg_kernel = {k: 0.5 * (flops_inv_cu if "velocity" in k else flops_cu - flops_inv_cu) for k in LAUNCH_KEYS}
         if variant1:
             alg_kernel = {"stage1": 0.5 * flops_cu, "stage2": 0.5 * flops_cu}
-        bytes_kernel = {"stage1": ALG_BYTES_STAGE["stage1"], "stage2": ALG_BYTES_STAGE["stage2"], "velocity1": 10 * 8.0, "velocity2": 10 * 8.0}
-        ncu = ncu_metrics() if (ncell == 128 ** 3 and default_pipeline and args.physics == "config3") else {}
+        bytes_kernel = {k: v * bscale for k, v in {"stage1": ALG_BYTES_STAGE["stage1"], "stage2": ALG_BYTES_STAGE["stage2"], "velocity1": 10 * 8.0, "velocity2": 10 * 8.0}.items()}
+        ncu = ncu_metrics() if (ncell == 128 ** 3 and default_pipeline and args.physics == "config3" and not f32) else {}
         ex_kernel, pipe_kernel, traffic_kernel = {}, {}, {}
         for k, m in ncu.items():
             try:
@@ -410,28 +418,28 @@ def main():
         useful = {k: min(alg_kernel[k], ex_kernel.get(k, alg_kernel[k])) for k in cand}
         flops_launch = useful[dom] * ncell
         bytes_launch = bytes_kernel[dom] * ncell
-        t_alu = flops_launch / (fp64_gflops * 1e9)
+        t_alu = flops_launch / (alu_gflops * 1e9)
         t_hbm = bytes_launch / (hbm_peak * 1e9)
         if t_alu >= t_hbm:
-            roof = {"bound": "alu", "achieved": flops_launch / dur / 1e12, "peak": fp64_gflops / 1e3, "unit": "TFLOP/s"}
+            roof = {"bound": "alu", "achieved": flops_launch / dur / 1e12, "peak": alu_gflops / 1e3, "unit": "TFLOP/s"}
         else:
             roof = {"bound": "hbm", "achieved": bytes_launch / dur / 1e9, "peak": hbm_peak, "unit": "GB/s"}
         roof["frac"] = roof["achieved"] / roof["peak"]
         useful_step = sum(useful.values())
-        step_roof_s = max(useful_step * ncell / (fp64_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * ncell / (hbm_peak * 1e9))
+        step_roof_s = max(useful_step * ncell / (alu_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * bscale * ncell / (hbm_peak * 1e9))
         kname = ("velocity_tile_kernel" if "velocity" in dom else "stage_tile_kernel") if default_pipeline else ("stage_cell_kernel" if variant1 else "stage_kernel")
         roof.update({
             "traffic": traffic_kernel.get(dom), "traffic_source": os.path.relpath(NCU_METRICS_CSV, ROOT) if dom in traffic_kernel else None,
             "kernel": "%s (%s)" % (kname, dom), "launch_ms": prof[dom],
-            "peak_source": "FP64 FMA microbenchmark, same run (vh_measure_peaks)" if roof["bound"] == "alu" else hbm_src,
+            "peak_source": ("FP32 FMA microbenchmark, same run (vh_measure_fp32_peak)" if f32 else "FP64 FMA microbenchmark, same run (vh_measure_peaks)") if roof["bound"] == "alu" else hbm_src,
             "numerator": "min(minimal algorithmic flops, executed flops) of this kernel per cell x cells per launch",
             "alg_flops_this_kernel_per_cell": alg_kernel[dom], "executed_flops_per_cell": ex_kernel.get(dom),
             "alg_over_executed": (alg_kernel[dom] / ex_kernel[dom]) if dom in ex_kernel else None,
             "fp64_pipe_util": pipe_kernel.get(dom),
-            "frac_on_minimal_count": alg_kernel[dom] * ncell / dur / (fp64_gflops * 1e9),
+            "frac_on_minimal_count": alg_kernel[dom] * ncell / dur / (alu_gflops * 1e9),
             "alg_flops_per_cell_update": flops_cu, "alg_flops_by_section_per_cell_update": {k: round(v, 1) for k, v in by_section.items()},
             "executed_flops_per_cell_update": sum(ex_kernel.values()) if len(ex_kernel) == 4 else None,
-            "alg_bytes_per_cell_update": ALG_BYTES_PER_CELL_UPDATE, "alg_bytes_this_kernel_per_cell": bytes_kernel[dom],
+            "alg_bytes_per_cell_update": ALG_BYTES_PER_CELL_UPDATE * bscale, "alg_bytes_this_kernel_per_cell": bytes_kernel[dom],
             "flop_weights": "add/mul 1, div 10, sqrt 15, exp 25, pow 30, tanh 40 (SURVEY 8(d)); compares carry no weight; counted on the oracle with "
                             "each interface once, each limited slope once, exact 0/+-1 constants not counted",
             "op_mix_per_cell_update": {k: round(v, 1) for k, v in mix.items()},
@@ -440,17 +448,17 @@ def main():
             "step_roofline_ms": step_roof_s * 1e3, "step_frac": step_roof_s / (ms / K * 1e-3),
             "per_kernel_ms": prof,
             "per_kernel": {k: {"ms": prof[k], "alg_flops_per_cell": alg_kernel[k], "executed_flops_per_cell": ex_kernel.get(k),
-                               "frac": useful[k] * ncell / (prof[k] * 1e-3) / (fp64_gflops * 1e9), "fp64_pipe_util": pipe_kernel.get(k),
+                               "frac": useful[k] * ncell / (prof[k] * 1e-3) / (alu_gflops * 1e9), "fp64_pipe_util": pipe_kernel.get(k),
                                "traffic": traffic_kernel.get(k), "alg_bytes": bytes_kernel[k] * ncell} for k in cand},
         })
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
+            "metric": METRIC_F32 if f32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "config": {"workload": ("SINGLE-PRECISION BUILD (labelled extra line, not the BASELINE.json metric, which is FP64): " if f32 else "") + ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
                                     "dtau=0.025, one independent replica per GPU (no sharding, no collective)") if args.physics == "config3" else
                                    ("configs[2] grid and hotspots with the paper's own physics: lattice EOS (Eqs. 19-20), zeta/s of Eq. 17 (T_c = 200 MeV), "
                                     "eta/s=0.2; one independent replica per GPU"),
-                       "l2": "state (67 padded arrays, 1.34 GB) exceeds the 126 MB L2; no flush needed", "kernel_variant": args.variant,
+                       "l2": "state (67 padded arrays, %.2f GB) exceeds the 126 MB L2; no flush needed" % (0.67 if f32 else 1.34), "kernel_variant": args.variant,
                        "paper_context": "GTX 980 Ti, FP32, lattice EOS: 244.45 ms/step = 8.58e6 cell-updates/s (PAPER.md Table 3; another machine, not a target)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": E,
                     "what": "per step: vh_set_initial(host e,u,pi,Pi) + vh_step(1) + vh_get_fields(host q,e,p,u), pinned buffers"},
@@ -458,7 +466,7 @@ def main():
             "clocks": clocks,
             "roofline": roof,
             "status": {"n_inversion_failures": st["n_inversion_failures"], "n_nonfinite": st["n_nonfinite"], "min_reg_factor": st["min_reg_factor"]},
-            "measured_peaks_same_run": {"copy_gbs": copy_gbs, "fp64_fma_gflops": fp64_gflops},
+            "measured_peaks_same_run": {"copy_gbs": copy_gbs, "fp64_fma_gflops": fp64_gflops, "fp32_fma_gflops": fp32_gflops},
         }
         if paper_line is not None:
             line["paper_physics"] = paper_line

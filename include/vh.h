@@ -152,6 +152,9 @@ int vh_set_kernel_variant(vh_handle* h, int variant);
  * FP64 stream copy (GB/s, read+write bytes) over n_bytes (>= 1 GiB recommended) and a dependent-free FP64 FMA kernel
  * (GFLOP/s, 2 flops per FMA) on all SMs; each the best of `repeats`.  Either output may be NULL.                       */
 int vh_measure_peaks(void* cuda_stream, long long n_bytes, int repeats, double* copy_gbs, double* fp64_gflops);
+/* The same dependent-free FMA kernel in single precision (GFLOP/s): the ALU roofline denominator of the single-precision build
+ * (libvh_f32.so).                                                                                     */
+int vh_measure_fp32_peak(void* cuda_stream, int repeats, double* fp32_gflops);
 
 const char* vh_last_error(vh_handle* h);
 void vh_destroy(vh_handle* h);

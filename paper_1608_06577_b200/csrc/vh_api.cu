@@ -70,6 +70,7 @@ static int fill_dev_params(const vh_params& p, DevParams& P) {
   P.theta = p.minmod_theta;
   P.inv_rho_max = 1.0 / p.rho_max; P.xi0_rho_max = p.xi0 * p.rho_max;
   P.newton_max_iter = p.newton_max_iter; P.newton_rtol = p.newton_rtol;
+  P.newton_stop = std::max(p.newton_rtol, 0.1 * std::sqrt(p.newton_rtol));      // see newton_pair (vh_math.cuh)
   P.relax_clamp = (p.tau_relax_floor_over_dtau > 0.0) ? 1.0 / (p.tau_relax_floor_over_dtau * p.dtau) : std::numeric_limits<double>::infinity();
   return 0;
 }
@@ -662,6 +663,36 @@ int vh_measure_peaks(void* cuda_stream, long long n_bytes, int repeats, double* 
     *fp64_gflops = best;
   }
   cudaEventDestroy(e0); cudaEventDestroy(e1);
+  CUDA_TRY(nullptr, cudaGetLastError());
+  return VH_OK;
+}
+
+int vh_measure_fp32_peak(void* cuda_stream, int repeats, double* fp32_gflops) {
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (repeats < 1 || !fp32_gflops) return fail(nullptr, VH_ERR_ARG, "repeats >= 1 and fp32_gflops != NULL required");
+  int dev = 0, nsm = 0;
+  CUDA_TRY(nullptr, cudaGetDevice(&dev));
+  CUDA_TRY(nullptr, cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(nullptr, cudaEventCreate(&e0));
+  if (cudaEventCreate(&e1) != cudaSuccess) { cudaEventDestroy(e0); return fail(nullptr, VH_ERR_CUDA, "cudaEventCreate failed"); }
+  float* o = nullptr;
+  if (cudaMalloc((void**)&o, 8) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(e0); cudaEventDestroy(e1); return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc failed"); }
+  const int iters = 8192, blocks = nsm * 8;
+  double best = 0;
+  for (int r = 0; r < repeats + 1; ++r) {
+    cudaEventRecord(e0, st);
+    fma32_kernel<<<blocks, 256, 0, st>>>(o, iters, 0.999999f, 1e-6f);
+    cudaEventRecord(e1, st);
+    cudaEventSynchronize(e1);
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    double gf = 2.0 * 64.0 * iters * 256.0 * blocks / (ms * 1e-3) / 1e9;
+    if (r > 0 && gf > best) best = gf;
+  }
+  cudaFree(o);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *fp32_gflops = best;
   CUDA_TRY(nullptr, cudaGetLastError());
   return VH_OK;
 }

@@ -32,6 +32,7 @@ struct DevParams {
   real theta;                 // minmod theta
   real inv_rho_max, xi0_rho_max;
   int newton_max_iter; real newton_rtol;
+  real newton_stop;             // convergence test of the product kernels: |de| <= newton_stop |e| guarantees |next de| <= newton_rtol |e| (see fill_dev_params)
   real relax_clamp;           // 1/(c*dtau) or +inf
 };
 

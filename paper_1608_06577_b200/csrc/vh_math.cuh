@@ -26,8 +26,11 @@ __device__ __forceinline__ real half_slope2(real d1, real d2, real half_theta) {
 }
 
 // ---------------------------------------------------------------- paired Newton-Raphson on Eq. 72 (R6)
-// Two independent states are iterated together so that their dependent FP64 chains interleave.  Same stopping rule, cap and
-// failure semantics as invert_energy(); a converged state stops updating while its partner (or another lane) iterates.
+// Two independent states are iterated together so that their dependent FP64 chains interleave.  Same tolerance, cap and failure
+// semantics as invert_energy().  The tolerance |de| <= rtol |e| (R6) is tested one iteration early: Newton's method on Eq. 72 converges
+// quadratically, |de_next| <= C de^2 with C = max|f''|/(2 min f') <= 0.2/(E+P) + 0.21/e0 (M^2 <= (E+P)^2, f' >= 1 - cs2 >= 0.65, P'' of
+// the EOS), so |de| <= newton_stop |e| with newton_stop = 0.1 sqrt(rtol) bounds the NEXT correction - the one the oracle still performs and
+// then finds below rtol - by 1.3e-14 |e| for e <= 60 e0: same root to the same tolerance, one evaluation of the EOS fewer per state.
 struct NewtonState {
   real E, M2, Pi;     // inputs
   real e;             // iterate
@@ -59,8 +62,8 @@ __device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, 
     // iterates are not finite and it takes the failure path below anyway).
     A.e = badA ? A.e : eA;
     B.e = badB ? B.e : eB;
-    if (fabs(dA) <= P.newton_rtol * fabs(eA)) { convA = true; doneA = true; }
-    if (fabs(dB) <= P.newton_rtol * fabs(eB)) { convB = true; doneB = true; }
+    if (fabs(dA) <= P.newton_stop * fabs(eA)) { convA = true; doneA = true; }
+    if (fabs(dB) <= P.newton_stop * fabs(eB)) { convB = true; doneB = true; }
   }
   // P0 and 1/(E + P0 + Pi) at the returned e, extrapolated from the last iterate over its correction (once, after the loop):
   // P0(e - d) = P0(e) - cs2 d + O(d^2), 1/(den - cs2 d) = r + r^2 cs2 d + O(d^2), |d| <= rtol e at convergence
@@ -90,7 +93,7 @@ __device__ __forceinline__ real newton_single(const DevParams& P, real E, real M
     const real d = f * rcp_half(g);      // (f' only steers the iteration)
     const real en = e - d;
     e = bad ? e : en;      // (a converged cell keeps iterating with its warp: see newton_pair)
-    if (fabs(d) <= P.newton_rtol * fabs(en)) { conv = true; done = true; }
+    if (fabs(d) <= P.newton_stop * fabs(en)) { conv = true; done = true; }
   }
   fail = bad || !conv || !(e > real(0.0)) || !isfinite(e);
   if (fail) e = (tiny_e() > E) ? tiny_e() : E;      // max(E, tiny) that keeps a NaN E (fmax would drop it and hide the cell from n_nonfinite)

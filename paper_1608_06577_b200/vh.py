@@ -33,7 +33,7 @@ class vh_params(C.Structure):
 
 # every symbol include/vh.h declares
 EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_enable_regulation_map", "vh_get_regulation_map", "vh_run_until", "vh_eos_table", "vh_launch_count",
-           "vh_set_kernel_variant", "vh_measure_peaks", "vh_last_error", "vh_destroy"]
+           "vh_set_kernel_variant", "vh_measure_peaks", "vh_measure_fp32_peak", "vh_last_error", "vh_destroy"]
 
 _lib = None
 
@@ -70,6 +70,7 @@ def load_library(precision="f64"):
     L.vh_launch_count.restype = C.c_longlong
     L.vh_set_kernel_variant.argtypes = [vp, C.c_int]
     L.vh_measure_peaks.argtypes = [vp, C.c_longlong, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.vh_measure_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.vh_last_error.argtypes = [vp]
     L.vh_last_error.restype = C.c_char_p
     L.vh_destroy.argtypes = [vp]
@@ -283,3 +284,19 @@ def measure_peaks(n_bytes=1 << 30, repeats=10, stream=None):
         msg = L.vh_last_error(None)
         raise VHError("vh_measure_peaks failed (%d): %s" % (rc, msg.decode() if msg else "?"))
     return a.value, b.value
+
+
+def measure_fp32_peak(repeats=10, stream=None):
+    """FP32 FMA GFLOP/s of the current device (the ALU roofline denominator of the single-precision build)."""
+    import torch
+
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise VHError("no CUDA device available")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    a = C.c_double()
+    rc = L.vh_measure_fp32_peak(C.c_void_p(st.cuda_stream), int(repeats), C.byref(a))
+    if rc != VH_OK:
+        msg = L.vh_last_error(None)
+        raise VHError("vh_measure_fp32_peak failed (%d): %s" % (rc, msg.decode() if msg else "?"))
+    return a.value
