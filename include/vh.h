@@ -60,6 +60,9 @@ typedef struct {
   int newton_max_iter;              /* Newton-Raphson cap for Eq. 72 (reading R6: 50)                                   */
   double newton_rtol;               /* stop when |de| <= rtol*|e| (1e-13)                                               */
   double tau_relax_floor_over_dtau; /* c: 1/tau_Pi, 1/tau_pi <= 1/(c*dtau) (reading R14); 0 disables                    */
+  int storage;                      /* 0: all ten pi^{mu nu} and four u^mu are state (the paper's choice, :333); 1: reduced storage (:476,
+                                       Eqs. 47-51, reading R22): pi^xx, pi^xy, pi^xeta, pi^yy, pi^yeta and u^x, u^y, u^eta only - 43 instead
+                                       of 61 state arrays; a slower kernel of its own                                                    */
 } vh_params;
 
 /* Create a solver for the grid / physics in *p on the current CUDA device.  cuda_stream: a cudaStream_t (may be NULL =

@@ -16,10 +16,13 @@
 //     viscous Gubser flow, boosted-static exact solution, a generic covariant evaluation of Eq. 8, closed-form
 //     inversion, invariants).  The vorticity sign (R4) is pinned to the governing equation, Eq. 8, by
 //     tests/test_oracle_covariant.py (the appendix list A.25-A.29 has the opposite sign).  The regularisation
-//     (Eqs. 73-74, reading R9) is pinned only through hand-computed values of rho for simple states
-//     (tests/test_oracle_units.py): "parity unpinned" beyond that - no printed solution exercises rho >~ 1; applied literally it makes
+//     (Eqs. 73-74, reading R9) and the order invert -> regulate (R8) are pinned by tests/test_oracle_regulation.py: every entry of the
+//     max of Eq. 74 for a moving fluid at tau != 1 from states built out of Lorentz-invariant pieces, the equilibrium pressure in the
+//     first entry, and e, u returned from the un-regulated state; the rest-frame values by tests/test_oracle_units.py.  Applied literally it makes
 //     the discrete Gubser run ill-conditioned ("config 2").  The lattice EOS (eos = 2, vh_oracle_lattice.hpp,
-//     readings R19, R20) is pinned by tests/test_oracle_lattice.py, zeta/s of Eq. 17, diagnostics() (incl. Eq. 90, reading R21, also tests/test_oracle_covariant.py) and regulation_map() by tests/test_oracle_units.py.
+//     readings R19, R20) is pinned by tests/test_oracle_lattice.py, zeta/s of Eq. 17, diagnostics() (incl. Eq. 90, reading R21, also tests/test_oracle_covariant.py) and regulation_map() by tests/test_oracle_units.py.  The viscous Cartesian mode (geometry = 1 with physics != 0) is pinned by the damped
+//     sound wave of the linearised equations, the 2+1d diagonal shock tube and the cylindrical blast (tests/test_oracle_cartesian.py).  No function is "parity unpinned".
+//     Solver<float> (vho_create_f32) is the same code with a float scalar: comparator of the single-precision build, pinned against Solver<double> (tests/test_f32.py).
 //
 // The scalar type is a template parameter so that an operation-counting type can be
 // substituted (oracle/vh_oracle_capi.cpp instantiates double and a counting type).
@@ -62,6 +65,8 @@ struct Params {
   double xi0, rho_max;         // Eq. 74 (:445)
   int newton_max_iter; double newton_rtol;    // R6
   double tau_relax_floor_over_dtau;           // R14; 0 disables
+  int storage;                                // 0: all ten pi^{mu nu} and four u^mu are propagated (the paper's choice, :333); 1: reduced storage
+                                              //    (:476, Eqs. 47-51): only pi^xx, pi^xy, pi^xeta, pi^yy, pi^yeta and u^x, u^y, u^eta are state, reading R22
 };
 
 // field order of q (Eqs. 56-58 with the lost pi^{y eta} restored, R2):
@@ -219,6 +224,13 @@ template <class R> class Solver {
       for (int m = 0; m < 4; ++m) uu[m] = u_in[m * np + c];
       R pi[10];
       for (int n = 0; n < 10; ++n) pi[n] = (pi_in && (P.physics & 1)) ? R(pi_in[n * np + c]) : R(0);
+      if (reduced()) {     // the dependent components that were passed in are not state: replace them before T^{tau mu} is built
+        const R t2i = tau2(R(P.tau0));
+        uu[0] = sqrt(R(1) + uu[1] * uu[1] + uu[2] * uu[2] + t2i * uu[3] * uu[3]);
+        R v[3] = {uu[1] / uu[0], uu[2] / uu[0], uu[3] / uu[0]}, d[5];
+        dependent_pi(v, t2i, pi[4], pi[5], pi[6], pi[7], pi[8], d);
+        pi[0] = d[0]; pi[1] = d[1]; pi[2] = d[2]; pi[3] = d[3]; pi[9] = d[4];
+      }
       q[0][s] = (ee + Pt) * uu[0] * uu[0] - Pt + pi[0];                 // Eq. 32
       for (int m = 1; m < 4; ++m) q[m][s] = (ee + Pt) * uu[0] * uu[m] + pi[m];   // Eq. 33
       for (int n = 0; n < 10; ++n) q[4 + n][s] = pi[n];
@@ -319,6 +331,34 @@ template <class R> class Solver {
       double v[10];
       cell_diagnostics(idx(i, j, k), v);
       for (int m = 0; m < 10; ++m) maps[m * np + c] = v[m];
+    }
+  }
+
+  // ------------------------------------------------------------ reduced storage (PAPER.md:476 with Eqs. 47-51, :318-331; reading R22)
+  // "it can be reduced by simply propagating only the independent components of pi^{mu nu} (five) and u^mu (three), with the remaining
+  // components determined algebraically."  The five are the paper's example (:316): pi^xx, pi^xy, pi^xeta, pi^yy, pi^yeta.  In this mode the
+  // other five components and u^tau are NOT state: wherever the algorithm reads them (at any stencil cell) they are the algebraic values
+  // below, evaluated with the velocity of that cell; what the Euler step computes for them is discarded.
+  bool reduced() const { return P.storage == 1 && (P.physics & 1); }
+  // Eqs. 48-51 then 47 (Eq. 49 with its typo fixed, R3: the last term is tau^2 pi^{y eta} v_eta) from v^i = u^i/u^tau
+  void dependent_pi(const R v[3], R t2, R pxx, R pxy, R pxn, R pyy, R pyn, R out[5]) const {     // out: pi^tt, pi^tx, pi^ty, pi^tn, pi^nn
+    const R vx = v[0], vy = v[1], vn = v[2];
+    R pnn = (pxx * (vx * vx - R(1)) + pyy * (vy * vy - R(1)) + R(2) * pxy * vx * vy + R(2) * t2 * (pxn * vx * vn + pyn * vy * vn)) /
+            (t2 * (R(1) - t2 * vn * vn));                                        // Eq. 51
+    R ptx = pxx * vx + pxy * vy + t2 * pxn * vn;                                // Eq. 48
+    R pty = pxy * vx + pyy * vy + t2 * pyn * vn;                                // Eq. 49
+    R ptn = pxn * vx + pyn * vy + t2 * pnn * vn;                                // Eq. 50
+    R ptt = ptx * vx + pty * vy + t2 * ptn * vn;                                // Eq. 47
+    out[0] = ptt; out[1] = ptx; out[2] = pty; out[3] = ptn; out[4] = pnn;
+  }
+  // u^tau from u.u = 1 (:489) and the five dependent components, at every cell incl. ghosts (ghost cells are copies of q and u alike)
+  void expand_all(std::vector<R>* qq, std::vector<R>* uu, R t) {
+    const R t2 = tau2(t);
+    for (size_t s = 0; s < N; ++s) {
+      uu[0][s] = sqrt(R(1) + uu[1][s] * uu[1][s] + uu[2][s] * uu[2][s] + t2 * uu[3][s] * uu[3][s]);
+      R v[3] = {uu[1][s] / uu[0][s], uu[2][s] / uu[0][s], uu[3][s] / uu[0][s]}, d[5];
+      dependent_pi(v, t2, qq[8][s], qq[9][s], qq[10][s], qq[11][s], qq[12][s], d);
+      qq[4][s] = d[0]; qq[5][s] = d[1]; qq[6][s] = d[2]; qq[7][s] = d[3]; qq[13][s] = d[4];
     }
   }
 
@@ -578,9 +618,64 @@ template <class R> class Solver {
     return fac;
   }
 
-  void post(std::vector<R>* qq, std::vector<R>* uo, R t) {
+  // Reduced storage: pi^{tau mu} in E = T^{tau tau} - pi^{tau tau}, M_i = T^{tau i} - pi^{tau i} depend on the unknown velocity (Eqs. 47-50),
+  // so Eqs. 52-54 become implicit.  Reading R22: fixed point on v - start from the velocity of the same cell at the stage's input,
+  // v <- M(v)/(E(v) + P(e)) with e from Eq. 72 at every sweep (guess: previous sweep's e), until max_i |dv_i| <= newton_rtol (eta
+  // component in units of the others) or newton_max_iter sweeps (then a failure is counted).  Returns the converged dependent components.
+  void implicit_inversion(std::vector<R>* qq, size_t s, R t, const R vguess[3], R eguess, R& ee, R M[3], R& E, int& fail) {
+    const R t2 = tau2(t), rt = sqrt(t2);
+    R v[3] = {vguess[0], vguess[1], vguess[2]};
+    R d[5];
+    bool conv = false;
+    fail = 0;
+    ee = eguess;
+    for (int sweep = 0; sweep < P.newton_max_iter && !conv; ++sweep) {
+      dependent_pi(v, t2, qq[8][s], qq[9][s], qq[10][s], qq[11][s], qq[12][s], d);
+      E = qq[0][s] - d[0];
+      M[0] = qq[1][s] - d[1]; M[1] = qq[2][s] - d[2]; M[2] = qq[3][s] - d[3];
+      R M2 = M[0] * M[0] + M[1] * M[1] + t2 * M[2] * M[2];
+      int it, f1;
+      ee = invert_energy(P, E, M2, qq[14][s], ee, &it, &f1);
+      if (f1) { fail = 1; break; }
+      Thermo<R> th = eos(P, ee);
+      R den = E + th.p + qq[14][s];
+      R vn[3] = {M[0] / den, M[1] / den, M[2] / den};
+      R dv = maxr(maxr(absr(vn[0] - v[0]), absr(vn[1] - v[1])), rt * absr(vn[2] - v[2]));
+      v[0] = vn[0]; v[1] = vn[1]; v[2] = vn[2];
+      if (dv <= R(P.newton_rtol)) conv = true;
+    }
+    if (!conv) fail = 1;
+    // the state that is kept: dependent components of the converged velocity (and E, M consistent with them)
+    dependent_pi(v, t2, qq[8][s], qq[9][s], qq[10][s], qq[11][s], qq[12][s], d);
+    qq[4][s] = d[0]; qq[5][s] = d[1]; qq[6][s] = d[2]; qq[7][s] = d[3]; qq[13][s] = d[4];
+    E = qq[0][s] - d[0];
+    M[0] = qq[1][s] - d[1]; M[1] = qq[2][s] - d[2]; M[2] = qq[3][s] - d[3];
+  }
+
+  // ug: velocity of the stage's input (used only by the reduced-storage mode as the starting point of its fixed point)
+  void post(std::vector<R>* qq, std::vector<R>* uo, R t, const std::vector<R>* ug = nullptr) {
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i) {
       size_t s = idx(i, j, k);
+      if (reduced()) {
+        R vg[3] = {ug[1][s] / ug[0][s], ug[2][s] / ug[0][s], ug[3][s] / ug[0][s]};
+        R ee, M[3], E;
+        int fail;
+        implicit_inversion(qq, s, t, vg, e[s], ee, M, E, fail);
+        if (fail) ++n_fail;
+        R Pic = qq[14][s];
+        Thermo<R> th = eos(P, ee);
+        R Pt = th.p + Pic;
+        R ut = sqrt((E + Pt) / (ee + Pt));                              // Eq. 53
+        R uu[4] = {ut, M[0] / ((ee + Pt) * ut), M[1] / ((ee + Pt) * ut), M[2] / ((ee + Pt) * ut)};   // Eq. 54
+        e[s] = ee; p[s] = th.p;
+        for (int m = 1; m < 4; ++m) uo[m][s] = uu[m];
+        uo[0][s] = sqrt(R(1) + uu[1] * uu[1] + uu[2] * uu[2] + tau2(t) * uu[3] * uu[3]);      // u^tau is not state: always from u.u = 1
+        if (!(std::isfinite((double)ee) && std::isfinite((double)ut))) ++n_nonfinite;
+        R fac = regulate_cell(qq, s, ee, th.p, uu, t);                  // step 3 (:511): all ten components scale alike, so Eqs. 47-51 keep holding
+        if ((double)fac < min_reg_factor) min_reg_factor = (double)fac;
+        reg_factor[s] = (double)fac;
+        continue;
+      }
       R E = qq[0][s] - qq[4][s];
       R M[3] = {qq[1][s] - qq[5][s], qq[2][s] - qq[6][s], qq[3][s] - qq[7][s]};
       R M2 = M[0] * M[0] + M[1] * M[1] + tau2(t) * M[2] * M[2];
@@ -608,15 +703,16 @@ template <class R> class Solver {
   // ------------------------------------------------------------ one full RK step, program-flow steps 1-9 (:503-529)
   void step() {
     R t = tau, dt = P.dtau;
+    if (reduced()) expand_all(q, u, t);           // (reduced storage: the dependent components of the state are their algebraic values)
     euler(q, e, p, u, up, t, qS);                 // 1. q* = E[q^n; e,p,u^n,u^{n-1}] at tau^n
-    post(qS, uS, t + dt);                         // 2-4. e*,p*,u* ; regulate q* ; ghosts      (R7: tau^n + dtau)
+    post(qS, uS, t + dt, u);                      // 2-4. e*,p*,u* ; regulate q* ; ghosts      (R7: tau^n + dtau)
     euler(qS, e, p, uS, u, t + dt, Q);            // 5. q** = E[q*; e*,p*,u*,u^n] at tau^n + dtau
     for (int k = 2; k < NZ - 2; ++k) for (int j = 2; j < NY - 2; ++j) for (int i = 2; i < NX - 2; ++i) {
       size_t s = idx(i, j, k);
       for (int n = 0; n < NQ; ++n) Q[n][s] = (q[n][s] + Q[n][s]) / R(2);   // 6. convex combination
     }
     for (int m = 0; m < 4; ++m) up[m].swap(u[m]); // 7. up <-> u
-    post(Q, u, t + dt);                           // 8. e,p,u^{n+1}; regulate; ghosts
+    post(Q, u, t + dt, uS);                       // 8. e,p,u^{n+1}; regulate; ghosts
     for (int n = 0; n < NQ; ++n) q[n].swap(Q[n]); // 9. q <-> Q
     ++n_steps;
     tau = P.tau0 + (double)n_steps * P.dtau;      // :493  tau = tau_0 + n dtau

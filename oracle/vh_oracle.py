@@ -32,6 +32,7 @@ class Params(C.Structure):
         ("minmod_theta", C.c_double), ("xi0", C.c_double), ("rho_max", C.c_double),
         ("newton_max_iter", C.c_int), ("newton_rtol", C.c_double),
         ("tau_relax_floor_over_dtau", C.c_double),
+        ("storage", C.c_int),
     ]
 
 

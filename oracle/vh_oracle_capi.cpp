@@ -138,7 +138,13 @@ void vho_regulation_map(vho_handle* h, double* out) {
   const size_t ne = (size_t)P.nx * P.ny * P.nz;
   for (size_t b = 0; b < h->ev.size(); ++b) h->ev[b]->regulation_map(out + b * ne);
 }
-void vho_post(vho_handle* h, int ev, double tau) { Sol* s = h->ev[ev]; s->post(s->q, s->u, tau); }
+void vho_post(vho_handle* h, int ev, double tau) { Sol* s = h->ev[ev]; s->post(s->q, s->u, tau, s->u); }
+// post() of q with the current u as the starting velocity of the reduced mode's fixed point (copied first: post overwrites u)
+void vho_post_guess(vho_handle* h, int ev, double tau) {
+  Sol* s = h->ev[ev];
+  std::vector<double> g[4] = {s->u[0], s->u[1], s->u[2], s->u[3]};
+  s->post(s->q, s->u, tau, g);
+}
 void vho_ghost(vho_handle* h, int ev) { Sol* s = h->ev[ev]; s->ghost(s->q, s->e, s->p, s->u); }
 
 // ---- scalar pieces

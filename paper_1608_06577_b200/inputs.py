@@ -33,6 +33,7 @@ def base_params(**over):
         minmod_theta=1.0, xi0=0.1, rho_max=1.0,
         newton_max_iter=50, newton_rtol=1e-13,
         tau_relax_floor_over_dtau=5.0,
+        storage=0,
     )
     for k, v in over.items():
         if k not in d:
