@@ -18,14 +18,14 @@ SO = os.path.join(HERE, "libvh.so")
 # real = double: libvh.so (the product, everything BASELINE.json measures); real = float: libvh_f32.so
 LIBS = {"f64": (SO, []), "f32": (os.path.join(HERE, "libvh_f32.so"), ["-DVH_REAL=float"])}
 N_COMBO = 12
-HEADERS = ["vh_real.cuh", "vh_peaks.cuh", "vh_device.cuh", "vh_math.cuh", "vh_kernels.cuh", "vh_kernels2.cuh", "vh_kernels3.cuh", "vh_kernels4.cuh", "vh_internal.cuh", "vh_eos_lattice.hpp",
+HEADERS = ["vh_real.cuh", "vh_peaks.cuh", "vh_device.cuh", "vh_math.cuh", "vh_kernels.cuh", "vh_kernels2.cuh", "vh_kernels3.cuh", "vh_kernels4.cuh", "vh_kernels5.cuh", "vh_internal.cuh", "vh_eos_lattice.hpp",
            os.path.join("..", "..", "include", "vh.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 
 def units():
     """(source, object, extra flags) of every translation unit."""
-    out = [("vh_api.cu", "vh_api.o", [])]
+    out = [("vh_api.cu", "vh_api.o", []), ("vh_launch_reduced.cu", "vh_launch_reduced.o", [])]
     for k in range(N_COMBO):
         out.append(("vh_launch.cu", "vh_launch_%d.o" % k, ["-DVH_COMBO=%d" % k]))
     return out
@@ -35,7 +35,7 @@ def up_to_date(so) -> bool:
     if not os.path.exists(so):
         return False
     t = os.path.getmtime(so)
-    deps = [os.path.join(CSRC, f) for f in ["vh_api.cu", "vh_launch.cu"] + HEADERS] + [os.path.abspath(__file__)]
+    deps = [os.path.join(CSRC, f) for f in ["vh_api.cu", "vh_launch.cu", "vh_launch_reduced.cu"] + HEADERS] + [os.path.abspath(__file__)]
     return all(os.path.getmtime(d) <= t for d in deps)
 
 

@@ -2,6 +2,7 @@
 #include "vh_internal.cuh"
 #include "vh_eos_lattice.hpp"
 #include "vh_peaks.cuh"
+#include "vh_kernels5.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -92,6 +93,8 @@ static int check_params(const vh_params* p, std::string& why) {
   if (!(p->minmod_theta >= 1.0 && p->minmod_theta <= 2.0)) { why = "minmod_theta must lie in [1,2] (Eq. 67)"; return -1; }
   if (!(p->rho_max > 0 && p->xi0 > 0)) { why = "xi0, rho_max must be > 0"; return -1; }
   if (p->newton_max_iter < 1 || !(p->newton_rtol > 0)) { why = "newton_max_iter >= 1 and newton_rtol > 0 required"; return -1; }
+  if (p->storage != 0 && p->storage != 1) { why = "storage must be 0 (all components) or 1 (reduced, PAPER.md:476)"; return -1; }
+  if (p->storage == 1 && !(p->physics & 1)) { why = "storage = 1 needs shear on: without pi^{mu nu} there is nothing to reduce"; return -1; }
   if (kF32 && p->newton_rtol < 1e-6) { why = "the single-precision library needs newton_rtol >= 1e-6 (a tighter stopping rule cannot be met in FP32)"; return -1; }
   if ((long long)p->nz * p->n_batch > 65535) { why = "nz*n_batch exceeds the grid z limit (65535)"; return -1; }
   return 0;
@@ -164,10 +167,11 @@ static int make_tensor_maps(vh_handle* h, int n_arrays) {
 }
 
 static cudaError_t launch_ghost(vh_handle* h, real* q, real* e, real* p, real* u) {
+  const int nq = h->reduced ? NQR : NQ, nu = h->reduced ? 3 : 4;
   const DevParams& P = h->P;
   long long W = h->two_d ? (long long)P.ny + P.nx : (long long)P.ny * P.nz + (long long)P.nx * P.nz + (long long)P.nx * P.ny;
-  dim3 grid((unsigned)((W + 255) / 256), 21, P.n_batch);
-  GhostArgs G{q, e, p, u};
+  dim3 grid((unsigned)((W + 255) / 256), nq + 2 + nu, P.n_batch);
+  GhostArgs G{q, e, p, u, nq};
   if (h->two_d) ghost_kernel<true><<<grid, 256, 0, h->stream>>>(P, G);
   else ghost_kernel<false><<<grid, 256, 0, h->stream>>>(P, G);
   h->launches++;
@@ -219,21 +223,23 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
   h->stream = (cudaStream_t)cuda_stream;
   cudaGetDevice(&h->device);
   const long long fs = h->P.fstride;
-  const size_t bytes = (size_t)67 * fs * sizeof(real);
+  h->reduced = (p->storage == 1);
+  const int nq = h->reduced ? NQR : NQ, nu = h->reduced ? 3 : 4;
+  const int n_arrays = 3 * nq + 3 * nu + 4 + (h->reduced ? 0 : 6);      // 67, or 43 in reduced storage (no state velocities: its kernel inverts in place)
+  const size_t bytes = (size_t)n_arrays * fs * sizeof(real);
   ce = cudaMalloc((void**)&h->pool, bytes);
   if (ce != cudaSuccess) { cudaGetLastError(); delete h; return fail(nullptr, VH_ERR_ALLOC, std::string("cudaMalloc of ") + std::to_string(bytes) + " bytes: " + cudaGetErrorString(ce)); }
   ce = cudaMalloc((void**)&h->cnt, sizeof(Counters));
   if (ce != cudaSuccess) { cudaGetLastError(); cudaFree(h->pool); delete h; return fail(nullptr, VH_ERR_ALLOC, "cudaMalloc(counters) failed"); }
   real* w = h->pool;
-  for (int i = 0; i < 3; ++i) { h->q[i] = w; w += 15 * fs; }
-  for (int i = 0; i < 3; ++i) { h->u[i] = w; w += 4 * fs; }
+  for (int i = 0; i < 3; ++i) { h->q[i] = w; w += nq * fs; }
+  for (int i = 0; i < 3; ++i) { h->u[i] = w; w += nu * fs; }
   for (int i = 0; i < 2; ++i) { h->e[i] = w; w += fs; }
   for (int i = 0; i < 2; ++i) { h->p[i] = w; w += fs; }
-  h->vL = w; w += 3 * fs;
-  h->vR = w; w += 3 * fs;
+  if (!h->reduced) { h->vL = w; w += 3 * fs; h->vR = w; w += 3 * fs; }
   ce = cudaMemsetAsync(h->pool, 0, bytes, h->stream);
   if (ce != cudaSuccess) { cudaFree(h->pool); cudaFree(h->cnt); delete h; return fail(nullptr, VH_ERR_CUDA, "cudaMemsetAsync failed"); }
-  if (make_tensor_maps(h, 67) != VH_OK) {
+  if (make_tensor_maps(h, n_arrays) != VH_OK) {
     std::string msg = h->err;
     cudaFree(h->pool); cudaFree(h->cnt); delete h;
     return fail(nullptr, VH_ERR_CUDA, msg);
@@ -283,6 +289,7 @@ long long vh_launch_count(vh_handle* h) { return h ? h->launches : 0; }
 int vh_set_kernel_variant(vh_handle* h, int variant) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   if (variant < 0 || variant > 2) return fail(h, VH_ERR_ARG, "unknown kernel variant");
+  if (h->reduced && variant != 0) return fail(h, VH_ERR_ARG, "reduced-storage mode has one kernel (variant 0)");
   h->variant = variant;
   return VH_OK;
 }
@@ -315,13 +322,24 @@ int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double
     de = s; du = s + np; dpi = pi10 ? s + 5 * np : nullptr; dPi = Pi ? s + 15 * np : nullptr;
   }
   unsigned nb = (unsigned)((np + 255) / 256);
-  if (h->prm.eos == 2) init_kernel<2><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
+  if (h->reduced) {
+    const real t0 = (real)h->prm.tau0;
+    const bool mil = (h->prm.geometry == 0);
+#define VH_INIT_RED(E)                                                                                                                        \
+  do {                                                                                                                                        \
+    if (mil) init_reduced_kernel<E, true><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, t0, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);   \
+    else init_reduced_kernel<E, false><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, t0, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);      \
+  } while (0)
+    if (h->prm.eos == 2) VH_INIT_RED(2); else if (h->prm.eos == 1) VH_INIT_RED(1); else VH_INIT_RED(0);
+#undef VH_INIT_RED
+  } else if (h->prm.eos == 2) init_kernel<2><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
   else if (h->prm.eos == 1) init_kernel<1><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
   else init_kernel<0><<<nb, 256, 0, h->stream>>>(P, de, du, dpi, dPi, h->q[0], h->e[0], h->p[0], h->u[0], h->u[1]);
   h->launches++;
   CUDA_TRY(h, cudaGetLastError());
   CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
   h->n_steps = 0;
+  h->uprev_initial = true;
   int rc = reset_counters(h);
   if (rc) return rc;
   CUDA_TRY(h, reset_regulation_map(h));
@@ -344,16 +362,22 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
     int rc = ensure_stage(h, &h->stage_in, &h->stage_in_bytes, (size_t)16 * np * sizeof(double));
     if (rc) return rc;
   }
-  for (const Item& it : items) {
+  for (int n = 0; n < 4; ++n) {
+    const Item& it = items[n];
     const double* src = it.src;
     if (mem_space == 0) {
       CUDA_TRY(h, cudaMemcpyAsync(h->stage_in, it.src, (size_t)it.nc * np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
       src = h->stage_in;
     }
-    pack_kernel<false><<<nb, 256, 0, h->stream>>>(P, it.dst, const_cast<double*>(src), it.nc);
+    if (h->reduced && n != 1) {      // q15 / u4 / u4_prev: only the stored subset is kept (the dependent components are not state)
+      import_reduced_kernel<<<nb, 256, 0, h->stream>>>(P, n == 0 ? src : nullptr, n == 0 ? nullptr : src, n == 0 ? it.dst : nullptr, n == 0 ? nullptr : it.dst);
+    } else {
+      pack_kernel<false><<<nb, 256, 0, h->stream>>>(P, it.dst, const_cast<double*>(src), it.nc);
+    }
     h->launches++;
     CUDA_TRY(h, cudaGetLastError());
   }
+  h->uprev_initial = false;      // u4_prev belongs to tau - dtau
   if (h->prm.eos == 2) pressure_kernel<2><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
   else if (h->prm.eos == 1) pressure_kernel<1><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
   else pressure_kernel<0><<<nb, 256, 0, h->stream>>>(P, h->e[0], h->p[0]);
@@ -382,14 +406,44 @@ int vh_set_uprev(vh_handle* h, const double* u4_prev, int mem_space) {
     CUDA_TRY(h, cudaMemcpyAsync(h->stage_in, u4_prev, 4 * np * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     src = h->stage_in;
   }
-  pack_kernel<false><<<(unsigned)((np + 255) / 256), 256, 0, h->stream>>>(P, h->u[1], const_cast<double*>(src), 4);
+  if (h->reduced) import_reduced_kernel<<<(unsigned)((np + 255) / 256), 256, 0, h->stream>>>(P, nullptr, src, nullptr, h->u[1]);
+  else pack_kernel<false><<<(unsigned)((np + 255) / 256), 256, 0, h->stream>>>(P, h->u[1], const_cast<double*>(src), 4);
+  h->uprev_initial = false;
   h->launches++;
   CUDA_TRY(h, cudaGetLastError());
   if (mem_space == 0) CUDA_TRY(h, cudaStreamSynchronize(h->stream));
   return VH_OK;
 }
 
+// reduced storage: (stage kernel, ghost kernel) per stage; same buffer rotation
+static int one_step_reduced(vh_handle* h, cudaEvent_t* ev) {
+  const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;
+  const double t1 = t + h->prm.dtau;
+  RedArgs A;
+  A.q_in = h->q[0]; A.e_in = h->e[0]; A.p_in = h->p[0]; A.u_in = h->u[0]; A.u_prev = h->u[1]; A.q_n = nullptr;
+  A.q_out = h->q[1]; A.e_out = h->e[1]; A.p_out = h->p[1]; A.u_out = h->u[2]; A.cnt = h->cnt;
+  A.t = (real)t; A.t_post = (real)t1; A.t_prev = (real)(h->uprev_initial ? t : t - h->prm.dtau);
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[0], h->stream));
+  CUDA_TRY(h, vh_launch_stage_reduced(h, 1, A));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[1], h->stream));
+  CUDA_TRY(h, launch_ghost(h, h->q[1], h->e[1], h->p[1], h->u[2]));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[2], h->stream));
+  A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
+  A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1];
+  A.t = (real)t1; A.t_post = (real)t1; A.t_prev = (real)t;
+  CUDA_TRY(h, vh_launch_stage_reduced(h, 2, A));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[3], h->stream));
+  CUDA_TRY(h, launch_ghost(h, h->q[2], h->e[0], h->p[0], h->u[1]));
+  if (ev) CUDA_TRY(h, cudaEventRecord(ev[4], h->stream));
+  real* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;
+  real* qn = h->q[2]; h->q[2] = h->q[0]; h->q[0] = qn;
+  h->n_steps++;
+  h->uprev_initial = false;
+  return VH_OK;
+}
+
 static int one_step(vh_handle* h, cudaEvent_t* ev) {
+  if (h->reduced) return one_step_reduced(h, ev);
   const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau;     // :493
   const double t1 = t + h->prm.dtau;
   StageArgs A;
@@ -474,9 +528,20 @@ int vh_get_fields(vh_handle* h, double* q15, double* e, double* p, double* u4, d
     int rc = ensure_stage(h, &h->stage_out, &h->stage_out_bytes, (size_t)15 * np * sizeof(double));
     if (rc) return rc;
   }
-  for (const Item& it : items) {
+  const real tnow = (real)(h->prm.tau0 + (double)h->n_steps * h->prm.dtau);
+  const real tprev = (real)(h->uprev_initial ? tnow : tnow - h->prm.dtau);
+  for (int n = 0; n < 5; ++n) {
+    const Item& it = items[n];
     if (!it.dst) continue;
     double* target = (mem_space == 1) ? it.dst : h->stage_out;
+    if (h->reduced && (n == 0 || n >= 3)) {      // q15, u4, u4_prev: expanded from the stored subset (Eqs. 47-51, u.u = 1)
+      const bool mil = (h->prm.geometry == 0);
+      const real* qs = (n == 0) ? h->q[0] : nullptr;
+      const real* us = (n == 4) ? h->u[1] : h->u[0];
+      const real tt = (n == 4) ? tprev : tnow;
+      if (mil) export_reduced_kernel<true><<<nb, 256, 0, h->stream>>>(P, qs, us, tt, n == 0 ? target : nullptr, n == 0 ? nullptr : target);
+      else export_reduced_kernel<false><<<nb, 256, 0, h->stream>>>(P, qs, us, tt, n == 0 ? target : nullptr, n == 0 ? nullptr : target);
+    } else
     pack_kernel<true><<<nb, 256, 0, h->stream>>>(P, it.src, target, it.nc);
     h->launches++;
     CUDA_TRY(h, cudaGetLastError());
@@ -514,6 +579,7 @@ int vh_eos_table(double* nodes4, double* x0, double* h) {
 int vh_get_diagnostics(vh_handle* h, double* out10) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
+  if (h->reduced) return fail(h, VH_ERR_STATE, "vh_get_diagnostics is not available in reduced-storage mode (storage = 1): the diagnostics kernels read the full set of arrays");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostics before vh_set_initial");
   if (!out10) return fail(h, VH_ERR_ARG, "out10 is NULL");
   if (!h->diag && cudaMalloc((void**)&h->diag, 10 * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); h->diag = nullptr; return fail(h, VH_ERR_ALLOC, "cudaMalloc(diagnostics) failed"); }
@@ -531,6 +597,7 @@ int vh_get_diagnostics(vh_handle* h, double* out10) {
 int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
+  if (h->reduced) return fail(h, VH_ERR_STATE, "vh_get_diagnostic_maps is not available in reduced-storage mode (storage = 1): the diagnostics kernels read the full set of arrays");
   if (!maps10) return fail(h, VH_ERR_ARG, "maps10 is NULL");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_get_diagnostic_maps before vh_set_initial");
@@ -554,6 +621,7 @@ int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space) {
 int vh_enable_regulation_map(vh_handle* h, int on) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
+  if (h->reduced) return fail(h, VH_ERR_STATE, "vh_enable_regulation_map is not available in reduced-storage mode (storage = 1): the diagnostics kernels read the full set of arrays");
   if (!on) {
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     cudaFree(h->regfac);
@@ -574,6 +642,7 @@ int vh_enable_regulation_map(vh_handle* h, int on) {
 int vh_get_regulation_map(vh_handle* h, double* map, int mem_space) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
+  if (h->reduced) return fail(h, VH_ERR_STATE, "vh_get_regulation_map is not available in reduced-storage mode (storage = 1): the diagnostics kernels read the full set of arrays");
   if (!map) return fail(h, VH_ERR_ARG, "map is NULL");
   if (mem_space != 0 && mem_space != 1) return fail(h, VH_ERR_ARG, "mem_space must be 0 (host) or 1 (device)");
   if (!h->regfac) return fail(h, VH_ERR_STATE, "vh_get_regulation_map without vh_enable_regulation_map(h, 1)");
@@ -596,6 +665,7 @@ int vh_get_regulation_map(vh_handle* h, double* map, int mem_space) {
 int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long long* steps_done) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
+  if (h->reduced) return fail(h, VH_ERR_STATE, "vh_run_until is not available in reduced-storage mode (storage = 1): the diagnostics kernels read the full set of arrays");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_run_until before vh_set_initial");
   if (max_steps < 0 || check_every < 1 || !(T_f >= 0.0)) return fail(h, VH_ERR_ARG, "max_steps >= 0, check_every >= 1, T_f >= 0 required");
   long long done = 0;

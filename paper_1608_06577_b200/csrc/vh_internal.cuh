@@ -36,6 +36,8 @@ struct vh_handle {
   long long launches = 0;
   bool initialised = false;
   bool two_d = false;
+  bool reduced = false;              // vh_params.storage == 1: 10 q + 3 u arrays per time level (vh_kernels5.cuh), own stage kernel
+  bool uprev_initial = true;         // u^{n-1} is the copy of u^0 made by vh_set_initial (reduced storage: its u^tau is normalised at tau0, not tau0 - dtau)
   int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
   CUtensorMap mapVA, mapVZ;          // velocity tile kernel: tile + 1-cell y halo, one eta-halo plane
   CUtensorMap mapA, mapZ, mapC;      // TMA tensor maps over the whole pool (box A: tile + xy halo, box Z: two eta-halo planes, box C: the tile)
@@ -69,3 +71,6 @@ inline cudaError_t vh_opt_in_smem(vh_handle* h, const void* kern, size_t smem) {
 VH_DECLARE_COMBO(0) VH_DECLARE_COMBO(1) VH_DECLARE_COMBO(2) VH_DECLARE_COMBO(3) VH_DECLARE_COMBO(4) VH_DECLARE_COMBO(5)
 VH_DECLARE_COMBO(6) VH_DECLARE_COMBO(7) VH_DECLARE_COMBO(8) VH_DECLARE_COMBO(9) VH_DECLARE_COMBO(10) VH_DECLARE_COMBO(11)
 #undef VH_DECLARE_COMBO
+// reduced-storage stage (vh_launch_reduced.cu): one launch of stage_reduced_kernel; A is a vh::RedArgs
+namespace vh { struct RedArgs; }
+cudaError_t vh_launch_stage_reduced(vh_handle* h, int stage, const vh::RedArgs& A);

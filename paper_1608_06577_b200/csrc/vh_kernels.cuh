@@ -295,13 +295,13 @@ __global__ void __launch_bounds__(256) stage_cell_kernel(const __grid_constant__
 }
 
 // ------------------------------------------------------------------------------------------------ ghost cells (Eqs. 75-76)
-struct GhostArgs { real* q; real* e; real* p; real* u; };
+struct GhostArgs { real* q; real* e; real* p; real* u; int nq; };      // nq conserved arrays (15, or 10 in reduced storage), then e, p, then the u arrays
 
-// grid: (ceil(W/256), 21, n_batch); W = ny*nz + nx*nz + nx*ny (3+1d) or ny + nx (2+1d)
+// grid: (ceil(W/256), nq + 2 + nu, n_batch); W = ny*nz + nx*nz + nx*ny (3+1d) or ny + nx (2+1d)
 template <bool TWO_D>
 __global__ void __launch_bounds__(256) ghost_kernel(const __grid_constant__ DevParams P, const GhostArgs G) {
   const int a = blockIdx.y;
-  real* f = (a < 15) ? G.q + (long long)a * P.fstride : (a == 15 ? G.e : (a == 16 ? G.p : G.u + (long long)(a - 17) * P.fstride));
+  real* f = (a < G.nq) ? G.q + (long long)a * P.fstride : (a == G.nq ? G.e : (a == G.nq + 1 ? G.p : G.u + (long long)(a - G.nq - 2) * P.fstride));
   f += (long long)blockIdx.z * P.bstride;
   const long long Wx = (long long)P.ny * P.nz, Wy = (long long)P.nx * P.nz, Wz = TWO_D ? 0 : (long long)P.nx * P.ny;
   long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
