@@ -268,6 +268,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-paper-physics", action="store_true", help="skip the second, labelled measurement with the lattice EOS and Eq. 17 zeta/s")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: the single-precision build (libvh_f32.so; SURVEY 8(f) NEXT-3), a labelled extra line")
+    ap.add_argument("--storage", type=int, default=0, choices=[0, 1], help="1: reduced-storage mode (5 pi + 3 u components, PAPER.md:476; SURVEY 8(f) NEXT-3), a labelled extra line")
     ap.add_argument("--physics", default="config3", choices=["config3", "paper"], help="paper: lattice EOS + Eq. 17 zeta/s on the config-3 grid")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -294,6 +295,7 @@ def main():
 
     prm, init = workload(rank, args.physics)
     f32 = (args.precision == "f32")
+    prm["storage"] = args.storage
     if f32:
         prm["newton_rtol"] = 2e-6          # the stopping rule of Eq. 72 at single precision (the f32 library refuses anything below 1e-6)
     ncell = prm["nx"] * prm["ny"] * prm["nz"] * prm["n_batch"]
@@ -364,7 +366,7 @@ def main():
 
     # ---------------- second, labelled workload: the paper's own physics (lattice EOS, Eq. 17 zeta/s) on the same grid
     paper_line = None
-    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics and not f32:
+    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics and not f32 and not args.storage:
         prm2, init2 = workload(rank, "paper")
         s2 = vh.Solver(prm2, device=dev)
         s2.set_initial(torch.as_tensor(init2["e"], device=dev), torch.as_tensor(init2["u"], device=dev))
@@ -391,8 +393,8 @@ def main():
                 pass
         flops_cu, mix, by_section = algorithmic_flops(prm, init)
         flops_inv_cu = by_section["invert"]
-        variant1 = (args.variant == 1)
-        default_pipeline = (args.variant == 0)
+        variant1 = (args.variant == 1) or args.storage == 1
+        default_pipeline = (args.variant == 0) and args.storage == 0
         # Kernel shares of the algorithmic work: the velocity kernel does the interface-state inversions
         # (Eq. 72 at every reconstructed state), the stage kernel everything else; one stage = half of a cell-update.
         alg_kernel = {k: 0.5 * (flops_inv_cu if "velocity" in k else flops_cu - flops_inv_cu) for k in LAUNCH_KEYS}
@@ -427,7 +429,7 @@ def main():
         roof["frac"] = roof["achieved"] / roof["peak"]
         useful_step = sum(useful.values())
         step_roof_s = max(useful_step * ncell / (alu_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * bscale * ncell / (hbm_peak * 1e9))
-        kname = ("velocity_tile_kernel" if "velocity" in dom else "stage_tile_kernel") if default_pipeline else ("stage_cell_kernel" if variant1 else "stage_kernel")
+        kname = ("velocity_tile_kernel" if "velocity" in dom else "stage_tile_kernel") if default_pipeline else ("stage_reduced_kernel" if args.storage else ("stage_cell_kernel" if variant1 else "stage_kernel"))
         roof.update({
             "traffic": traffic_kernel.get(dom), "traffic_source": os.path.relpath(NCU_METRICS_CSV, ROOT) if dom in traffic_kernel else None,
             "kernel": "%s (%s)" % (kname, dom), "launch_ms": prof[dom],
@@ -454,7 +456,7 @@ def main():
         line = {
             "metric": METRIC_F32 if f32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
-            "config": {"workload": ("SINGLE-PRECISION BUILD (labelled extra line, not the BASELINE.json metric, which is FP64): " if f32 else "") + ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
+            "config": {"workload": ("SINGLE-PRECISION BUILD (labelled extra line, not the BASELINE.json metric, which is FP64): " if f32 else "") + ("REDUCED-STORAGE MODE (5 pi + 3 u components stored, 43 instead of 67 arrays; labelled extra line): " if args.storage else "") + ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
                                     "dtau=0.025, one independent replica per GPU (no sharding, no collective)") if args.physics == "config3" else
                                    ("configs[2] grid and hotspots with the paper's own physics: lattice EOS (Eqs. 19-20), zeta/s of Eq. 17 (T_c = 200 MeV), "
                                     "eta/s=0.2; one independent replica per GPU"),

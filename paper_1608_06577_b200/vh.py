@@ -188,10 +188,10 @@ class Solver:
 
     def step_profile(self, n=1):
         """n steps with CUDA events around each of the four launches of a step; mean ms per launch, keyed by kernel:
-        variants 0, 2: velocity1, stage1, velocity2, stage2; variant 1: stage1, ghost1, stage2, ghost2."""
+        variants 0, 2: velocity1, stage1, velocity2, stage2; variant 1 and reduced storage: stage1, ghost1, stage2, ghost2."""
         ms = (C.c_double * 4)()
         self._check(self.L.vh_step_profile(self.h, int(n), ms), "vh_step_profile")
-        names = ("stage1", "ghost1", "stage2", "ghost2") if self.variant == 1 else ("velocity1", "stage1", "velocity2", "stage2")
+        names = ("stage1", "ghost1", "stage2", "ghost2") if (self.variant == 1 or self.d.get("storage", 0) == 1) else ("velocity1", "stage1", "velocity2", "stage2")
         return dict(zip(names, list(ms)))
 
     def get_fields(self, device=None, with_uprev=False, out=None):
