@@ -290,7 +290,7 @@ def test_error_codes_and_status(vh):
     assert L.vh_step(s.h, -1) == -1
     n0 = s.launch_count()
     s.step(2)
-    assert s.launch_count() - n0 == 8                    # 2 stage + 2 ghost kernels per step
+    assert s.launch_count() - n0 == 8                    # default pipeline: (velocity kernel + stage kernel) per Euler stage = 4 launches per step
     st = s.status()
     assert st["n_steps"] == 2 and st["tau"] == pytest.approx(0.5 + 2 * 0.025) and st["n_inversion_failures"] == 0
     s.close()
