@@ -123,7 +123,7 @@ namespace vh {
 // the factor 1/2 of the half-cell extrapolation is folded into the caller's FMA.
 __device__ __forceinline__ real minmod2(real d1, real d2) {
   const real t = (fabs(d1) < fabs(d2)) ? d1 : d2;
-  return sign_differs(d1, d2) ? real(0.0) : t;
+  return zero_if(sign_differs(d1, d2), t);
 }
 // general theta: minmod(theta d1, (d1 + d2)/2, theta d2); `theta` in [1, 2]
 __device__ __forceinline__ real minmod3(real d1, real d2, real theta) {
