@@ -82,11 +82,17 @@ def host_cpu():
     return model, os.cpu_count()
 
 
-def workload(rank=0, physics="config3"):
+def workload(rank=0, physics="config3", which="config3"):
     """configs[2] of BASELINE.json (default); physics="paper": the same grid and hotspots with the paper's own equation of state
-    (lattice, Eqs. 19-20) and zeta/s(T) (Eq. 17, T_c = 200 MeV) - SURVEY 8(f) NEXT-1 - for a second, labelled bench line."""
+    (lattice, Eqs. 19-20) and zeta/s(T) (Eq. 17, T_c = 200 MeV) - SURVEY 8(f) NEXT-1 - for a second, labelled bench line.
+    which = "config4" / "config5": the batched 2+1d and the large 3+1d configurations of BASELINE.json (labelled extra lines)."""
     over = dict(eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC) if physics == "paper" else {}
-    prm, init, _ = inputs.config_3d(seed=inputs.BASE_SEED + rank, **over)
+    if which == "config4":
+        prm, init, _ = inputs.config_batched2d(seed=inputs.BASE_SEED + 1000 * rank, **over)
+    elif which == "config5":
+        prm, init, _ = inputs.config_3d(512, 512, 128, 0.05, 0.05, 0.1, n_hot=200, n_steps=50, seed=inputs.BASE_SEED + rank, **over)
+    else:
+        prm, init, _ = inputs.config_3d(seed=inputs.BASE_SEED + rank, **over)
     return prm, init
 
 
@@ -204,9 +210,10 @@ class ClockSampler:
 
 def oracle_sample(prm, init, nx, ny, nz):
     """Central cut-out of the workload for the CPU oracle (bounded sample of the same initial data)."""
+    nz = min(nz, prm["nz"])
     z0, y0, x0 = (prm["nz"] - nz) // 2, (prm["ny"] - ny) // 2, (prm["nx"] - nx) // 2
-    cut = lambda a: np.ascontiguousarray(a[..., z0:z0 + nz, y0:y0 + ny, x0:x0 + nx])
-    sub = dict(prm, nx=nx, ny=ny, nz=nz)
+    cut = lambda a: np.ascontiguousarray(a[..., 0:1, z0:z0 + nz, y0:y0 + ny, x0:x0 + nx])
+    sub = dict(prm, nx=nx, ny=ny, nz=nz, n_batch=1)
     return sub, cut(init["e"]), cut(init["u"])
 
 
@@ -268,6 +275,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-paper-physics", action="store_true", help="skip the second, labelled measurement with the lattice EOS and Eq. 17 zeta/s")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: the single-precision build (libvh_f32.so; SURVEY 8(f) NEXT-3), a labelled extra line")
+    ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config5"],
+                    help="config4 (256 batched 2+1d events) / config5 (512x512x128): labelled extra lines; the default is the BASELINE.json metric")
     ap.add_argument("--storage", type=int, default=0, choices=[0, 1], help="1: reduced-storage mode (5 pi + 3 u components, PAPER.md:476; SURVEY 8(f) NEXT-3), a labelled extra line")
     ap.add_argument("--physics", default="config3", choices=["config3", "paper"], help="paper: lattice EOS + Eq. 17 zeta/s on the config-3 grid")
     args = ap.parse_args()
@@ -293,7 +302,8 @@ def main():
     W = max(args.warmup, 3)
     K = args.steps
 
-    prm, init = workload(rank, args.physics)
+    prm, init = workload(rank, args.physics, args.workload)
+    other = (args.workload != "config3")
     f32 = (args.precision == "f32")
     prm["storage"] = args.storage
     if f32:
@@ -305,6 +315,8 @@ def main():
     e_d = torch.as_tensor(init["e"], device=dev)
     u_d = torch.as_tensor(init["u"], device=dev)
     s.set_initial(e_d, u_d)
+    xoff = 4 if f32 else 2
+    s_bytes = (43 if args.storage else 67) * ((prm["nx"] + xoff + 2 + 15) // 16 * 16) * (prm["ny"] + 4) * (prm["nz"] + 4 if prm["nz"] > 1 else 1) * prm["n_batch"] * (4 if f32 else 8)
 
     def barrier():
         torch.cuda.synchronize()
@@ -333,7 +345,7 @@ def main():
     # ---------------- per-kernel durations (CUDA events around each launch on the launching stream)
     prof = s.step_profile(min(K, 10))       # keyed by kernel: velocity1, stage1, velocity2, stage2 (variant 1: stage1, ghost1, stage2, ghost2)
 
-    # ---------------- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    # ---------------- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region (default workload only)
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
     f_dev = s.get_fields()
     h_e, h_u = pin(f_dev["e"].cpu().numpy()), pin(f_dev["u"].cpu().numpy())
@@ -344,7 +356,7 @@ def main():
     del f_dev
     h2d = (h_e.numel() + h_u.numel() + h_pi.numel() + h_Pi.numel()) * 8
     d2h = sum(v.numel() for v in out.values()) * 8
-    E = max(1, args.e2e_steps)
+    E = 1 if other else max(1, args.e2e_steps)
     s.set_initial(h_e, h_u, h_pi, h_Pi); s.step(1); s.get_fields(out=out)      # warm-up (allocates staging buffers)
     barrier()
     t0 = time.perf_counter()
@@ -366,7 +378,7 @@ def main():
 
     # ---------------- second, labelled workload: the paper's own physics (lattice EOS, Eq. 17 zeta/s) on the same grid
     paper_line = None
-    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics and not f32 and not args.storage:
+    if world == 1 and args.physics == "config3" and not args.variant and not args.no_paper_physics and not f32 and not args.storage and not other:
         prm2, init2 = workload(rank, "paper")
         s2 = vh.Solver(prm2, device=dev)
         s2.set_initial(torch.as_tensor(init2["e"], device=dev), torch.as_tensor(init2["u"], device=dev))
@@ -401,7 +413,7 @@ def main():
         if variant1:
             alg_kernel = {"stage1": 0.5 * flops_cu, "stage2": 0.5 * flops_cu}
         bytes_kernel = {k: v * bscale for k, v in {"stage1": ALG_BYTES_STAGE["stage1"], "stage2": ALG_BYTES_STAGE["stage2"], "velocity1": 10 * 8.0, "velocity2": 10 * 8.0}.items()}
-        ncu = ncu_metrics() if (ncell == 128 ** 3 and default_pipeline and args.physics == "config3" and not f32) else {}
+        ncu = ncu_metrics() if (ncell == 128 ** 3 and default_pipeline and args.physics == "config3" and not f32 and not other) else {}
         ex_kernel, pipe_kernel, traffic_kernel = {}, {}, {}
         for k, m in ncu.items():
             try:
@@ -434,7 +446,8 @@ def main():
             "traffic": traffic_kernel.get(dom), "traffic_source": os.path.relpath(NCU_METRICS_CSV, ROOT) if dom in traffic_kernel else None,
             "kernel": "%s (%s)" % (kname, dom), "launch_ms": prof[dom],
             "peak_source": ("FP32 FMA microbenchmark, same run (vh_measure_fp32_peak)" if f32 else "FP64 FMA microbenchmark, same run (vh_measure_peaks)") if roof["bound"] == "alu" else hbm_src,
-            "numerator": "min(minimal algorithmic flops, executed flops) of this kernel per cell x cells per launch",
+            "numerator": "min(minimal algorithmic flops, executed flops) of this kernel per cell x cells per launch" if dom in ex_kernel else
+                         "minimal algorithmic flops (NO ncu capture of this configuration is committed: on config 3 the kernels execute 1.4x fewer flops than this count, so frac here is that much too kind)",
             "alg_flops_this_kernel_per_cell": alg_kernel[dom], "executed_flops_per_cell": ex_kernel.get(dom),
             "alg_over_executed": (alg_kernel[dom] / ex_kernel[dom]) if dom in ex_kernel else None,
             "fp64_pipe_util": pipe_kernel.get(dom),
@@ -454,13 +467,13 @@ def main():
                                "traffic": traffic_kernel.get(k), "alg_bytes": bytes_kernel[k] * ncell} for k in cand},
         })
         line = {
-            "metric": METRIC_F32 if f32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "metric": (METRIC_F32 if f32 else METRIC).replace("at 128^3 viscous", {"config4": "on 256 x 201^2 batched 2+1d viscous events", "config5": "at 512x512x128 viscous"}.get(args.workload, "at 128^3 viscous")), "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
-            "config": {"workload": ("SINGLE-PRECISION BUILD (labelled extra line, not the BASELINE.json metric, which is FP64): " if f32 else "") + ("REDUCED-STORAGE MODE (5 pi + 3 u components stored, 43 instead of 67 arrays; labelled extra line): " if args.storage else "") + ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
+            "config": {"workload": ("SINGLE-PRECISION BUILD (labelled extra line, not the BASELINE.json metric, which is FP64): " if f32 else "") + ("REDUCED-STORAGE MODE (5 pi + 3 u components stored, 43 instead of 67 arrays; labelled extra line): " if args.storage else "") + ({"config4": "configs[3] (labelled extra line): 256 independent 2+1d events of 201x201 in one launch; physics of ", "config5": "configs[4] (labelled extra line): 512x512x128, 200 hotspots; physics of "}.get(args.workload, "")) + ("configs[2]: 128x128x128 3+1d viscous non-conformal (EOS 1, eta/s=0.2, Gaussian zeta/s), 40 seeded hotspots, "
                                     "dtau=0.025, one independent replica per GPU (no sharding, no collective)") if args.physics == "config3" else
                                    ("configs[2] grid and hotspots with the paper's own physics: lattice EOS (Eqs. 19-20), zeta/s of Eq. 17 (T_c = 200 MeV), "
                                     "eta/s=0.2; one independent replica per GPU"),
-                       "l2": "state (67 padded arrays, %.2f GB) exceeds the 126 MB L2; no flush needed" % (0.67 if f32 else 1.34), "kernel_variant": args.variant,
+                       "l2": "state (%d padded arrays, %.2f GB) exceeds the 126 MB L2; no flush needed" % (43 if args.storage else 67, s_bytes / 1e9), "kernel_variant": args.variant,
                        "paper_context": "GTX 980 Ti, FP32, lattice EOS: 244.45 ms/step = 8.58e6 cell-updates/s (PAPER.md Table 3; another machine, not a target)"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": E,
                     "what": "per step: vh_set_initial(host e,u,pi,Pi) + vh_step(1) + vh_get_fields(host q,e,p,u), pinned buffers"},
@@ -472,7 +485,7 @@ def main():
         }
         if paper_line is not None:
             line["paper_physics"] = paper_line
-        if world == 1 and not args.no_cpu_baseline:
+        if world == 1 and not args.no_cpu_baseline and not other:
             # SURVEY 8(d) "Oracle timing": the serial oracle on the FULL workload for 3 steps (about 40 s), 1 core, CPU model and core count stated
             v, dt, sample = time_oracle(prm, init, (prm["nx"], prm["ny"], prm["nz"]), 3)
             model, ncores = host_cpu()
