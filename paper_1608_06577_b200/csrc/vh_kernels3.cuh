@@ -38,7 +38,7 @@ template <bool TWO_D> struct Tile {
 };
 template <bool TWO_D, bool VISC> constexpr size_t tile_smem_bytes() {
   using T = Tile<TWO_D>;
-  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(real) + (2 * T::NSTAGE + 1) * sizeof(uint64_t);
+  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(real) + (2 * T::NSTAGE + 1) * sizeof(uint64_t) + T::NW * sizeof(int);
 }
 
 struct TileArgs {
@@ -271,7 +271,7 @@ __device__ __forceinline__ real regulation_factor_fast(const DevParams& P, const
 
 // ------------------------------------------------------------------------------------------------ the kernel
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1, int STAGE, bool REGMAP = false>
-__global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
+__global__ void __launch_bounds__(Tile<TWO_D>::NT, kF32 ? 2 : 1)      // single precision: 64 registers, two CTAs per SM (8 % faster despite 48 bytes of spills)
     stage_tile_kernel(const __grid_constant__ DevParams P, const __grid_constant__ TileArgs A, const __grid_constant__ CUtensorMap mapA,
                       const __grid_constant__ CUtensorMap mapZ, const __grid_constant__ CUtensorMap mapC) {
   using T = Tile<TWO_D>;
@@ -335,13 +335,21 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
     return ring + (s % NSTAGE) * T::SLOT;
   };
   const bool lane0 = (tid & 31) == 0;
-  auto release = [&](int s) {
+  // `witness`: a word that depends on EVERY value the warp loaded from the slot.  Lane 0 stores it to shared memory before it arrives: the
+  // store cannot issue until all those loads have written their registers, so no load of this warp is still in flight when the arrival
+  // becomes visible and the last warp out hands the slot to the TMA unit.  (Issuing the loads before the arrival is not enough: an
+  // arrival does not wait for earlier loads to complete, and the refill of an L2-resident halo can land within a few hundred cycles.
+  // Found in round 2 with two resident CTAs per SM, where a queued load of the refilling warp itself was overtaken about once per launch.)
+  int* witness_sink = reinterpret_cast<int*>(empty + NSTAGE);      // [NW] one word per warp
+  auto release = [&](int s, int witness) {
     __syncwarp();
     if (lane0 && s + NSTAGE < NSTREAM) {
+      *reinterpret_cast<volatile int*>(witness_sink + (tid >> 5)) = witness;
       // the arrival that finds one arrival pending is the last one of this use of the slot: that warp refills it
       if (mbar_arrive_pending(&empty[s % NSTAGE]) == 1u) issue(s + NSTAGE);
     }
   };
+  auto hi = [](real x) -> int { return kF32 ? __float_as_int((float)x) : __double2hiint((double)x); };
 
   // ---- per-thread offsets into a slot: centre in box A, and the four eta neighbours (box A, or the halo boxes at the tile faces)
   const int oc = (tz * AY + (ty + 2)) * AX + (tx + XOFF);
@@ -387,7 +395,6 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       const real xm = s[-1], xp = s[1], ym = s[-AX], yp = s[AX];
       real zm = real(0.0), zp = real(0.0);
       if (!TWO_D) { const real* sb = s - oc; zm = sb[ozm1]; zp = sb[ozp1]; }
-      release(m);
       const real nm[3] = {xm, ym, zm}, np[3] = {xp, yp, zp};
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
@@ -400,13 +407,13 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
           if (m == d + 1) { vm[d] = real(0.0); vp[d] = real(0.0); }
         }
       }
+      release(m, hi(uc[m]) ^ hi(du[1][m]) ^ hi(du[2][m]) ^ hi(du[3][m]));      // (the differences depend on all six neighbours)
     }
     const real* s = acquire(4) + oc;
     const real pc = s[0];
     const real xm = s[-1], xp = s[1], ym = s[-AX], yp = s[AX];
     real zm = real(0.0), zp = real(0.0);
     if (!TWO_D) { const real* sb = s - oc; zm = sb[ozm1]; zp = sb[ozp1]; }
-    release(4);
     // P (v^i delta^nu_tau - g^{i nu}) part of B.2-B.5 (the Pi part follows when Pi streams through)
     acc[0] = fma(wd[0], fma(vm[0], xm, -vp[0] * xp), acc[0]);
     acc[0] = fma(wd[1], fma(vm[1], ym, -vp[1] * yp), acc[0]);
@@ -416,6 +423,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       acc[0] = fma(wd[2], fma(vm[2], zm, -vp[2] * zp), acc[0]);
       acc[3] = wd[2] * it2 * (zm - zp);
     }
+    release(4, hi(pc) ^ hi(acc[0]) ^ hi(acc[1]) ^ hi(acc[2]) ^ hi(acc[3]));
     if (MILNE) {
       // G_c^tau = -(T^{tau tau} + tau^2 T^{eta eta})/tau with T^{eta eta} = (e + P)(u^eta)^2 + P/tau^2 + pi^{eta eta}, P = p + Pi (Eq. 34):
       // the e, p part here; the Pi, pi^{eta eta} and T^{tau mu} parts are added when those fields stream through
@@ -465,7 +473,6 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       const real y0 = s[-2 * AX], y1 = s[-AX], y3 = s[AX], y4 = s[2 * AX];
       real z0 = real(0.0), z1 = real(0.0), z3 = real(0.0), z4 = real(0.0);
       if (!TWO_D) { z0 = sb[ozm2]; z1 = sb[ozm1]; z3 = sb[ozp1]; z4 = sb[ozp2]; }
-      release(5 + n);
       real r = a2;
       if (VISC && n >= PTT) r += park[n * NT + tid];
       if (MILNE && n < 4) r = fma((n == 3) ? -real(3.0) * wt : -wt, a2, r);      // G_c (:1013): -T^{tau mu}/tau, -3 T^{tau eta}/tau
@@ -475,6 +482,7 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, 1)
       if (!TWO_D) r += flux_line<THETA1>(z0, z1, a2, z3, z4, cf[2][0], cf[2][1], cf[2][2], cf[2][3], theta, real(0.0));
       r += rx + ry;
       park[n * NT + tid] = r;
+      release(5 + n, hi(r));      // r = the flux divergence of all three directions: it depends on every value of the star
       if (VISC && n >= PTT) {
         // this field's part of A^{i nu} = P (v^i delta^nu_tau - g^{i nu}) - v^i pi^{tau nu} + pi^{i nu}, differenced (B.2-B.5)
         const real gx = wd[0] * (x1 - x3), gy = wd[1] * (y1 - y3), gz = TWO_D ? real(0.0) : wd[2] * (z1 - z3);
