@@ -103,3 +103,26 @@ def test_f32_gpu_config3_physics_2plus1d_and_lattice(vo):
         bad = {k: v for k, v in errs.items() if not v <= TOL_F32}
         assert not bad, (prm["eos"], prm["nz"], bad)
         assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_full_size_runs_are_bit_reproducible(precision):
+    """Regression test of the ring hand-back of the stage kernel: the 128^3 workload, whose 4096 tiles per
+    launch keep every SM busy with as many CTAs as fit (two in single precision), must give bitwise the same fields on every run and no
+    inversion failure.  Before the fix the two-CTA configuration corrupted about one tile per launch, differently each time."""
+    import torch
+    from paper_1608_06577_b200 import vh
+
+    prm, init, _ = inputs.config_3d(newton_rtol=2e-6 if precision == "f32" else 1e-13)
+    runs = []
+    for _ in range(3):
+        s = vh.Solver(prm, precision=precision)
+        s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
+        s.step(3)
+        f = s.get_fields()
+        st = s.status()
+        s.close()
+        assert st["n_inversion_failures"] == 0 and st["n_nonfinite"] == 0
+        runs.append(torch.cat([f["q"].reshape(-1), f["e"].reshape(-1), f["u"].reshape(-1)]))
+    assert torch.equal(runs[0], runs[1]) and torch.equal(runs[0], runs[2])
