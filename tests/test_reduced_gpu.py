@@ -83,3 +83,24 @@ def test_reduced_storage_uses_less_memory_and_restarts(vh, vo):
     for k in ("q", "e", "u"):
         assert torch.equal(fa[k], fb[k]), k
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("dims", [(1, 1, 1), (3, 2, 1), (2, 1, 3), (1, 5, 2), (33, 5, 5)])
+@pytest.mark.parametrize("mode", ["reduced", "f32"])
+def test_degenerate_grids_in_the_other_modes(vh, vo, dims, mode):
+    # grids smaller than a tile, extents of 1 in any direction, ragged tiles: reduced storage (1e-9) and the single-precision build (1e-4)
+    from test_gpu_parity import field_errors
+    prm = inputs.base_params(nx=dims[0], ny=dims[1], nz=dims[2], tau0=0.7, dtau=0.01, newton_rtol=2e-6 if mode == "f32" else 1e-13,
+                             storage=1 if mode == "reduced" else 0)
+    st = inputs.smooth_random_state(prm, seed=3)
+    o = vo.Oracle(prm)
+    o.set_initial(st["e"], st["u"], st["pi"], st["Pi"])
+    o.step(5)
+    s = vh.Solver(prm, precision="f32" if mode == "f32" else "f64")
+    s.set_initial(_t(st["e"]), _t(st["u"]), _t(st["pi"]), _t(st["Pi"]))
+    s.step(5)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields(with_uprev=True).items()}
+    sg = s.status()
+    s.close()
+    assert max(field_errors(o.get_fields(with_uprev=True), fg).values()) <= (1e-4 if mode == "f32" else 1e-9)
+    assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
