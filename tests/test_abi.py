@@ -129,3 +129,22 @@ def test_diagnostic_names_agree_with_the_header_and_the_oracle(vo):
     n = int(re.search(r"#define\s+VH_N_DIAGNOSTICS\s+(\d+)", src).group(1))
     assert n == len(vh.Solver.DIAG_NAMES) == len(vo.DIAG_NAMES) == 10
     assert tuple(vh.Solver.DIAG_NAMES) == tuple(vo.DIAG_NAMES)
+
+
+def test_committed_ncu_metrics_file_is_what_bench_reads():
+    """bench.py takes roofline.traffic, executed_flops_per_cell and fp64_pipe_util from the committed raw ncu CSV: it must hold exactly one
+    RK2 step of the default pipeline (velocity, stage, velocity, stage) with every metric bench.py uses, and plausible magnitudes."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    m = bench.ncu_metrics()
+    assert list(m) == list(bench.LAUNCH_KEYS)
+    ncell = 128 ** 3
+    for key, row in m.items():
+        assert ("velocity" in key) == ("velocity" in row["kernel"])
+        flops = (2 * row["smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"] + row["smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"]
+                 + row["smsp__sass_thread_inst_executed_op_dmul_pred_on.sum"]) / ncell
+        assert 500 < flops < 5000, (key, flops)
+        assert 0.2 < row["sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"] / 100 < 1.0
+        traffic = row["dram__bytes_read.sum"] + row["dram__bytes_write.sum"]
+        assert 1e8 < traffic < 3e9
