@@ -196,3 +196,23 @@ def test_diagonal_shock_tube_and_blast(vh, vo):
     assert_parity(fo, so, fg, sg, tol=1e-6)
     e = fg["e"][0, 0]
     assert np.max(np.abs(e - e.T)) <= 1e-11 * np.max(e) and np.max(np.abs(e - e[:, ::-1])) <= 1e-11 * np.max(e)
+
+
+@pytest.mark.parametrize("mode", ["paper_physics", "reduced_storage"])
+def test_full_size_other_modes_sampled_subbox(vh, vo, mode):
+    """128^3 in the launch configuration bench.py times for its labelled extra lines: the paper's own physics (lattice EOS, Eq. 17 zeta/s) and the
+    reduced-storage mode; 5 steps, one 56^3 oracle sub-box around the hottest cell with a 20-cell halo (4 cells per step)."""
+    over = dict(eos=2, zeta_model=3, zeta_amp=1.0, zeta_T0=0.2 / inputs.HBARC) if mode == "paper_physics" else dict(storage=1)
+    prm, init, _ = inputs.config_3d(**over)
+    s = vh.Solver(prm)
+    s.set_initial(_t(init["e"]), _t(init["u"]))
+    s.step(5)
+    fg = {k: v.cpu().numpy() for k, v in s.get_fields().items()}
+    sg = s.status()
+    s.close()
+    assert sg["n_inversion_failures"] == 0 and sg["n_nonfinite"] == 0
+    B, H = 56, 20
+    kz, ky, kx = np.unravel_index(np.argmax(init["e"][0]), init["e"][0].shape)
+    clamp = lambda c: int(min(max(c - B // 2, 0), 128 - B))
+    worst = _subbox_worst(vo, prm, init, fg, [(clamp(kx), clamp(ky), clamp(kz))], B, H, 5)
+    assert worst <= TOL, worst
