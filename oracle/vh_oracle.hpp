@@ -248,7 +248,10 @@ template <class R> class Solver {
     size_t np = (size_t)P.nx * P.ny * P.nz;
     for (int k = 0; k < P.nz; ++k) for (int j = 0; j < P.ny; ++j) for (int i = 0; i < P.nx; ++i) {
       size_t c = (size_t)i + (size_t)P.nx * ((size_t)j + (size_t)P.ny * k);
-      for (int m = 0; m < 4; ++m) up[m][idx(i + 2, j + 2, k + 2)] = up_in[m * np + c];
+      size_t s = idx(i + 2, j + 2, k + 2);
+      for (int m = 0; m < 4; ++m) up[m][s] = up_in[m * np + c];
+      // reduced storage: u^tau is not state - it is always the normalisation at the time level the velocity belongs to (here tau0 - dtau)
+      if (reduced()) up[0][s] = sqrt(R(1) + up[1][s] * up[1][s] + up[2][s] * up[2][s] + tau2(R(P.tau0 - P.dtau)) * up[3][s] * up[3][s]);
     }
   }
 

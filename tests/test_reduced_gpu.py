@@ -14,12 +14,16 @@ def _t(a):
     return None if a is None else torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device="cuda:0")
 
 
-def _pair(vh, vo, prm, st, n_steps):
+def _pair(vh, vo, prm, st, n_steps, uprev=None):
     o = vo.Oracle(prm)
     o.set_initial(st["e"], st["u"], st.get("pi"), st.get("Pi"))
+    if uprev is not None:
+        o.set_uprev(uprev)
     o.step(n_steps)
     s = vh.Solver(prm)
     s.set_initial(_t(st["e"]), _t(st["u"]), _t(st.get("pi")), _t(st.get("Pi")))
+    if uprev is not None:
+        s.set_uprev(_t(uprev))
     s.step(n_steps)
     fg = {k: v.cpu().numpy() for k, v in s.get_fields(with_uprev=True).items()}
     sg = s.status()
@@ -30,7 +34,9 @@ def _pair(vh, vo, prm, st, n_steps):
 def test_reduced_generic_state_3d_and_constraints(vh, vo):
     prm = inputs.base_params(nx=36, ny=12, nz=6, dx=0.12, dy=0.1, dz=0.15, tau0=0.8, dtau=0.02, storage=1)
     st = inputs.smooth_random_state(prm, seed=21)
-    fo, so, fg, sg = _pair(vh, vo, prm, st, 10)
+    up = st["u"] * 1.0
+    up[1:] *= 0.97      # u^{n-1} != u^n: the time derivatives of the sources are exercised from the first step (u^tau of it is not state)
+    fo, so, fg, sg = _pair(vh, vo, prm, st, 10, uprev=up)
     assert so["n_inversion_failures"] == 0
     assert_parity(fo, so, fg, sg)
     # the exported tensor satisfies Eqs. 47-51 to rounding (dense check as in tests/test_oracle_reduced.py)
