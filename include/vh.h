@@ -88,6 +88,23 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
 /* Advance n_steps full RK2 steps (program-flow steps 1-9, :503-529).  Asynchronous on the handle's stream.             */
 int vh_step(vh_handle* h, int n_steps);
 
+/* Slab decomposition along eta (8(f) NEXT-4; the paper's own multi-GPU outlook is independent events, :899).  A caller that owns
+ * one eta-slab of a larger grid takes the RK2 step in four parts and exchanges boundary planes with the owners of the neighbouring slabs
+ * in between (paper_1608_06577_b200/vh.py: SlabSolver does this with torch.distributed send / recv, NCCL over NVLink between GPUs):
+ *   part 0: velocity kernel of stage 1     -> exchange what = 0 (the state velocity of the eta direction at the slab faces, one plane)
+ *   part 1: stage kernel of stage 1        -> exchange what = 1 (the new state q*, e*, p*, u*: two planes x 21 arrays per face)
+ *   part 2: velocity kernel of stage 2     -> exchange what = 0
+ *   part 3: stage kernel of stage 2, buffer rotation, step counter -> exchange what = 1
+ * (and one exchange of what = 1 after vh_set_initial / vh_set_state).  vh_halo_export copies the slab's outermost PHYSICAL planes at a face
+ * (side 0: low eta, 1: high eta) into buf; vh_halo_import writes buf into the GHOST planes beyond that face, replacing the outflow copies
+ * (Eqs. 75-76) the kernels put there - a face without a neighbour simply keeps them.  buf: DEVICE memory of vh_halo_size doubles (whole
+ * padded planes, always double).  Asynchronous on the handle's stream.  Default pipeline, 3+1d, n_batch = 1 only (VH_ERR_STATE otherwise);
+ * the result is bit-identical to a single handle over the whole grid.                                                                     */
+int vh_step_part(vh_handle* h, int part);
+int vh_halo_size(vh_handle* h, int what, long long* n_doubles);
+int vh_halo_export(vh_handle* h, int what, int side, double* buf_device);
+int vh_halo_import(vh_handle* h, int what, int side, const double* buf_device);
+
 /* Same as vh_step, but brackets each of the four launches of a step (default pipeline: velocity kernel 1, stage kernel 1,
  * velocity kernel 2, stage kernel 2; kernel variant 1: stage 1, ghost 1, stage 2, ghost 2) with CUDA events
  * on the handle's stream and returns their mean durations in milliseconds in ms4[0..3] (for per-kernel roofline numbers;

@@ -103,21 +103,21 @@ static int check_params(const vh_params* p, std::string& why) {
 // ------------------------------------------------------------------------------------------------ dispatch
 #define debug_sync vh_debug_sync
 // one Euler stage with the handle's kernel variant: the launch units are compiled per (EOS, viscous, Milne) combination
-static cudaError_t launch_stage_any(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+static cudaError_t launch_stage_any(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid, int part = 0) {
   const int phys = (h->prm.physics != 0) ? ((h->prm.geometry == 0) ? 0 : 3) : ((h->prm.geometry == 0) ? 1 : 2);
   switch (h->prm.eos + 3 * phys) {
-    case 0: return vh_launch_stage_combo0(h, stage, A, mid);
-    case 1: return vh_launch_stage_combo1(h, stage, A, mid);
-    case 2: return vh_launch_stage_combo2(h, stage, A, mid);
-    case 3: return vh_launch_stage_combo3(h, stage, A, mid);
-    case 4: return vh_launch_stage_combo4(h, stage, A, mid);
-    case 5: return vh_launch_stage_combo5(h, stage, A, mid);
-    case 6: return vh_launch_stage_combo6(h, stage, A, mid);
-    case 7: return vh_launch_stage_combo7(h, stage, A, mid);
-    case 8: return vh_launch_stage_combo8(h, stage, A, mid);
-    case 9: return vh_launch_stage_combo9(h, stage, A, mid);
-    case 10: return vh_launch_stage_combo10(h, stage, A, mid);
-    default: return vh_launch_stage_combo11(h, stage, A, mid);
+    case 0: return vh_launch_stage_combo0(h, stage, A, mid, part);
+    case 1: return vh_launch_stage_combo1(h, stage, A, mid, part);
+    case 2: return vh_launch_stage_combo2(h, stage, A, mid, part);
+    case 3: return vh_launch_stage_combo3(h, stage, A, mid, part);
+    case 4: return vh_launch_stage_combo4(h, stage, A, mid, part);
+    case 5: return vh_launch_stage_combo5(h, stage, A, mid, part);
+    case 6: return vh_launch_stage_combo6(h, stage, A, mid, part);
+    case 7: return vh_launch_stage_combo7(h, stage, A, mid, part);
+    case 8: return vh_launch_stage_combo8(h, stage, A, mid, part);
+    case 9: return vh_launch_stage_combo9(h, stage, A, mid, part);
+    case 10: return vh_launch_stage_combo10(h, stage, A, mid, part);
+    default: return vh_launch_stage_combo11(h, stage, A, mid, part);
   }
 }
 
@@ -339,6 +339,8 @@ int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double
   CUDA_TRY(h, cudaGetLastError());
   CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
   h->n_steps = 0;
+  h->next_part = 0;
+  h->cur[0] = h->q[0]; h->cur[1] = h->e[0]; h->cur[2] = h->p[0]; h->cur[3] = h->u[0];
   h->uprev_initial = true;
   int rc = reset_counters(h);
   if (rc) return rc;
@@ -385,6 +387,8 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
   CUDA_TRY(h, cudaGetLastError());
   CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
   h->n_steps = n_steps_done;
+  h->next_part = 0;
+  h->cur[0] = h->q[0]; h->cur[1] = h->e[0]; h->cur[2] = h->p[0]; h->cur[3] = h->u[0];
   int rc = reset_counters(h);
   if (rc) return rc;
   CUDA_TRY(h, reset_regulation_map(h));
@@ -480,13 +484,95 @@ static int one_step(vh_handle* h, cudaEvent_t* ev) {
   real* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;
   real* qn = h->q[2]; h->q[2] = h->q[0]; h->q[0] = qn;
   h->n_steps++;
+  h->cur[0] = h->q[0]; h->cur[1] = h->e[0]; h->cur[2] = h->p[0]; h->cur[3] = h->u[0];
   return VH_OK;
+}
+
+// ---- eta-slab decomposition: the step in four parts, boundary planes in between
+static int slab_checks(vh_handle* h, const char* who) {
+  if (!h->initialised) return fail(h, VH_ERR_STATE, std::string(who) + " before vh_set_initial");
+  if (h->variant != 0 || h->reduced || h->two_d || h->P.n_batch != 1 || h->P.nz < 2)
+    return fail(h, VH_ERR_STATE, std::string(who) + " needs the default pipeline (variant 0, storage 0), a 3+1d grid with nz >= 2 and n_batch = 1");
+  return VH_OK;
+}
+
+int vh_step_part(vh_handle* h, int part) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
+  if (int rc = slab_checks(h, "vh_step_part")) return rc;
+  if (part != h->next_part) return fail(h, VH_ERR_STATE, "vh_step_part: the parts of a step run in the order 0, 1, 2, 3 (next is " + std::to_string(h->next_part) + ")");
+  const double t = h->prm.tau0 + (double)h->n_steps * h->prm.dtau, t1 = t + h->prm.dtau;
+  StageArgs A;
+  A.cnt = h->cnt;
+  if (part < 2) {
+    A.q_in = h->q[0]; A.e_in = h->e[0]; A.p_in = h->p[0]; A.u_in = h->u[0]; A.u_prev = h->u[1]; A.q_n = nullptr;
+    A.q_out = h->q[1]; A.e_out = h->e[1]; A.p_out = h->p[1]; A.u_out = h->u[2]; A.t = t; A.t_post = t1; A.regfac = nullptr;
+  } else {
+    A.q_in = h->q[1]; A.e_in = h->e[1]; A.p_in = h->p[1]; A.u_in = h->u[2]; A.u_prev = h->u[0]; A.q_n = h->q[0];
+    A.q_out = h->q[2]; A.e_out = h->e[0]; A.p_out = h->p[0]; A.u_out = h->u[1]; A.t = t1; A.t_post = t1; A.regfac = h->regfac;
+  }
+  CUDA_TRY(h, launch_stage_any(h, part < 2 ? 1 : 2, A, nullptr, (part % 2 == 0) ? 1 : 2));
+  if (part == 1) { h->cur[0] = h->q[1]; h->cur[1] = h->e[1]; h->cur[2] = h->p[1]; h->cur[3] = h->u[2]; }
+  if (part == 3) {
+    real* un = h->u[1]; h->u[1] = h->u[0]; h->u[0] = un;
+    real* qn = h->q[2]; h->q[2] = h->q[0]; h->q[0] = qn;
+    h->n_steps++;
+    h->cur[0] = h->q[0]; h->cur[1] = h->e[0]; h->cur[2] = h->p[0]; h->cur[3] = h->u[0];
+  }
+  h->next_part = (part + 1) % 4;
+  return VH_OK;
+}
+
+int vh_halo_size(vh_handle* h, int what, long long* n_doubles) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  if ((what != 0 && what != 1) || !n_doubles) return fail(h, VH_ERR_ARG, "what must be 0 (state velocity) or 1 (state); n_doubles != NULL");
+  *n_doubles = (what == 0 ? 1LL : 2LL * 21) * h->P.plane;
+  return VH_OK;
+}
+
+static int halo_copy(vh_handle* h, int what, int side, double* buf, bool exporting) {
+  if (int rc = slab_checks(h, exporting ? "vh_halo_export" : "vh_halo_import")) return rc;
+  if ((what != 0 && what != 1) || (side != 0 && side != 1) || !buf) return fail(h, VH_ERR_ARG, "what in {0, 1}, side in {0, 1}, buf != NULL required");
+  const DevParams& P = h->P;
+  const long long fs = P.fstride;
+  PlaneArgs G;
+  if (what == 0) {
+    // low face: the lower neighbour needs v of the state at the low face of my first plane (vL, eta direction) as its ghost plane nz, and gives me
+    // v of the state at the high face of its last plane (vR) for my ghost plane -1; high face: the mirror image
+    G.n_arr = 1; G.n_planes = 1;
+    const bool lowface = (side == 0);
+    G.arr[0] = (exporting == lowface) ? h->vL + 2 * fs : h->vR + 2 * fs;
+    G.z0 = exporting ? (lowface ? 2 : P.nz + 1) : (lowface ? 1 : P.nz + 2);
+  } else {
+    G.n_arr = 21; G.n_planes = 2;
+    for (int n = 0; n < 15; ++n) G.arr[n] = h->cur[0] + n * fs;
+    G.arr[15] = h->cur[1]; G.arr[16] = h->cur[2];
+    for (int n = 0; n < 4; ++n) G.arr[17 + n] = h->cur[3] + n * fs;
+    G.z0 = exporting ? (side == 0 ? 2 : P.nz) : (side == 0 ? 0 : P.nz + 2);
+  }
+  dim3 grid((unsigned)((P.plane + 255) / 256), G.n_arr * G.n_planes);
+  if (exporting) plane_kernel<true><<<grid, 256, 0, h->stream>>>(P, G, buf);
+  else plane_kernel<false><<<grid, 256, 0, h->stream>>>(P, G, buf);
+  h->launches++;
+  CUDA_TRY(h, cudaGetLastError());
+  return VH_OK;
+}
+int vh_halo_export(vh_handle* h, int what, int side, double* buf_device) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
+  return halo_copy(h, what, side, buf_device, true);
+}
+int vh_halo_import(vh_handle* h, int what, int side, const double* buf_device) {
+  if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
+  VH_ENTER(h);
+  return halo_copy(h, what, side, const_cast<double*>(buf_device), false);
 }
 
 int vh_step(vh_handle* h, int n_steps) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_step before vh_set_initial");
+  if (h->next_part != 0) return fail(h, VH_ERR_STATE, "vh_step in the middle of a step taken with vh_step_part");
   if (n_steps < 0) return fail(h, VH_ERR_ARG, "n_steps must be >= 0");
   for (int it = 0; it < n_steps; ++it) {
     int rc = one_step(h, nullptr);

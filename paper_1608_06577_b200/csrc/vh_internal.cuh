@@ -36,6 +36,8 @@ struct vh_handle {
   long long launches = 0;
   bool initialised = false;
   bool two_d = false;
+  vh::real* cur[4] = {nullptr, nullptr, nullptr, nullptr};   // q, e, p, u of the most recently written state (what vh_halo_export(what = 1) reads)
+  int next_part = 0;                 // vh_step_part: the part of the RK2 step that comes next (0..3)
   bool reduced = false;              // vh_params.storage == 1: 10 q + 3 u arrays per time level (vh_kernels5.cuh), own stage kernel
   bool uprev_initial = true;         // u^{n-1} is the copy of u^0 made by vh_set_initial (reduced storage: its u^tau is normalised at tau0, not tau0 - dtau)
   int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
@@ -66,8 +68,9 @@ inline cudaError_t vh_opt_in_smem(vh_handle* h, const void* kern, size_t smem) {
 }
 
 // One Euler stage (kernels of the handle's variant) for one combination of template parameters; defined in vh_launch.cu.
+// part: 0 = both kernels of the stage, 1 = velocity kernel only, 2 = stage kernel only (default pipeline; vh_step_part).
 // combo = eos + 3 * (0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian, 3: viscous Cartesian), eos = 0, 1, 2.  mid (optional) is recorded between the two launches.
-#define VH_DECLARE_COMBO(K) cudaError_t vh_launch_stage_combo##K(vh_handle* h, int stage, const vh::StageArgs& A, cudaEvent_t mid);
+#define VH_DECLARE_COMBO(K) cudaError_t vh_launch_stage_combo##K(vh_handle* h, int stage, const vh::StageArgs& A, cudaEvent_t mid, int part);
 VH_DECLARE_COMBO(0) VH_DECLARE_COMBO(1) VH_DECLARE_COMBO(2) VH_DECLARE_COMBO(3) VH_DECLARE_COMBO(4) VH_DECLARE_COMBO(5)
 VH_DECLARE_COMBO(6) VH_DECLARE_COMBO(7) VH_DECLARE_COMBO(8) VH_DECLARE_COMBO(9) VH_DECLARE_COMBO(10) VH_DECLARE_COMBO(11)
 #undef VH_DECLARE_COMBO

@@ -546,6 +546,19 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(const __grid_constant_
   }
 }
 
+// Whole padded eta planes of up to 21 arrays <-> a contiguous buffer of doubles (vh_halo_export / vh_halo_import: the exchange of an eta-slab
+// decomposition).  buf[(a * n_planes + pl) * plane + w]; z0 = first padded plane index.
+struct PlaneArgs { real* arr[21]; int n_arr; int z0; int n_planes; };
+template <bool EXPORT>
+__global__ void __launch_bounds__(256) plane_kernel(const __grid_constant__ DevParams P, const __grid_constant__ PlaneArgs G, double* __restrict__ buf) {
+  const long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= P.plane) return;
+  const int pl = blockIdx.y % G.n_planes, a = blockIdx.y / G.n_planes;
+  real* f = G.arr[a] + (long long)(G.z0 + pl) * P.plane + w;
+  double* b = buf + ((long long)a * G.n_planes + pl) * P.plane + w;
+  if (EXPORT) *b = (double)*f; else *f = (real)*b;
+}
+
 static __global__ void __launch_bounds__(256) fill_kernel(real* __restrict__ a, long long n, real v) {
   for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < n; w += (long long)gridDim.x * blockDim.x) a[w] = v;
 }

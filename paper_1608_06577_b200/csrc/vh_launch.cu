@@ -67,10 +67,10 @@ static cudaError_t launch_tile_kernel(vh_handle* h, const TileArgs& A) {
   return debug_sync(h, STAGE == 1 ? "stage 1 tile kernel" : "stage 2 tile kernel");
 }
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
-static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid) {
+static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cudaEvent_t mid, int part) {
   const DevParams& P = h->P;
   const long long fs = P.fstride;
-  {
+  if (part != 2) {      // part: 0 both kernels, 1 velocity kernel only, 2 stage kernel only (vh_step_part)
     using V = VTile<TWO_D>;
     constexpr size_t vsmem = vtile_smem_bytes<TWO_D, VISC>();
     auto vkern = velocity_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1>;
@@ -83,24 +83,25 @@ static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cu
     if (e != cudaSuccess) return e;
   }
   if (mid) cudaEventRecord(mid, h->stream);
+  if (part == 1) return cudaSuccess;
   TileArgs A{S.q_in, S.e_in, S.p_in, S.u_in, S.u_prev, S.q_n, h->vL, h->vR, S.q_out, S.e_out, S.p_out, S.u_out, S.cnt, S.t, S.t_post,
              (int)((S.q_in - h->pool) / fs), (int)((S.u_in - h->pool) / fs), (int)((S.p_in - h->pool) / fs), S.regfac};
   return (stage == 1) ? launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 1>(h, A) : launch_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1, 2>(h, A);
 }
 template <int EOS, bool VISC, bool MILNE>
-static cudaError_t launch_tile_d(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+static cudaError_t launch_tile_d(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid, int part) {
   const bool th1 = h->prm.minmod_theta == 1.0;
-  if (h->two_d) return th1 ? launch_tile_t<EOS, VISC, MILNE, true, true>(h, stage, A, mid) : launch_tile_t<EOS, VISC, MILNE, true, false>(h, stage, A, mid);
-  return th1 ? launch_tile_t<EOS, VISC, MILNE, false, true>(h, stage, A, mid) : launch_tile_t<EOS, VISC, MILNE, false, false>(h, stage, A, mid);
+  if (h->two_d) return th1 ? launch_tile_t<EOS, VISC, MILNE, true, true>(h, stage, A, mid, part) : launch_tile_t<EOS, VISC, MILNE, true, false>(h, stage, A, mid, part);
+  return th1 ? launch_tile_t<EOS, VISC, MILNE, false, true>(h, stage, A, mid, part) : launch_tile_t<EOS, VISC, MILNE, false, false>(h, stage, A, mid, part);
 }
 
 #define VH_CAT2(a, b) a##b
 #define VH_CAT(a, b) VH_CAT2(a, b)
-cudaError_t VH_CAT(vh_launch_stage_combo, VH_COMBO)(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid) {
+cudaError_t VH_CAT(vh_launch_stage_combo, VH_COMBO)(vh_handle* h, int stage, const StageArgs& A, cudaEvent_t mid, int part) {
   constexpr int EOS = VH_COMBO % 3;
   constexpr int G = VH_COMBO / 3;      // 0: viscous Milne, 1: ideal Milne, 2: ideal Cartesian, 3: viscous Cartesian
   constexpr bool VISC = (G == 0) || (G == 3), MILNE = (G < 2);
-  if (h->variant == 0) return launch_tile_d<EOS, VISC, MILNE>(h, stage, A, mid);
+  if (h->variant == 0) return launch_tile_d<EOS, VISC, MILNE>(h, stage, A, mid, part);
   if (h->variant == 2) return launch_split_d<EOS, VISC, MILNE>(h, stage, A, mid);
   return launch_stage_d<EOS, VISC, MILNE>(h, stage, A);
 }

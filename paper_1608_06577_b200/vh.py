@@ -33,7 +33,7 @@ class vh_params(C.Structure):
 
 
 # every symbol include/vh.h declares
-EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_enable_regulation_map", "vh_get_regulation_map", "vh_run_until", "vh_eos_table", "vh_launch_count",
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_part", "vh_halo_size", "vh_halo_export", "vh_halo_import", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_enable_regulation_map", "vh_get_regulation_map", "vh_run_until", "vh_eos_table", "vh_launch_count",
            "vh_set_kernel_variant", "vh_measure_peaks", "vh_measure_fp32_peak", "vh_last_error", "vh_destroy"]
 
 _lib = None
@@ -58,6 +58,10 @@ def load_library(precision="f64"):
     L.vh_set_uprev.argtypes = [vp, vp, C.c_int]
     L.vh_set_state.argtypes = [vp, vp, vp, vp, vp, C.c_longlong, C.c_int]
     L.vh_step.argtypes = [vp, C.c_int]
+    L.vh_step_part.argtypes = [vp, C.c_int]
+    L.vh_halo_size.argtypes = [vp, C.c_int, C.POINTER(C.c_longlong)]
+    L.vh_halo_export.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.vh_halo_import.argtypes = [vp, C.c_int, C.c_int, vp]
     L.vh_step_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.vh_get_fields.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
     L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
@@ -186,6 +190,20 @@ class Solver:
     def step(self, n=1):
         self._check(self.L.vh_step(self.h, int(n)), "vh_step")
 
+    def step_part(self, part):
+        self._check(self.L.vh_step_part(self.h, int(part)), "vh_step_part")
+
+    def halo_size(self, what):
+        n = C.c_longlong()
+        self._check(self.L.vh_halo_size(self.h, int(what), C.byref(n)), "vh_halo_size")
+        return n.value
+
+    def halo_export(self, what, side, buf):
+        self._check(self.L.vh_halo_export(self.h, int(what), int(side), _ptr(buf)), "vh_halo_export")
+
+    def halo_import(self, what, side, buf):
+        self._check(self.L.vh_halo_import(self.h, int(what), int(side), _ptr(buf)), "vh_halo_import")
+
     def step_profile(self, n=1):
         """n steps with CUDA events around each of the four launches of a step; mean ms per launch, keyed by kernel:
         variants 0, 2: velocity1, stage1, velocity2, stage2; variant 1 and reduced storage: stage1, ghost1, stage2, ghost2."""
@@ -301,3 +319,82 @@ def measure_fp32_peak(repeats=10, stream=None):
         msg = L.vh_last_error(None)
         raise VHError("vh_measure_fp32_peak failed (%d): %s" % (rc, msg.decode() if msg else "?"))
     return a.value
+
+
+class SlabSolver:
+    """One eta-slab of a larger 3+1d grid per rank of a torch.distributed group: rank r owns planes
+    [r nz/W, (r+1) nz/W) and exchanges two boundary planes of the 21 state arrays (and one plane of state velocities) with its neighbours after
+    every kernel of the step - neighbour send / recv, NCCL over NVLink 5 / NVSwitch between GPUs (device buffers go to the backend as they are);
+    with the gloo backend the planes are staged through host memory.  Argument marshalling and the exchange only: every step of the path runs in
+    the library's kernels, and the result is bit-identical to a single Solver over the whole grid."""
+
+    def __init__(self, params: dict, group=None, device="cuda:0", precision="f64"):
+        import torch
+        import torch.distributed as dist
+
+        self.torch, self.dist, self.group = torch, dist, group
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        nz = params["nz"]
+        if nz % self.world or nz // self.world < 2:
+            raise VHError("nz must be a multiple of the number of ranks with at least two planes per slab")
+        self.nzl = nz // self.world
+        self.z0 = self.rank * self.nzl
+        local = dict(params, nz=self.nzl)
+        self.s = Solver(local, device=device, precision=precision)
+        self.device = self.s.device
+        self.host_staging = dist.get_backend(group) == "gloo"
+        self.buf = {w: [[torch.empty(self.s.halo_size(w), dtype=torch.float64, device=self.device) for _ in range(2)] for _ in range(2)] for w in (0, 1)}
+        self.lo = self.rank - 1 if self.rank > 0 else None
+        self.hi = self.rank + 1 if self.rank + 1 < self.world else None
+
+    def _slab(self, a):
+        return None if a is None else a[..., self.z0:self.z0 + self.nzl, :, :].contiguous()
+
+    def _exchange(self, what):
+        """send my outermost physical planes at each face to the neighbour beyond it, receive its planes into my ghost planes"""
+        dist, torch = self.dist, self.torch
+        ops, staged = [], []
+        for side, nb in ((0, self.lo), (1, self.hi)):
+            if nb is None:
+                continue
+            out, inp = self.buf[what][side]
+            self.s.halo_export(what, side, out)
+            self.s.stream.synchronize()
+            if self.host_staging:
+                out_h, inp_h = out.cpu(), torch.empty(inp.shape, dtype=inp.dtype)
+                ops += [dist.P2POp(dist.isend, out_h, nb, self.group), dist.P2POp(dist.irecv, inp_h, nb, self.group)]
+                staged.append((side, inp, inp_h))
+            else:
+                ops += [dist.P2POp(dist.isend, out, nb, self.group), dist.P2POp(dist.irecv, inp, nb, self.group)]
+                staged.append((side, inp, None))
+        if ops:
+            for r in dist.batch_isend_irecv(ops):
+                r.wait()
+        for side, inp, inp_h in staged:
+            if inp_h is not None:
+                inp.copy_(inp_h)
+            self.s.halo_import(what, side, inp)
+
+    def set_initial(self, e, u4, pi10=None, Pi=None):
+        """global arrays [..., nz, ny, nx]; every rank takes its own planes"""
+        self.s.set_initial(self._slab(e), self._slab(u4), self._slab(pi10), self._slab(Pi))
+        self._exchange(1)
+
+    def set_uprev(self, u4_prev):
+        self.s.set_uprev(self._slab(u4_prev))
+
+    def step(self, n=1):
+        for _ in range(int(n)):
+            for part in range(4):
+                self.s.step_part(part)
+                self._exchange(part % 2)
+
+    def get_fields(self, **kw):
+        """this rank's slab"""
+        return self.s.get_fields(**kw)
+
+    def status(self):
+        return self.s.status()
+
+    def close(self):
+        self.s.close()
