@@ -264,6 +264,53 @@ def run_reference(args):
     return 0
 
 
+def run_slab(args, vh, torch, dist, dev, rank, world, local):
+    """ONE grid split into eta-slabs, one per rank, neighbour exchange of boundary planes after every kernel (vh.SlabSolver):
+    strong scaling.  A labelled extra line - the default N > 1 mode stays independent replicas (north_star: no sharding).  The same event on
+    every rank (seed of rank 0); time = max over ranks of the CUDA-event time of K steps including the exchanges."""
+    if dist is None:
+        import torch.distributed as dist      # a 1-rank group: SlabSolver then owns the whole grid and exchanges nothing
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29533")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    prm, init = workload(0, args.physics, args.workload)
+    if args.precision == "f32":
+        prm["newton_rtol"] = 2e-6
+    W, K = max(args.warmup, 3), args.steps
+    s = vh.SlabSolver(prm, device=dev, precision=args.precision)
+    s.set_initial(torch.as_tensor(init["e"], device=dev), torch.as_tensor(init["u"], device=dev))
+    s.step(W)
+    torch.cuda.synchronize(); dist.barrier(); torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = s.s.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    s.step(K)
+    ev1.record()
+    torch.cuda.synchronize(); dist.barrier(); torch.cuda.synchronize()
+    launches = s.s.launch_count() - n0
+    clocks = sampler.stop()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), dist, dev)
+    st = s.status()
+    fails = torch.tensor([float(st["n_inversion_failures"])], device=dev, dtype=torch.float64)
+    dist.all_reduce(fails)
+    halo = (s.s.halo_size(0) + s.s.halo_size(1)) * 8 * 2          # bytes a rank sends per face per step (two exchanges of each kind)
+    s.close()
+    ncell = prm["nx"] * prm["ny"] * prm["nz"]
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC.replace("at 128^3 viscous", "at %dx%dx%d viscous, ONE grid in %d eta-slabs" % (prm["nx"], prm["ny"], prm["nz"], world)),
+            "value": ncell * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "config": {"workload": "labelled extra line (the default N > 1 mode is independent replicas): %s split along eta, %d planes per rank, neighbour "
+                                   "send/recv of 2 planes x 21 arrays + 1 plane of state velocities per face after every kernel (%s backend)"
+                                   % (args.workload, prm["nz"] // world, dist.get_backend()), "halo_bytes_per_face_per_step": halo},
+            "gpu_launches": int(launches), "clocks": clocks, "status": {"n_inversion_failures": int(fails.item())}}))
+    dist.barrier()
+    dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -277,6 +324,9 @@ def main():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: the single-precision build (libvh_f32.so; SURVEY 8(f) NEXT-3), a labelled extra line")
     ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config5"],
                     help="config4 (256 batched 2+1d events) / config5 (512x512x128): labelled extra lines; the default is the BASELINE.json metric")
+    ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (the default: BASELINE.json north_star fixes one GPU, no sharding) or ONE grid split into eta-slabs "
+                         "with neighbour exchange over NCCL (vh.SlabSolver; SURVEY 8(e), strong scaling; a labelled extra line)")
     ap.add_argument("--storage", type=int, default=0, choices=[0, 1], help="1: reduced-storage mode (5 pi + 3 u components, PAPER.md:476; SURVEY 8(f) NEXT-3), a labelled extra line")
     ap.add_argument("--physics", default="config3", choices=["config3", "paper"], help="paper: lattice EOS + Eq. 17 zeta/s on the config-3 grid")
     args = ap.parse_args()
@@ -302,6 +352,8 @@ def main():
     W = max(args.warmup, 3)
     K = args.steps
 
+    if args.decomposition == "slab":
+        return run_slab(args, vh, torch, dist, dev, rank, world, local)
     prm, init = workload(rank, args.physics, args.workload)
     other = (args.workload != "config3")
     f32 = (args.precision == "f32")
