@@ -22,6 +22,10 @@
  * All work of vh_set_initial / vh_step / vh_get_fields is enqueued on the CUDA stream given to vh_create;
  * vh_step is asynchronous; vh_get_fields and vh_get_status synchronise that stream before returning.
  * There is no CPU fallback: without a CUDA device vh_create fails with VH_ERR_CUDA.
+ *
+ * Two libraries export this ABI: libvh.so computes in double precision (the product; everything BASELINE.json measures) and libvh_f32.so
+ * is the same source compiled with a float scalar (the paper's own runs are single precision).  Array arguments are double
+ * in both; libvh_f32.so converts on the way in and out and refuses a Newton tolerance below 1e-6.
  */
 #ifndef VH_H_
 #define VH_H_
@@ -66,7 +70,7 @@ typedef struct {
 } vh_params;
 
 /* Create a solver for the grid / physics in *p on the current CUDA device.  cuda_stream: a cudaStream_t (may be NULL =
- * default stream).  Allocates 67 padded SoA arrays (3 x 15 q, 3 x 4 u, 2 x e, 2 x p; :470-476 plus the ping-pong copy of
+ * default stream).  Allocates 67 padded SoA arrays (43 with storage = 1) (3 x 15 q, 3 x 4 u, 2 x e, 2 x p; :470-476 plus the ping-pong copy of
  * e, p needed because inversion is fused into the stage kernel; and the 6 state-velocity arrays the velocity kernel hands
  * to the stage kernel).  The handle belongs to that device: every later call switches to it.  *out is set only on success. */
 int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out);
