@@ -106,15 +106,20 @@ def test_f32_gpu_config3_physics_2plus1d_and_lattice(vo):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("workload", ["3d", "batched2d"])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
-def test_full_size_runs_are_bit_reproducible(precision):
+def test_full_size_runs_are_bit_reproducible(precision, workload):
     """Regression test of the ring hand-back of the stage kernel: the 128^3 workload, whose 4096 tiles per
     launch keep every SM busy with as many CTAs as fit (two in single precision), must give bitwise the same fields on every run and no
     inversion failure.  Before the fix the two-CTA configuration corrupted about one tile per launch, differently each time."""
     import torch
     from paper_1608_06577_b200 import vh
 
-    prm, init, _ = inputs.config_3d(newton_rtol=2e-6 if precision == "f32" else 1e-13)
+    rtol = 2e-6 if precision == "f32" else 1e-13
+    if workload == "3d":
+        prm, init, _ = inputs.config_3d(newton_rtol=rtol)
+    else:       # the 2+1d instantiation of the same kernel: 64 events of 201 x 201 = 5824 tiles per launch
+        prm, init, _ = inputs.config_batched2d(n_batch=64, newton_rtol=rtol)
     runs = []
     for _ in range(3):
         s = vh.Solver(prm, precision=precision)
