@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, TWO_D ? 3 : 6)
     NewtonState SL, SR;
     SL.E = wL[0]; SL.Pi = wL[4]; SL.M2 = wL[1] * wL[1] + wL[2] * wL[2] + t2 * wL[3] * wL[3];     // :339
     SR.E = wR[0]; SR.Pi = wR[4]; SR.M2 = wR[1] * wR[1] + wR[2] * wR[2] + t2 * wR[3] * wR[3];
-    newton_pair<EOS>(P, SL, SR, guess);
+    newton_pair<EOS>(P, SL, SR, guess, guess);
     real vl = wL[d + 1] * SL.rden, vr = wR[d + 1] * SR.rden;      // v^r = M_r/(E + P0 + Pi)  (Eqs. 53-54)
     if (SL.fail) vl = clip_velocity(vl);
     if (SR.fail) vr = clip_velocity(vr);

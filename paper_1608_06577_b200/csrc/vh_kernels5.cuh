@@ -10,6 +10,7 @@
 // One thread per cell, stencils through L1/L2 (the layout of variant 1): this is the memory-saving mode, not the fast path.
 #pragma once
 #include "vh_kernels.cuh"
+#include "vh_math.cuh"
 
 namespace vh {
 
@@ -28,8 +29,8 @@ struct RedArgs {
 // Eqs. 51, 48-50, 47 (Eq. 49 with its typo fixed, R3): out = pi^tt, pi^tx, pi^ty, pi^tn, pi^nn
 __device__ __forceinline__ void dependent_pi(const real v[3], real t2, real pxx, real pxy, real pxn, real pyy, real pyn, real out[5]) {
   const real vx = v[0], vy = v[1], vn = v[2];
-  const real pnn = (pxx * (vx * vx - real(1.0)) + pyy * (vy * vy - real(1.0)) + real(2.0) * pxy * vx * vy + real(2.0) * t2 * (pxn * vx * vn + pyn * vy * vn)) /
-                   (t2 * (real(1.0) - t2 * vn * vn));
+  const real pnn = (pxx * (vx * vx - real(1.0)) + pyy * (vy * vy - real(1.0)) + real(2.0) * pxy * vx * vy + real(2.0) * t2 * (pxn * vx * vn + pyn * vy * vn)) *
+                   rcp_fast(t2 * (real(1.0) - t2 * vn * vn));
   const real ptx = pxx * vx + pxy * vy + t2 * pxn * vn;
   const real pty = pxy * vx + pyy * vy + t2 * pyn * vn;
   const real ptn = pxn * vx + pyn * vy + t2 * pnn * vn;
@@ -42,8 +43,8 @@ __device__ __forceinline__ void load_expanded(const DevParams& P, const real* __
                                               real uf[4]) {
   const long long fs = P.fstride;
   uf[1] = u[c]; uf[2] = u[fs + c]; uf[3] = u[2 * fs + c];
-  uf[0] = sqrt(real(1.0) + uf[1] * uf[1] + uf[2] * uf[2] + t2 * uf[3] * uf[3]);
-  const real iut = real(1.0) / uf[0];
+  uf[0] = sqrt_fast(real(1.0) + uf[1] * uf[1] + uf[2] * uf[2] + t2 * uf[3] * uf[3]);
+  const real iut = rcp_fast(uf[0]);
   const real v[3] = {uf[1] * iut, uf[2] * iut, uf[3] * iut};
 #pragma unroll
   for (int n = 0; n < 4; ++n) qf[n] = q[n * fs + c];
@@ -129,10 +130,19 @@ __global__ void __launch_bounds__(128) stage_reduced_kernel(const __grid_constan
     recon4(BPI, Pi4);
     const bool count_hi = ext[d] > 1, count_lo = ext[d] > 1 && pos[d] == 0;
     real v[4];
-    v[0] = state_velocity<EOS, MILNE>(P, E[0], Mx[0], My[0], Mn[0], Pi4[0], t2, e5[1], d, count_hi, nfail);
-    v[1] = state_velocity<EOS, MILNE>(P, E[1], Mx[1], My[1], Mn[1], Pi4[1], t2, e5[2], d, count_hi, nfail);
-    v[2] = state_velocity<EOS, MILNE>(P, E[2], Mx[2], My[2], Mn[2], Pi4[2], t2, e5[0], d, count_lo, nfail);
-    v[3] = state_velocity<EOS, MILNE>(P, E[3], Mx[3], My[3], Mn[3], Pi4[3], t2, e5[1], d, count_lo, nfail);
+    {      // the four states as two pairs through the paired Newton iteration of the default path (same root, cap and tolerance, R6)
+      const real* Mr = (d == 0) ? Mx : ((d == 1) ? My : Mn);
+      NewtonState S[4];
+#pragma unroll
+      for (int m = 0; m < 4; ++m) { S[m].E = E[m]; S[m].Pi = Pi4[m]; S[m].M2 = Mx[m] * Mx[m] + My[m] * My[m] + t2 * Mn[m] * Mn[m]; }
+      newton_pair<EOS>(P, S[0], S[1], e5[1], e5[2]);      // the upper interface: state from this cell, state from the next one
+      newton_pair<EOS>(P, S[2], S[3], e5[0], e5[1]);      // the lower interface
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        v[m] = Mr[m] * S[m].rden;
+        if (S[m].fail) { v[m] = clip_velocity(v[m]); if (m < 2 ? count_hi : count_lo) ++nfail; }
+      }
+    }
     const real ap = fmax(fabs(v[1]), fabs(v[0])), am = fmax(fabs(v[3]), fabs(v[2]));      // Eq. 62
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {

@@ -38,14 +38,15 @@ struct NewtonState {
   bool fail;
 };
 
+// (guessA, guessB: e of the cells the two states were extrapolated from, R6)
 template <int EOS>
-__device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, NewtonState& B, real guess) {
-  const bool gok = (guess > real(0.0)) && isfinite(guess);
+__device__ __forceinline__ void newton_pair(const DevParams& P, NewtonState& A, NewtonState& B, real guessA, real guessB) {
+  const bool gokA = (guessA > real(0.0)) && isfinite(guessA), gokB = (guessB > real(0.0)) && isfinite(guessB);
   // (one finiteness test on the sum: it is finite exactly when E, M2 and Pi all are, short of an overflow that no state reaches)
   bool badA = !(A.E > real(0.0)) || !isfinite(A.E + A.M2 + A.Pi);
   bool badB = !(B.E > real(0.0)) || !isfinite(B.E + B.M2 + B.Pi);
-  A.e = gok ? guess : A.E;
-  B.e = gok ? guess : B.E;
+  A.e = gokA ? guessA : A.E;
+  B.e = gokB ? guessB : B.E;
   bool doneA = badA, doneB = badB, convA = false, convB = false;
   real pA = real(0.0), cA = real(0.0), rA = real(0.0), dA = real(0.0), pB = real(0.0), cB = real(0.0), rB = real(0.0), dB = real(0.0);      // last iterate's P0, cs2, 1/(E + P0 + Pi), correction
   for (int it = 0; it < P.newton_max_iter; ++it) {
