@@ -153,6 +153,39 @@ int vh_get_diagnostic_maps(vh_handle* h, double* maps10, int mem_space);
 int vh_enable_regulation_map(vh_handle* h, int on);
 int vh_get_regulation_map(vh_handle* h, double* map, int mem_space);
 
+/* The ten diagnostics above for a caller that must not allocate device memory - no handle, no cudaMalloc, no cudaFree, no library
+ * routine that allocates.  Who needs this: a host program that has already handed the GPU's free memory to an allocator of its own (a
+ * framework's caching pool, a fixed arena sized at start-up), where a cudaMalloc made behind its back fails or eats into what the pool
+ * thinks it owns; and a time loop that cannot afford the device-wide synchronisation a cudaMalloc / cudaFree implies.  vh_create and the
+ * lazily allocated reduction slots and staging buffers of vh_get_diagnostics / vh_get_diagnostic_maps are out of reach for such callers;
+ * this entry point works directly on the caller's own arrays instead.
+ *
+ * Inputs (all DEVICE pointers on the current device, the layout of vh_get_fields: physical cells only, x fastest, component-major):
+ *   p        grid and physics as for vh_create (same checks; `storage` is ignored - the arrays below are the full set),
+ *   tau      the time of the state (Milne geometry: tau > 0),
+ *   q15, e, u4, u4_prev   15 + 1 + 4 + 4 arrays of np = n_batch*nz*ny*nx doubles (u4_prev = u at tau - dtau; pass u4 twice for an
+ *            initial state).  The pressure is P0(e).  Differences across the edge of the grid use the outflow ghost cells of
+ *            Eqs. 75-76 (:459-464), i.e. the value of the outermost physical cell, exactly as the solver's padded arrays hold them.
+ * Outputs:
+ *   out10    the ten maxima (order of vh_get_diagnostics); out_mem_space 0: HOST pointer, the call copies them out and synchronises the
+ *            stream before returning; 1: DEVICE pointer, the call only enqueues work on cuda_stream,
+ *   maps10   NULL, or a DEVICE pointer to 10*np doubles that receives the ten quantities cell by cell (layout of vh_get_diagnostic_maps).
+ * Results agree with vh_get_diagnostics / vh_get_diagnostic_maps of a handle holding this state (the same per-cell arithmetic; tested to 1e-9).
+ *
+ * Scratch: one kernel; its per-block maxima, the ticket that tells the last block to combine them, and the EOS-2 table live in arrays
+ * compiled into the library (`static __device__`, about 390 KB in total), which every GPU that loads the library holds until the
+ * process exits.  The price is a size limit: np <= VH_NOALLOC_MAX_CELLS (2^20, e.g. 128 x 128 x 64 or 100^3); a larger grid is refused
+ * with VH_ERR_ARG and a message naming both numbers - use a handle and vh_get_diagnostics for it.
+ * First call on a device: looks up the device addresses of those arrays and uploads the EOS-2 table (host work plus one stream
+ * synchronisation, once per device and process).  Make that first call during start-up, and before any stream capture is begun.
+ * Every call on a device shares the same scratch and finds in it what the previous call left; the call clears the ticket itself (an
+ * asynchronous 4-byte memset on cuda_stream), nothing else has to start from zero.  Two calls whose kernels can overlap on one GPU
+ * (different streams, or different host threads on different streams) race on the scratch and give wrong maxima: issue them on one
+ * stream or order them with events.  Runs on the CURRENT device; cuda_stream (NULL = default stream) must belong to it.               */
+#define VH_NOALLOC_MAX_CELLS 1048576
+int vh_diagnostics_noalloc(const vh_params* p, double tau, const double* q15, const double* e, const double* u4, const double* u4_prev,
+                           double* out10, int out_mem_space, double* maps10, void* cuda_stream);
+
 /* Program-flow steps 6-8 (:492-494): advance until T < T_f (fm^-1) everywhere or max_steps steps have been taken, testing the
  * temperature every check_every steps (>= 1) with the reduction of vh_get_diagnostics.  *steps_done (may be NULL) receives the
  * number of steps taken by this call; returns VH_OK in both cases (compare vh_get_diagnostics()[0] with T_f to tell them apart). */

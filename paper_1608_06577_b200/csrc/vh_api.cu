@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -854,3 +855,237 @@ int vh_measure_fp32_peak(void* cuda_stream, int repeats, double* fp32_gflops) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ diagnostics without allocation
+// vh_diagnostics_noalloc (include/vh.h): the ten diagnostics for callers that may not allocate device memory - the host program gave the
+// GPU's free memory to its own pool, or sits in a loop that cannot take the device-wide stall of cudaMalloc / cudaFree.  A variant of
+// diagnostics_kernel (vh_kernels.cuh) that reads the caller's compact arrays and keeps everything it needs beyond them - per-block
+// maxima, the last-block ticket, the EOS-2 table - in the two arrays below.  They are part of the library image: each GPU that loads the
+// library carries them (about 390 KB) until the process exits, and every call on that GPU reuses them.
+namespace vh {
+constexpr int NA_THREADS = 256;                                        // one cell per thread, no grid-stride loop: block b owns cells [256 b, 256 b + 256)
+constexpr int NA_MAX_BLOCKS = VH_NOALLOC_MAX_CELLS / NA_THREADS;        // 4096
+constexpr int NA_RESULT = 10 * NA_MAX_BLOCKS;                          // [0, NA_RESULT): maximum s of block b at s * NA_MAX_BLOCKS + b
+constexpr int NA_TICKET = NA_RESULT + 32;                              // [NA_RESULT, +10): the ten results when out10 is a host pointer
+constexpr int NA_DOUBLES = NA_TICKET + 32;                             // [NA_TICKET]: the ticket (an unsigned int in a 256-byte line of its own)
+static_assert(VH_NOALLOC_MAX_CELLS % NA_THREADS == 0, "the size limit is a whole number of blocks");
+}  // namespace vh
+
+// In HOST code these two names are only handles for cudaGetSymbolAddress; they are not device addresses and must never be passed to a
+// kernel (noalloc_setup below does the lookup once per device).
+static __device__ __align__(256) double vh_noalloc_scratch[vh::NA_DOUBLES];
+static __device__ __align__(256) vh::real vh_noalloc_eos_table[4 * VH_EOS_TABLE_NODES];
+
+namespace vh {
+
+// max over the block of each of ten values; the result is valid in thread s < 10 (for value s)
+__device__ __forceinline__ real block_max10(real (&m)[10], real (*sm)[NA_THREADS / 32]) {
+#pragma unroll
+  for (int s = 0; s < 10; ++s) {
+    real v = m[s];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) sm[s][threadIdx.x >> 5] = v;
+  }
+  __syncthreads();
+  real r = real(0.0);
+  if (threadIdx.x < 10) {
+#pragma unroll
+    for (int w = 0; w < NA_THREADS / 32; ++w) r = fmax(r, sm[threadIdx.x][w]);
+  }
+  __syncthreads();      // sm may be reused by the caller
+  return r;
+}
+
+// The per-cell arithmetic is that of diagnostics_kernel, statement by statement; what differs is where the data comes from (compact double
+// arrays; a neighbour beyond the edge is the edge cell itself, which is what the ghost cells of Eqs. 75-76 hold; p = P0(e) computed here)
+// and where the maxima go (no atomics on a zeroed array: per-block maxima into `scratch`, combined by whichever block draws the last ticket).
+template <int EOS, bool MILNE>
+__global__ void __launch_bounds__(NA_THREADS) diagnostics_noalloc_kernel(const __grid_constant__ DevParams P, const double* __restrict__ q, const double* __restrict__ e,
+                                                                         const double* __restrict__ u, const double* __restrict__ u_prev, real t,
+                                                                         double* scratch, double* result, double* __restrict__ maps) {
+  __shared__ real sm[10][NA_THREADS / 32];
+  __shared__ bool last_block;
+  const long long np = (long long)P.nx * P.ny * P.nz * P.n_batch;
+  const real t2 = MILNE ? t * t : real(1.0);
+  real v[10] = {real(0.0), real(0.0), real(0.0), real(0.0), real(0.0), real(0.0), real(0.0), real(0.0), real(0.0), real(0.0)};
+  const long long n = (long long)blockIdx.x * NA_THREADS + threadIdx.x;
+  if (n < np) {
+    const int i = (int)(n % P.nx);
+    const int j = (int)((n / P.nx) % P.ny);
+    const int k = (int)((n / ((long long)P.nx * P.ny)) % P.nz);
+    const long long sy = P.nx, sz = (long long)P.nx * P.ny;
+    const long long xm = n - (i > 0 ? 1 : 0), xp = n + (i < P.nx - 1 ? 1 : 0);
+    const long long ym = n - (j > 0 ? sy : 0), yp = n + (j < P.ny - 1 ? sy : 0);
+    const long long zm = n - (k > 0 ? sz : 0), zp = n + (k < P.nz - 1 ? sz : 0);
+    const bool has_z = P.nz > 1;                      // nz = 1 is the 2+1d mode: no eta differences
+    const real ee = (real)e[n], pp = eos_p<EOS>(P, ee);
+    const real ut = (real)u[n], ux = (real)u[np + n], uy = (real)u[2 * np + n], un = (real)u[3 * np + n];
+    real pi[10];
+#pragma unroll
+    for (int s = 0; s < 10; ++s) pi[s] = (real)q[(PTT + s) * np + n];
+    const real Pi = (real)q[BPI * np + n];
+    const real norm = ut * ut - ux * ux - uy * uy - t2 * un * un;
+    const real tr = pi[0] - pi[4] - pi[7] - t2 * pi[9];
+    const real pipi = pi[0] * pi[0] - real(2.0) * (pi[1] * pi[1] + pi[2] * pi[2] + t2 * pi[3] * pi[3]) + pi[4] * pi[4] + real(2.0) * pi[5] * pi[5] +
+                        real(2.0) * t2 * pi[6] * pi[6] + pi[7] * pi[7] + real(2.0) * t2 * pi[8] * pi[8] + t2 * t2 * pi[9] * pi[9];
+    const real c0 = pi[0] * ut - pi[1] * ux - pi[2] * uy - t2 * pi[3] * un;
+    const real c1 = pi[1] * ut - pi[4] * ux - pi[5] * uy - t2 * pi[6] * un;
+    const real c2 = pi[2] * ut - pi[5] * ux - pi[7] * uy - t2 * pi[8] * un;
+    const real c3 = (pi[3] * ut - pi[6] * ux - pi[8] * uy - t2 * pi[9] * un) * (MILNE ? t : real(1.0));
+    const real iw = real(1.0) / (ee + pp), ip = real(1.0) / pp;
+    v[1] = fabs(norm - real(1.0));
+    v[2] = fabs(tr) * iw;
+    v[3] = fmax(fmax(fabs(c0), fabs(c1)), fmax(fabs(c2), fabs(c3))) * iw;
+    v[4] = sqrt(fabs(pipi)) * ip;
+    v[5] = fabs(Pi) * ip;
+    real theta = (MILNE ? ut / t : real(0.0)) + (ut - (real)u_prev[n]) * P.inv_dtau;
+    theta += ((real)u[np + xp] - (real)u[np + xm]) * (real(0.5) * P.inv_dx) + ((real)u[2 * np + yp] - (real)u[2 * np + ym]) * (real(0.5) * P.inv_dy);
+    if (has_z) theta += ((real)u[3 * np + zp] - (real)u[3 * np + zm]) * (real(0.5) * P.inv_dz);
+    if (P.shear || P.bulk) {
+      const real uc[4] = {ut, ux, uy, un};
+      real dt[4], dx[4], dy[4], dn[4];
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        const double* ua = u + a * np;
+        dt[a] = ((real)ua[n] - (real)u_prev[a * np + n]) * P.inv_dtau;
+        dx[a] = ((real)ua[xp] - (real)ua[xm]) * (real(0.5) * P.inv_dx);
+        dy[a] = ((real)ua[yp] - (real)ua[ym]) * (real(0.5) * P.inv_dy);
+        dn[a] = has_z ? ((real)ua[zp] - (real)ua[zm]) * (real(0.5) * P.inv_dz) : real(0.0);
+      }
+      Kin K;
+      kinematics<MILNE>(uc, dt, dx, dy, dn, t, K);
+      real r2s, r2b;
+      second_order_reynolds<EOS, MILNE>(P, t, uc, K, pi, Pi, ee, r2s, r2b);
+      v[8] = (P.shear && isfinite(r2s)) ? r2s : real(0.0);
+      v[9] = (P.bulk && isfinite(r2b)) ? r2b : real(0.0);
+    }
+    const real T = eos_temperature<EOS>(P, ee);
+    v[0] = T;
+    real p0, cs2;
+    eos_p_cs2<EOS>(P, ee, p0, cs2);
+    const real itp = fmin(T * P.inv_ctaupi_etas, P.relax_clamp);
+    const real zs = zeta_over_s(P, T), bb = (real(1.0) / real(3.0)) - cs2;
+    const real itP = fmin((zs > real(0.0)) ? T * bb * bb * P.inv_ctauPi / zs : inf_r(), P.relax_clamp);
+    const real kp = fabs(theta) / itp, kP = fabs(theta) / itP;
+    v[6] = (P.shear && isfinite(kp)) ? kp : real(0.0);
+    v[7] = (P.bulk && isfinite(kP)) ? kP : real(0.0);
+    if (maps) {
+#pragma unroll
+      for (int s = 0; s < 10; ++s) maps[s * np + n] = (double)v[s];
+    }
+  }
+  // this block's maxima (fmax drops a NaN, as the loop of diagnostics_kernel does)
+  real m[10];
+#pragma unroll
+  for (int s = 0; s < 10; ++s) m[s] = fmax(real(0.0), v[s]);
+  const real mine = block_max10(m, sm);
+  if (threadIdx.x < 10) {
+    __stcg(scratch + threadIdx.x * NA_MAX_BLOCKS + blockIdx.x, (double)mine);
+    __threadfence();                                  // the maxima are visible device-wide before this block takes its ticket
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const unsigned int ticket = atomicAdd(reinterpret_cast<unsigned int*>(scratch + NA_TICKET), 1u);      // the host zeroed it before this launch
+    last_block = (ticket == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!last_block) return;
+  __threadfence();
+  // last block: combine the gridDim.x per-block maxima (only those - older, larger calls left more behind them in the array)
+#pragma unroll
+  for (int s = 0; s < 10; ++s) {
+    real r = real(0.0);
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += NA_THREADS) r = fmax(r, (real)__ldcg(scratch + s * NA_MAX_BLOCKS + b));
+    m[s] = r;
+  }
+  const real all = block_max10(m, sm);
+  if (threadIdx.x < 10) result[threadIdx.x] = (double)all;
+}
+
+}  // namespace vh
+
+// Once per device and process, with that device current: the device addresses of the two arrays (checked), and the EOS-2 table
+// uploaded into its array.  No allocation on the device; the table is built on the host as vh_create builds it.
+namespace {
+struct NoallocDevice {
+  bool ready = false;
+  double* scratch = nullptr;          // device address of vh_noalloc_scratch on this device
+  vh::real* table = nullptr;          // device address of vh_noalloc_eos_table on this device
+};
+constexpr int kNoallocMaxDevices = 64;
+NoallocDevice g_noalloc_dev[kNoallocMaxDevices];
+vh_eos::LatticeTable g_noalloc_lattice;      // host copy (the scalars that go into DevParams), built with the first device
+std::mutex g_noalloc_mutex;
+}  // namespace
+
+static int noalloc_setup(int dev, cudaStream_t st, const NoallocDevice** out) {
+  if (dev < 0 || dev >= kNoallocMaxDevices) return fail(nullptr, VH_ERR_ARG, "vh_diagnostics_noalloc: device ordinal " + std::to_string(dev) + " is beyond the " + std::to_string(kNoallocMaxDevices) + " this entry point keeps books for");
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  NoallocDevice& d = g_noalloc_dev[dev];
+  if (!d.ready) {
+    double* scratch = nullptr;
+    vh::real* table = nullptr;
+    CUDA_TRY(nullptr, cudaGetSymbolAddress((void**)&scratch, vh_noalloc_scratch));
+    CUDA_TRY(nullptr, cudaGetSymbolAddress((void**)&table, vh_noalloc_eos_table));
+    if (!scratch || !table) return fail(nullptr, VH_ERR_CUDA, "vh_diagnostics_noalloc: cudaGetSymbolAddress returned a null address");
+    if (g_noalloc_lattice.node.empty()) g_noalloc_lattice = vh_eos::Builder().build();
+    const std::vector<real> nodes(g_noalloc_lattice.node.begin(), g_noalloc_lattice.node.end());      // the table in the library's precision
+    if (nodes.size() != (size_t)4 * VH_EOS_TABLE_NODES) return fail(nullptr, VH_ERR_STATE, "vh_diagnostics_noalloc: EOS table size does not match its array");
+    CUDA_TRY(nullptr, cudaMemcpyAsync(table, nodes.data(), nodes.size() * sizeof(real), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(nullptr, cudaStreamSynchronize(st));      // nodes lives on this stack frame
+    d.scratch = scratch; d.table = table; d.ready = true;
+  }
+  *out = &d;
+  return VH_OK;
+}
+
+extern "C" int vh_diagnostics_noalloc(const vh_params* p, double tau, const double* q15, const double* e, const double* u4, const double* u4_prev,
+                                      double* out10, int out_mem_space, double* maps10, void* cuda_stream) {
+  // argument checks first: none of them touches the device
+  std::string why;
+  if (check_params(p, why)) return fail(nullptr, VH_ERR_ARG, "vh_diagnostics_noalloc: " + why);
+  if (!q15 || !e || !u4 || !u4_prev || !out10) return fail(nullptr, VH_ERR_ARG, "vh_diagnostics_noalloc: q15, e, u4, u4_prev and out10 are required");
+  if (out_mem_space != 0 && out_mem_space != 1) return fail(nullptr, VH_ERR_ARG, "vh_diagnostics_noalloc: out_mem_space must be 0 (host) or 1 (device)");
+  if (p->geometry == 0 && !(tau > 0)) return fail(nullptr, VH_ERR_ARG, "vh_diagnostics_noalloc: Milne geometry needs tau > 0");
+  const long long np = (long long)p->nx * p->ny * p->nz * p->n_batch;
+  if (np > VH_NOALLOC_MAX_CELLS)
+    return fail(nullptr, VH_ERR_ARG, "vh_diagnostics_noalloc: the grid has " + std::to_string(np) + " cells, the fixed scratch array of this entry point serves at most " +
+                                         std::to_string((long long)VH_NOALLOC_MAX_CELLS) + " (VH_NOALLOC_MAX_CELLS); use a handle and vh_get_diagnostics for larger grids");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = -1;
+  CUDA_TRY(nullptr, cudaGetDevice(&dev));
+  const NoallocDevice* d = nullptr;
+  if (int rc = noalloc_setup(dev, st, &d)) return rc;
+  DevParams P;
+  fill_dev_params(*p, P);
+  if (p->eos == 2) {      // as in vh_create, with the table in its fixed array
+    const vh_eos::LatticeTable& tab = g_noalloc_lattice;
+    const int n = vh_eos::VH_EOS_N;
+    const double* nd = tab.node.data();
+    const double e0 = std::pow(tab.x0, 4), eN = std::pow(tab.xN, 4);
+    P.eos_tab = reinterpret_cast<const real2*>(d->table);
+    P.eos_n = n; P.eos_x0 = tab.x0; P.eos_xN = tab.xN; P.eos_inv_h = 1.0 / tab.h;
+    P.eos_lo_slope = nd[0] / e0; P.eos_pN = nd[4 * n]; P.eos_eN = eN;
+    P.eos_T0_over_x0 = nd[2] / tab.x0; P.eos_TN_over_xN = nd[4 * n + 2] / tab.xN;
+  }
+  // the one word that has to start from zero; the per-block maxima are overwritten before they are read
+  CUDA_TRY(nullptr, cudaMemsetAsync(d->scratch + NA_TICKET, 0, sizeof(unsigned int), st));
+  double* result = (out_mem_space == 1) ? out10 : d->scratch + NA_RESULT;
+  const unsigned nb = (unsigned)((np + NA_THREADS - 1) / NA_THREADS);
+  const real t = (real)tau;
+  const bool mil = (p->geometry == 0);
+#define VH_NA_LAUNCH(E)                                                                                                               \
+  do {                                                                                                                                \
+    if (mil) diagnostics_noalloc_kernel<E, true><<<nb, NA_THREADS, 0, st>>>(P, q15, e, u4, u4_prev, t, d->scratch, result, maps10);    \
+    else diagnostics_noalloc_kernel<E, false><<<nb, NA_THREADS, 0, st>>>(P, q15, e, u4, u4_prev, t, d->scratch, result, maps10);       \
+  } while (0)
+  if (p->eos == 2) VH_NA_LAUNCH(2); else if (p->eos == 1) VH_NA_LAUNCH(1); else VH_NA_LAUNCH(0);
+#undef VH_NA_LAUNCH
+  CUDA_TRY(nullptr, cudaGetLastError());
+  if (out_mem_space == 0) {
+    CUDA_TRY(nullptr, cudaMemcpyAsync(out10, result, 10 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(nullptr, cudaStreamSynchronize(st));
+  }
+  return VH_OK;
+}

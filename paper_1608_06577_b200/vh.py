@@ -33,7 +33,7 @@ class vh_params(C.Structure):
 
 
 # every symbol include/vh.h declares
-EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_part", "vh_halo_size", "vh_halo_export", "vh_halo_import", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_enable_regulation_map", "vh_get_regulation_map", "vh_run_until", "vh_eos_table", "vh_launch_count",
+EXPORTS = ["vh_create", "vh_set_initial", "vh_set_state", "vh_set_uprev", "vh_step", "vh_step_part", "vh_halo_size", "vh_halo_export", "vh_halo_import", "vh_step_profile", "vh_get_fields", "vh_get_status", "vh_get_diagnostics", "vh_get_diagnostic_maps", "vh_diagnostics_noalloc", "vh_enable_regulation_map", "vh_get_regulation_map", "vh_run_until", "vh_eos_table", "vh_launch_count",
            "vh_set_kernel_variant", "vh_measure_peaks", "vh_measure_fp32_peak", "vh_last_error", "vh_destroy"]
 
 _lib = None
@@ -67,6 +67,7 @@ def load_library(precision="f64"):
     L.vh_get_status.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     L.vh_get_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
     L.vh_get_diagnostic_maps.argtypes = [vp, vp, C.c_int]
+    L.vh_diagnostics_noalloc.argtypes = [C.POINTER(vh_params), C.c_double, vp, vp, vp, vp, vp, C.c_int, vp, vp]
     L.vh_enable_regulation_map.argtypes = [vp, C.c_int]
     L.vh_get_regulation_map.argtypes = [vp, vp, C.c_int]
     L.vh_run_until.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_longlong)]
@@ -274,6 +275,39 @@ class Solver:
     def set_kernel_variant(self, v):
         self._check(self.L.vh_set_kernel_variant(self.h, int(v)), "vh_set_kernel_variant")
         self.variant = int(v)
+
+
+NOALLOC_MAX_CELLS = 1 << 20      # VH_NOALLOC_MAX_CELLS of include/vh.h
+
+
+def diagnostics_noalloc(params: dict, tau, q15, e, u4, u4_prev, maps=None, stream=None, precision="f64"):
+    """vh_diagnostics_noalloc: the ten diagnostics of Solver.diagnostics() computed straight from CUDA tensors the caller already holds,
+    for programs that must not let the library allocate device memory (their own pool owns the GPU's memory, or a cudaMalloc stall is
+    not acceptable where they call this).  No Solver is involved; the library's fixed scratch array limits the grid to NOALLOC_MAX_CELLS
+    cells.  q15 [15, ...], e [...], u4 / u4_prev [4, ...]: contiguous float64 CUDA tensors on the current device, shape [..., n_batch, nz, ny, nx];
+    maps: None or a float64 CUDA tensor of 10 * cells elements that receives the per-cell values.  Returns the dict of ten maxima
+    (the call synchronises `stream`).  Marshalling only - this function itself creates no tensor.  Calls on different streams must not
+    overlap (they share the scratch), and the first call on a device does a one-time set-up: make it before capturing a stream."""
+    import torch
+
+    L = load_library(precision)
+    if not torch.cuda.is_available():
+        raise VHError("no CUDA device available (there is no CPU fallback)")
+    P = make_params(params)
+    np_ = P.nx * P.ny * P.nz * P.n_batch
+    for name, a, lead in (("q15", q15, 15), ("e", e, 1), ("u4", u4, 4), ("u4_prev", u4_prev, 4), ("maps", maps, 10)):
+        if a is None and name == "maps":
+            continue
+        if not (isinstance(a, torch.Tensor) and a.is_cuda and a.dtype == torch.float64 and a.is_contiguous() and a.numel() == lead * np_):
+            raise ValueError("%s must be a contiguous float64 CUDA tensor of %d elements" % (name, lead * np_))
+    st = stream if stream is not None else torch.cuda.current_stream()
+    out = (C.c_double * 10)()
+    rc = L.vh_diagnostics_noalloc(C.byref(P), float(tau), _ptr(q15), _ptr(e), _ptr(u4), _ptr(u4_prev), C.cast(out, C.c_void_p), 0, _ptr(maps),
+                                  C.c_void_p(st.cuda_stream))
+    if rc != VH_OK:
+        msg = L.vh_last_error(None)
+        raise VHError("vh_diagnostics_noalloc failed (%d): %s" % (rc, msg.decode() if msg else "?"))
+    return dict(zip(Solver.DIAG_NAMES, list(out)))
 
 
 def eos_table():
