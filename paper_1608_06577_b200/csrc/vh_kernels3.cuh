@@ -335,18 +335,27 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, kF32 ? 2 : 1)      // single 
     return ring + (s % NSTAGE) * T::SLOT;
   };
   const bool lane0 = (tid & 31) == 0;
-  // `witness`: a word that depends on EVERY value the warp loaded from the slot.  Lane 0 stores it to shared memory before it arrives: the
-  // store cannot issue until all those loads have written their registers, so no load of this warp is still in flight when the arrival
-  // becomes visible and the last warp out hands the slot to the TMA unit.  (Issuing the loads before the arrival is not enough: an
-  // arrival does not wait for earlier loads to complete, and the refill of an L2-resident halo can land within a few hundred cycles.
-  // Found in round 2 with two resident CTAs per SM, where a queued load of the refilling warp itself was overtaken about once per launch.)
+  // `witness`: a word that depends on EVERY value the warp loaded from the slot: each lane folds what it loaded into an int, and the
+  // warp-wide xor below makes lane 0's word depend on all 32 of them.  Lane 0 stores it to shared memory before it arrives: the reduction
+  // cannot produce its result until every lane's loads have written their registers, so no load of this warp is still in flight when the
+  // arrival becomes visible.  (Issuing the loads before the arrival is not enough: an arrival does not wait for earlier loads to complete, and
+  // the refill of an L2-resident halo can land within a few hundred cycles.  Found in round 2 with two resident CTAs per SM, where a queued
+  // load of the refilling warp itself was overtaken about once per launch.)
+  // The warp whose arrival completes the count refills the slot.  Before it hands the slot to the TMA unit it waits on the phase it has
+  // just completed (returns at once): that wait is the acquire that pairs with the release-arrivals of the other warps, so the order
+  // "all reads of the slot, then the refill" rests on the mbarrier's release / acquire and not on issue order.
   int* witness_sink = reinterpret_cast<int*>(empty + NSTAGE);      // [NW] one word per warp
   auto release = [&](int s, int witness) {
-    __syncwarp();
-    if (lane0 && s + NSTAGE < NSTREAM) {
-      *reinterpret_cast<volatile int*>(witness_sink + (tid >> 5)) = witness;
-      // the arrival that finds one arrival pending is the last one of this use of the slot: that warp refills it
-      if (mbar_arrive_pending(&empty[s % NSTAGE]) == 1u) issue(s + NSTAGE);
+    if (s + NSTAGE < NSTREAM) {      // (uniform) a slot that is not used again needs no hand-back
+      witness = __reduce_xor_sync(0xffffffffu, witness);
+      if (lane0) {
+        *reinterpret_cast<volatile int*>(witness_sink + (tid >> 5)) = witness;
+        // the arrival that finds one arrival pending is the last one of this use of the slot: that warp refills it
+        if (mbar_arrive_pending(&empty[s % NSTAGE]) == 1u) {
+          mbar_wait(&empty[s % NSTAGE], (unsigned)((s / NSTAGE) & 1));
+          issue(s + NSTAGE);
+        }
+      }
     }
   };
   auto hi = [](real x) -> int { return kF32 ? __float_as_int((float)x) : __double2hiint((double)x); };

@@ -106,28 +106,38 @@ def test_f32_gpu_config3_physics_2plus1d_and_lattice(vo):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("workload", ["3d", "batched2d"])
-@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("precision,workload", [("f64", "3d"), ("f32", "3d"), ("f64", "batched2d"), ("f32", "batched2d"), ("f32", "config5")])
 def test_full_size_runs_are_bit_reproducible(precision, workload):
     """Regression test of the ring hand-back of the stage kernel: the 128^3 workload, whose 4096 tiles per
     launch keep every SM busy with as many CTAs as fit (two in single precision), must give bitwise the same fields on every run and no
-    inversion failure.  Before the fix the two-CTA configuration corrupted about one tile per launch, differently each time."""
+    inversion failure.  Before the fix the two-CTA configuration corrupted about one tile per launch, differently each time; twenty runs of
+    three steps are 120 stage launches = half a million tiles per case.  "config5" is the two-CTA build at the size of BASELINE.json
+    configs[4] (512 x 512 x 128: 65 536 tiles per launch), five runs of two steps."""
     import torch
     from paper_1608_06577_b200 import vh
 
     rtol = 2e-6 if precision == "f32" else 1e-13
+    n_runs, n_steps = 20, 3
     if workload == "3d":
         prm, init, _ = inputs.config_3d(newton_rtol=rtol)
+    elif workload == "config5":
+        prm, init, _ = inputs.config_3d(512, 512, 128, dx=0.05, dy=0.05, n_hot=200, newton_rtol=rtol)
+        n_runs, n_steps = 5, 2
     else:       # the 2+1d instantiation of the same kernel: 64 events of 201 x 201 = 5824 tiles per launch
         prm, init, _ = inputs.config_batched2d(n_batch=64, newton_rtol=rtol)
-    runs = []
-    for _ in range(3):
+    e0, u0 = torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0")
+    first = None
+    for run in range(n_runs):
         s = vh.Solver(prm, precision=precision)
-        s.set_initial(torch.as_tensor(init["e"], device="cuda:0"), torch.as_tensor(init["u"], device="cuda:0"))
-        s.step(3)
+        s.set_initial(e0, u0)
+        s.step(n_steps)
         f = s.get_fields()
         st = s.status()
         s.close()
         assert st["n_inversion_failures"] == 0 and st["n_nonfinite"] == 0
-        runs.append(torch.cat([f["q"].reshape(-1), f["e"].reshape(-1), f["u"].reshape(-1)]))
-    assert torch.equal(runs[0], runs[1]) and torch.equal(runs[0], runs[2])
+        got = torch.cat([f["q"].reshape(-1), f["e"].reshape(-1), f["u"].reshape(-1)])
+        del f
+        if first is None:
+            first = got
+        else:
+            assert torch.equal(first, got), "run %d differs from run 0" % run
