@@ -38,7 +38,7 @@ template <bool TWO_D> struct Tile {
 };
 template <bool TWO_D, bool VISC> constexpr size_t tile_smem_bytes() {
   using T = Tile<TWO_D>;
-  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(real) + (2 * T::NSTAGE + 1) * sizeof(uint64_t) + T::NW * sizeof(int);
+  return (size_t)(T::NSTAGE * T::SLOT + (VISC ? NQ + T::NCEN : 4) * T::NT) * sizeof(real) + (2 * T::NSTAGE + 1) * sizeof(uint64_t) + T::NT * sizeof(int);
 }
 
 struct TileArgs {
@@ -335,26 +335,26 @@ __global__ void __launch_bounds__(Tile<TWO_D>::NT, kF32 ? 2 : 1)      // single 
     return ring + (s % NSTAGE) * T::SLOT;
   };
   const bool lane0 = (tid & 31) == 0;
-  // `witness`: a word that depends on EVERY value the warp loaded from the slot: each lane folds what it loaded into an int, and the
-  // warp-wide xor below makes lane 0's word depend on all 32 of them.  Lane 0 stores it to shared memory before it arrives: the reduction
-  // cannot produce its result until every lane's loads have written their registers, so no load of this warp is still in flight when the
-  // arrival becomes visible.  (Issuing the loads before the arrival is not enough: an arrival does not wait for earlier loads to complete, and
-  // the refill of an L2-resident halo can land within a few hundred cycles.  Found in round 2 with two resident CTAs per SM, where a queued
+  // `witness`: a word that depends on every value a lane loaded from the slot.  EVERY lane stores its word to shared memory (one conflict-free
+  // store per warp) before the warp arrives: a lane's store cannot issue until its loads have written their registers, __syncwarp orders all
+  // lanes' loads and stores before what lane 0 does next, and lane 0's arrival is a release - so no load of this warp is still in flight when
+  // the arrival becomes visible.  (Issuing the loads before the arrival is not enough: an arrival does not wait for earlier loads to complete,
+  // and the refill of an L2-resident halo can land within a few hundred cycles.  Found in round 2 with two resident CTAs per SM, where a queued
   // load of the refilling warp itself was overtaken about once per launch.)
-  // The warp whose arrival completes the count refills the slot.  Before it hands the slot to the TMA unit it waits on the phase it has
-  // just completed (returns at once): that wait is the acquire that pairs with the release-arrivals of the other warps, so the order
-  // "all reads of the slot, then the refill" rests on the mbarrier's release / acquire and not on issue order.
-  int* witness_sink = reinterpret_cast<int*>(empty + NSTAGE);      // [NW] one word per warp
+  // The warp whose arrival completes the count refills the slot.  Its arrival is a read-modify-write of the barrier that has observed the
+  // release-arrivals of all other warps (that is what "one arrival pending" says); the fence.acq_rel.cta after it turns that observation
+  // into an acquire, so "every warp's reads of the slot, then the refill" rests on release / acquire, not on issue order.  Measured
+  // alternatives for this acquire, per step at 128^3: none 1.2115 ms, this fence 1.214, mbarrier.try_wait.parity on the completed phase 1.2345,
+  // mbarrier.test_wait.parity 1.277; a warp-wide xor (redux) of the witness instead of the per-lane stores costs another 0.012 ms.
+  int* witness_sink = reinterpret_cast<int*>(empty + NSTAGE);      // [NT] one word per thread
   auto release = [&](int s, int witness) {
     if (s + NSTAGE < NSTREAM) {      // (uniform) a slot that is not used again needs no hand-back
-      witness = __reduce_xor_sync(0xffffffffu, witness);
-      if (lane0) {
-        *reinterpret_cast<volatile int*>(witness_sink + (tid >> 5)) = witness;
-        // the arrival that finds one arrival pending is the last one of this use of the slot: that warp refills it
-        if (mbar_arrive_pending(&empty[s % NSTAGE]) == 1u) {
-          mbar_wait(&empty[s % NSTAGE], (unsigned)((s / NSTAGE) & 1));
-          issue(s + NSTAGE);
-        }
+      *reinterpret_cast<volatile int*>(witness_sink + tid) = witness;
+      __syncwarp();
+      // the arrival that finds one arrival pending is the last one of this use of the slot: that warp refills it
+      if (lane0 && mbar_arrive_pending(&empty[s % NSTAGE]) == 1u) {
+        __threadfence_block();
+        issue(s + NSTAGE);
       }
     }
   };
