@@ -62,7 +62,9 @@ typedef struct {
   double minmod_theta;              /* flux limiter theta in [1,2], Eq. 67                                              */
   double xi0, rho_max;              /* Eq. 74: 0.1, 1 (:445)                                                            */
   int newton_max_iter;              /* Newton-Raphson cap for Eq. 72 (reading R6: 50)                                   */
-  double newton_rtol;               /* stop when |de| <= rtol*|e| (1e-13)                                               */
+  double newton_rtol;               /* accuracy of the root: the last Newton correction satisfies |de| <= rtol*|e| (1e-13).  The kernels test
+                                       |de| <= max(rtol, 0.1*sqrt(rtol))*|e| and then apply that correction: by quadratic convergence the
+                                       next one is below rtol*|e| (R6), which saves the iteration that would only confirm it    */
   double tau_relax_floor_over_dtau; /* c: 1/tau_Pi, 1/tau_pi <= 1/(c*dtau) (reading R14); 0 disables                    */
   int storage;                      /* 0: all ten pi^{mu nu} and four u^mu are state (the paper's choice, :333); 1: reduced storage (:476,
                                        Eqs. 47-51, reading R22): pi^xx, pi^xy, pi^xeta, pi^yy, pi^yeta and u^x, u^y, u^eta only - 43 instead
@@ -103,7 +105,10 @@ int vh_step(vh_handle* h, int n_steps);
  * (side 0: low eta, 1: high eta) into buf; vh_halo_import writes buf into the GHOST planes beyond that face, replacing the outflow copies
  * (Eqs. 75-76) the kernels put there - a face without a neighbour simply keeps them.  buf: DEVICE memory of vh_halo_size doubles (whole
  * padded planes, always double).  Asynchronous on the handle's stream.  Default pipeline, 3+1d, n_batch = 1 only (VH_ERR_STATE otherwise);
- * the result is bit-identical to a single handle over the whole grid.                                                                     */
+ * the result is bit-identical to a single handle over the whole grid, and the failure counters of the slabs add up to the single handle's: a
+ * face that has received a vh_halo_import has a neighbour (until the next vh_set_initial / vh_set_state), which counts the interface states on
+ * its side.  Between part 0 and part 3 of a step only vh_step_part, the halo calls and the read-only getters are allowed: vh_step,
+ * vh_step_profile, vh_run_until and vh_set_kernel_variant return VH_ERR_STATE.                                                              */
 int vh_step_part(vh_handle* h, int part);
 int vh_halo_size(vh_handle* h, int what, long long* n_doubles);
 int vh_halo_export(vh_handle* h, int what, int side, double* buf_device);

@@ -30,18 +30,28 @@ static int fail(vh_handle* h, int code, const std::string& msg) {
     if (_e != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(_e)); \
   } while (0)
 
-// every entry point that touches the device runs on the handle's device, whatever the caller's current device is
-static int enter(vh_handle* h) {
+// every entry point that touches the device runs on the handle's device, whatever the caller's current device is - and hands the caller's
+// device back when it returns (on every path: the guard lives on the entry point's stack frame), so that a host framework's notion of the
+// current device (later allocations, its current stream) is not changed behind its back by a call on a handle of another GPU
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+static int enter(vh_handle* h, DeviceGuard& g) {
   int dev = -1;
-  if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) {
+  const bool known = (cudaGetDevice(&dev) == cudaSuccess);
+  if (!known || dev != h->device) {
     cudaError_t e = cudaSetDevice(h->device);
     if (e != cudaSuccess) return fail(h, VH_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+    if (known) { g.prev = dev; g.switched = true; }
   }
   return VH_OK;
 }
-#define VH_ENTER(h)                         \
-  do {                                      \
-    if (int _rc = enter(h)) return _rc;     \
+#define VH_ENTER(h)                                   \
+  DeviceGuard _vh_device_guard;                       \
+  do {                                                \
+    if (int _rc = enter(h, _vh_device_guard)) return _rc; \
   } while (0)
 
 static long long round_up(long long a, long long m) { return (a + m - 1) / m * m; }
@@ -272,7 +282,8 @@ int vh_create(const vh_params* p, void* cuda_stream, vh_handle** out) {
 
 void vh_destroy(vh_handle* h) {
   if (!h) return;
-  enter(h);
+  DeviceGuard guard;
+  enter(h, guard);
   cudaStreamSynchronize(h->stream);
   cudaFree(h->pool);
   cudaFree(h->cnt);
@@ -291,6 +302,7 @@ int vh_set_kernel_variant(vh_handle* h, int variant) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   if (variant < 0 || variant > 2) return fail(h, VH_ERR_ARG, "unknown kernel variant");
   if (h->reduced && variant != 0) return fail(h, VH_ERR_ARG, "reduced-storage mode has one kernel (variant 0)");
+  if (h->next_part != 0) return fail(h, VH_ERR_STATE, "vh_set_kernel_variant in the middle of a step taken with vh_step_part");
   h->variant = variant;
   return VH_OK;
 }
@@ -341,6 +353,7 @@ int vh_set_initial(vh_handle* h, const double* e, const double* u4, const double
   CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
   h->n_steps = 0;
   h->next_part = 0;
+  h->slab_nb[0] = h->slab_nb[1] = false;
   h->cur[0] = h->q[0]; h->cur[1] = h->e[0]; h->cur[2] = h->p[0]; h->cur[3] = h->u[0];
   h->uprev_initial = true;
   int rc = reset_counters(h);
@@ -389,6 +402,7 @@ int vh_set_state(vh_handle* h, const double* q15, const double* e, const double*
   CUDA_TRY(h, launch_ghost(h, h->q[0], h->e[0], h->p[0], h->u[0]));
   h->n_steps = n_steps_done;
   h->next_part = 0;
+  h->slab_nb[0] = h->slab_nb[1] = false;
   h->cur[0] = h->q[0]; h->cur[1] = h->e[0]; h->cur[2] = h->p[0]; h->cur[3] = h->u[0];
   int rc = reset_counters(h);
   if (rc) return rc;
@@ -554,6 +568,7 @@ static int halo_copy(vh_handle* h, int what, int side, double* buf, bool exporti
   dim3 grid((unsigned)((P.plane + 255) / 256), G.n_arr * G.n_planes);
   if (exporting) plane_kernel<true><<<grid, 256, 0, h->stream>>>(P, G, buf);
   else plane_kernel<false><<<grid, 256, 0, h->stream>>>(P, G, buf);
+  if (!exporting) h->slab_nb[side] = true;      // from now on the interface states beyond this face are the neighbour's to count
   h->launches++;
   CUDA_TRY(h, cudaGetLastError());
   return VH_OK;
@@ -586,6 +601,7 @@ int vh_step_profile(vh_handle* h, int n_steps, double* ms4) {
   if (!h) return fail(nullptr, VH_ERR_ARG, "handle is NULL");
   VH_ENTER(h);
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_step_profile before vh_set_initial");
+  if (h->next_part != 0) return fail(h, VH_ERR_STATE, "vh_step_profile in the middle of a step taken with vh_step_part");
   if (n_steps < 1 || !ms4) return fail(h, VH_ERR_ARG, "n_steps >= 1 and ms4 != NULL required");
   cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   struct Guard { cudaEvent_t* e; ~Guard() { for (int i = 0; i < 5; ++i) if (e[i]) cudaEventDestroy(e[i]); } } guard{ev};      // also on every early return
@@ -754,6 +770,7 @@ int vh_run_until(vh_handle* h, double T_f, int max_steps, int check_every, long 
   VH_ENTER(h);
   if (h->reduced) return fail(h, VH_ERR_STATE, "vh_run_until is not available in reduced-storage mode (storage = 1): the diagnostics kernels read the full set of arrays");
   if (!h->initialised) return fail(h, VH_ERR_STATE, "vh_run_until before vh_set_initial");
+  if (h->next_part != 0) return fail(h, VH_ERR_STATE, "vh_run_until in the middle of a step taken with vh_step_part");
   if (max_steps < 0 || check_every < 1 || !(T_f >= 0.0)) return fail(h, VH_ERR_ARG, "max_steps >= 0, check_every >= 1, T_f >= 0 required");
   long long done = 0;
   double d[10];

@@ -38,6 +38,7 @@ struct vh_handle {
   bool two_d = false;
   vh::real* cur[4] = {nullptr, nullptr, nullptr, nullptr};   // q, e, p, u of the most recently written state (what vh_halo_export(what = 1) reads)
   int next_part = 0;                 // vh_step_part: the part of the RK2 step that comes next (0..3)
+  bool slab_nb[2] = {false, false};  // a neighbouring eta-slab exists beyond the low / high face: set by vh_halo_import, cleared by vh_set_initial / vh_set_state
   bool reduced = false;              // vh_params.storage == 1: 10 q + 3 u arrays per time level (vh_kernels5.cuh), own stage kernel
   bool uprev_initial = true;         // u^{n-1} is the copy of u^0 made by vh_set_initial (reduced storage: its u^tau is normalised at tau0, not tau0 - dtau)
   int variant = 0;                   // 0: velocity kernel + TMA tile kernel; 1: one-thread-per-cell kernel + ghost kernel; 2: velocity + L1 stage kernel
@@ -47,14 +48,18 @@ struct vh_handle {
 };
 
 
-// VH_DEBUG_SYNC=1 in the environment: synchronise after every launch and name the kernel that faulted.
+// Launch check of every kernel.  A debugging build (nvcc -DVH_DEBUG_SYNC) also synchronises after each launch and names the kernel that
+// faulted; the product build reads nothing from the environment.
 inline cudaError_t vh_debug_sync(vh_handle* h, const char* what) {
   cudaError_t e = cudaGetLastError();
-  static const bool on = getenv("VH_DEBUG_SYNC") != nullptr;
-  if (e == cudaSuccess && on) {
+#ifdef VH_DEBUG_SYNC
+  if (e == cudaSuccess) {
     e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) fprintf(stderr, "[vh] %s faulted at step %lld: %s\n", what, h->n_steps, cudaGetErrorString(e));
   }
+#else
+  (void)h; (void)what;
+#endif
   return e;
 }
 

@@ -33,6 +33,7 @@ struct VelTileArgs {
   Counters* cnt;
   real t;
   int a_q;                       // index of q_in in the pool of padded arrays (outermost tensor-map coordinate)
+  int nb_lo, nb_hi;              // eta-slab decomposition: another slab owns the cells beyond the low / high eta face (it counts that interface's outer state)
 };
 
 template <int EOS, bool VISC, bool MILNE, bool TWO_D, bool THETA1>
@@ -133,8 +134,9 @@ __global__ void __launch_bounds__(VTile<TWO_D>::NT, TWO_D ? 3 : 6)
     // status counter: every state of every interface once (see velocity_kernel); nothing along a direction of extent 1
     if (ext > 1) {
       nfail += (SL.fail ? 1u : 0u) + (SR.fail ? 1u : 0u);
-      if (pos == 0 && SL.fail) ++nfail;
-      if (pos == ext - 1 && SR.fail) ++nfail;
+      // the outer state of a boundary interface is the ghost cell's, equal to this one (Eqs. 75-76) - unless a neighbouring slab owns it
+      if (pos == 0 && SL.fail && !(d == 2 && A.nb_lo)) ++nfail;
+      if (pos == ext - 1 && SR.fail && !(d == 2 && A.nb_hi)) ++nfail;
     }
     if (valid) {
       real* vL = A.vL + d * fs + c;

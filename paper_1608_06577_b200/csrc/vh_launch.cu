@@ -76,7 +76,7 @@ static cudaError_t launch_tile_t(vh_handle* h, int stage, const StageArgs& S, cu
     auto vkern = velocity_tile_kernel<EOS, VISC, MILNE, TWO_D, THETA1>;
     if (cudaError_t e = vh_opt_in_smem(h, (const void*)vkern, vsmem); e != cudaSuccess) return e;
     dim3 grid((P.nx + V::VX - 1) / V::VX, (P.ny + V::VY - 1) / V::VY, ((P.nz + V::VZ - 1) / V::VZ) * P.n_batch);
-    VelTileArgs VA{S.e_in, h->vL, h->vR, S.cnt, S.t, (int)((S.q_in - h->pool) / fs)};
+    VelTileArgs VA{S.e_in, h->vL, h->vR, S.cnt, S.t, (int)((S.q_in - h->pool) / fs), h->slab_nb[0] ? 1 : 0, h->slab_nb[1] ? 1 : 0};
     vkern<<<grid, V::NT, vsmem, h->stream>>>(P, VA, h->mapVA, h->mapVZ);
     h->launches++;
     cudaError_t e = debug_sync(h, "velocity tile kernel");

@@ -130,3 +130,52 @@ def test_slab_solver_two_ranks_gloo(vh, tmp_path):
         want = torch.cat([fr["q"][..., z, :, :].reshape(-1), fr["e"][..., z, :, :].reshape(-1), fr["u"][..., z, :, :].reshape(-1)]).cpu().numpy()
         assert np.array_equal(got, want), r
         assert json.loads(outs[r][0].strip().splitlines()[-1])["n_inversion_failures"] == 0
+
+
+def test_slab_failure_counters_add_up_and_half_steps_are_guarded(vh):
+    # a cell in the last plane of slab 0 whose inversion fails (E < 0, E + Pi > 0: reading R6) - the states extrapolated from it sit on the
+    # interface between slab 0 and slab 1.  In one grid every interface state is counted once; with slabs each interior face has an owner on
+    # either side, so the counters of the slabs must add up to the single grid's, and the fields stay bit-identical
+    import torch
+    prm, st, up = _case()
+    W, nzl = 2, prm["nz"] // 2
+    s0 = vh.Solver(prm)
+    s0.set_initial(_t(st["e"]), _t(st["u"]), _t(st["pi"]), _t(st["Pi"]))
+    s0.set_uprev(_t(up))
+    f0 = s0.get_fields(with_uprev=True)
+    for k, j, i in ((nzl - 1, 5, 20), (nzl, 7, 9), (0, 3, 3), (prm["nz"] - 1, 8, 30)):      # both sides of the cut, and the two physical boundaries
+        e_c = float(f0["e"][0, k, j, i])
+        f0["q"][0][0, k, j, i] = -0.05 * e_c + float(f0["q"][4][0, k, j, i])
+        f0["q"][14][0, k, j, i] = 0.5 * e_c
+    s0.set_state(f0["q"], f0["e"], f0["u"], f0["up"])
+    s0.step(1)
+    fr, n_ref = s0.get_fields(with_uprev=True), s0.status()["n_inversion_failures"]
+    s0.close()
+    assert n_ref >= 24
+    sl = [vh.Solver(dict(prm, nz=nzl)) for _ in range(W)]
+    cut = lambda a, r: a[..., r * nzl:(r + 1) * nzl, :, :].contiguous()
+    bufs = {w: torch.empty(sl[0].halo_size(w), dtype=torch.float64, device="cuda:0") for w in (0, 1)}
+
+    def exchange(what):
+        sl[0].halo_export(what, 1, bufs[what]); sl[1].halo_import(what, 0, bufs[what])
+        sl[1].halo_export(what, 0, bufs[what]); sl[0].halo_import(what, 1, bufs[what])
+
+    for r, s in enumerate(sl):
+        s.set_state(cut(f0["q"], r), cut(f0["e"], r), cut(f0["u"], r), cut(f0["up"], r))
+    exchange(1)
+    for part in range(4):
+        for s in sl:
+            s.step_part(part)
+        if part == 1:      # in the middle of a step nothing that assumes a whole state may run
+            for call in (lambda: sl[0].step(1), lambda: sl[0].step_profile(1), lambda: sl[0].run_until(0.1, 3), lambda: sl[0].set_kernel_variant(1)):
+                with pytest.raises(vh.VHError):
+                    call()
+        exchange(part % 2)
+    total = 0
+    for r, s in enumerate(sl):
+        f = s.get_fields(with_uprev=True)
+        for k in ("q", "e", "p", "u", "up"):
+            assert torch.equal(f[k], fr[k][..., r * nzl:(r + 1) * nzl, :, :]), (r, k)
+        total += s.status()["n_inversion_failures"]
+        s.close()
+    assert total == n_ref, (total, n_ref)
