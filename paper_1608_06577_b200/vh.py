@@ -358,11 +358,14 @@ def measure_fp32_peak(repeats=10, stream=None):
 class SlabSolver:
     """One eta-slab of a larger 3+1d grid per rank of a torch.distributed group: rank r owns planes
     [r nz/W, (r+1) nz/W) and exchanges two boundary planes of the 21 state arrays (and one plane of state velocities) with its neighbours after
-    every kernel of the step - neighbour send / recv, NCCL over NVLink 5 / NVSwitch between GPUs (device buffers go to the backend as they are);
-    with the gloo backend the planes are staged through host memory.  Argument marshalling and the exchange only: every step of the path runs in
-    the library's kernels, and the result is bit-identical to a single Solver over the whole grid."""
+    every kernel of the step - neighbour send / recv.  With the NCCL backend the device buffers go to the backend as they are and the whole
+    exchange is ordered on the solver's stream (export kernel -> send / recv -> import kernel; the host neither synchronises nor waits); with
+    the gloo backend the planes are staged through host memory.  Argument marshalling and the exchange only: every step of the path runs in
+    the library's kernels, and the result is bit-identical to a single Solver over the whole grid.
+    Tested with gloo (two ranks sharing one GPU) and with several handles in one process; the NCCL path has NOT been run on more than one GPU
+    (no multi-GPU box was available to this repository's tests).  device = None takes cuda:LOCAL_RANK."""
 
-    def __init__(self, params: dict, group=None, device="cuda:0", precision="f64"):
+    def __init__(self, params: dict, group=None, device=None, precision="f64"):
         import torch
         import torch.distributed as dist
 
@@ -374,6 +377,8 @@ class SlabSolver:
         self.nzl = nz // self.world
         self.z0 = self.rank * self.nzl
         local = dict(params, nz=self.nzl)
+        if device is None:
+            device = "cuda:%d" % int(os.environ.get("LOCAL_RANK", "0"))
         self.s = Solver(local, device=device, precision=precision)
         self.device = self.s.device
         self.host_staging = dist.get_backend(group) == "gloo"
@@ -385,29 +390,32 @@ class SlabSolver:
         return None if a is None else a[..., self.z0:self.z0 + self.nzl, :, :].contiguous()
 
     def _exchange(self, what):
-        """send my outermost physical planes at each face to the neighbour beyond it, receive its planes into my ghost planes"""
+        """send my outermost physical planes at each face to the neighbour beyond it, receive its planes into my ghost planes.
+        Everything is issued with the solver's stream as torch's current stream: NCCL orders its transfers after the work already on the
+        current stream and `wait()` makes the current stream (not the host) wait for them, so export -> transfer -> import is a chain on
+        the device; the host-staged copies of the gloo path are ordered by the same stream."""
         dist, torch = self.dist, self.torch
-        ops, staged = [], []
-        for side, nb in ((0, self.lo), (1, self.hi)):
-            if nb is None:
-                continue
-            out, inp = self.buf[what][side]
-            self.s.halo_export(what, side, out)
-            self.s.stream.synchronize()
-            if self.host_staging:
-                out_h, inp_h = out.cpu(), torch.empty(inp.shape, dtype=inp.dtype)
-                ops += [dist.P2POp(dist.isend, out_h, nb, self.group), dist.P2POp(dist.irecv, inp_h, nb, self.group)]
-                staged.append((side, inp, inp_h))
-            else:
-                ops += [dist.P2POp(dist.isend, out, nb, self.group), dist.P2POp(dist.irecv, inp, nb, self.group)]
-                staged.append((side, inp, None))
-        if ops:
-            for r in dist.batch_isend_irecv(ops):
-                r.wait()
-        for side, inp, inp_h in staged:
-            if inp_h is not None:
-                inp.copy_(inp_h)
-            self.s.halo_import(what, side, inp)
+        with torch.cuda.stream(self.s.stream):
+            ops, staged = [], []
+            for side, nb in ((0, self.lo), (1, self.hi)):
+                if nb is None:
+                    continue
+                out, inp = self.buf[what][side]
+                self.s.halo_export(what, side, out)
+                if self.host_staging:
+                    out_h, inp_h = out.cpu(), torch.empty(inp.shape, dtype=inp.dtype)      # (.cpu() waits for the export on the current stream)
+                    ops += [dist.P2POp(dist.isend, out_h, nb, self.group), dist.P2POp(dist.irecv, inp_h, nb, self.group)]
+                    staged.append((side, inp, inp_h))
+                else:
+                    ops += [dist.P2POp(dist.isend, out, nb, self.group), dist.P2POp(dist.irecv, inp, nb, self.group)]
+                    staged.append((side, inp, None))
+            if ops:
+                for r in dist.batch_isend_irecv(ops):
+                    r.wait()      # gloo: the host waits for the planes; NCCL: the current stream does
+            for side, inp, inp_h in staged:
+                if inp_h is not None:
+                    inp.copy_(inp_h)
+                self.s.halo_import(what, side, inp)
 
     def set_initial(self, e, u4, pi10=None, Pi=None):
         """global arrays [..., nz, ny, nx]; every rank takes its own planes"""
