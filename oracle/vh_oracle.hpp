@@ -250,7 +250,8 @@ template <class R> class Solver {
       size_t c = (size_t)i + (size_t)P.nx * ((size_t)j + (size_t)P.ny * k);
       size_t s = idx(i + 2, j + 2, k + 2);
       for (int m = 0; m < 4; ++m) up[m][s] = up_in[m * np + c];
-      // reduced storage: u^tau is not state - it is always the normalisation at the time level the velocity belongs to (here tau0 - dtau)
+      // reduced storage: u^tau is not state - it is always the normalisation at the time level the velocity belongs to (here tau0 - dtau;
+    // pinned by tests/test_oracle_reduced.py::test_reduced_mode_normalises_u_prev_at_its_own_time_level)
       if (reduced()) up[0][s] = sqrt(R(1) + up[1][s] * up[1][s] + up[2][s] * up[2][s] + tau2(R(P.tau0 - P.dtau)) * up[3][s] * up[3][s]);
     }
   }

@@ -149,3 +149,48 @@ def test_implicit_inversion_returns_the_state_it_was_built_from(vo):
     assert np.allclose(f1["u"][:, 0, 0, 0, 0], [ut, *ui], rtol=1e-11)
     assert np.allclose(f1["q"][:, 0, 0, 0, 0], f0["q"][:, 0, 0, 0, 0], rtol=1e-10, atol=1e-13)
     assert o.status()["n_inversion_failures"] == 0
+
+
+def test_reduced_mode_normalises_u_prev_at_its_own_time_level(vo):
+    """Pin of Solver::set_uprev in reduced mode (DESIGN.md R22: u^tau of a stored velocity is the normalisation u.u = 1 with the metric of the
+    time level the velocity belongs to - for u^{n-1} that is tau0 - dtau, g_{eta eta} = -(tau0 - dtau)^2, Eq. 27).  The exact boosted-static
+    solution fixes it: D u^tau = (u^tau_n - u^tau_{n-1})/dtau enters sigma^{mu nu} at the first step (A.5-A.12, :424), and a u^tau_{n-1}
+    normalised with tau0 instead is off by ~ tau0 (u^eta)^2 dtau / u^tau - an O(1) error in that derivative, which drives pi^{mu nu} away
+    from the solution ninety times faster than the truncation error does.  The u^tau handed to set_uprev is deliberately wrong (zero):
+    in reduced mode it is not state and must not be used."""
+    nz = 41
+    e0 = 30.0
+    amp = 0.05 * e0
+
+    def first_step_error(storage, u_tau_prev):
+        prm = inputs.base_params(nx=3, ny=3, nz=nz, dz=0.025, tau0=2.0, dtau=0.002, eos=0, physics=1, zeta_model=0, rho_max=1e30,
+                                 tau_relax_floor_over_dtau=0.0, storage=storage)
+        tau0 = prm["tau0"]
+        itp = (e0 / 13.8) ** 0.25 / (5 * 0.2)
+        eta = inputs.centred_axis(nz, prm["dz"])
+        t0 = tau0 * np.cosh(eta)
+
+        def state(tau):
+            dec = np.exp(-(tau * np.cosh(eta) - t0.min()) * itp)[:, None, None]
+            e, u, pi = boosted_static_state(prm, 1.0, 0.6, -0.3, 0.4, tau, e0)
+            return e, u, pi * amp * dec[None, None]
+
+        e, u, pi = state(tau0)
+        up = state(tau0 - prm["dtau"])[1].copy()
+        if u_tau_prev == "zero":
+            up[0] = 0.0
+        elif u_tau_prev == "normalised at tau0":
+            up[0] = np.sqrt(1.0 + up[1] ** 2 + up[2] ** 2 + tau0 ** 2 * up[3] ** 2)
+        o = vo.Oracle(prm)
+        o.set_initial(e, u, pi)
+        o.set_uprev(up)
+        o.step(1)
+        f, pp = o.get_fields(), state(o.status()["tau"])[2]
+        k = slice(nz // 2 - 6, nz // 2 + 7)
+        return max(np.max(np.abs(f["q"][4 + n][0, k] - pp[n][0, k])) for n in range(10)) / amp
+
+    bar = 2e-6
+    assert first_step_error(1, "zero") < bar                       # measured 5.2e-7: truncation error of one step
+    # what the bar would catch - the full mode takes u^tau_{n-1} as given, so the mistake can be fed to it from outside:
+    assert first_step_error(0, "exact") < bar
+    assert first_step_error(0, "normalised at tau0") > 10 * bar    # measured 4.6e-5
