@@ -33,7 +33,18 @@ ALG_BYTES_STAGE = {"stage1": (25 + 21) * 8.0, "stage2": (40 + 21) * 8.0}
 # Raw `ncu --csv` metric page of one RK2 step of THIS workload (four launches, in launch order), committed with the build it was taken
 # from; the command is in profiles/r02_metrics.md.  bench.py reads DRAM traffic, executed DFMA/DADD/DMUL and FP64-pipe utilisation per
 # launch from it (they are properties of the build, not of a run: ncu replays kernels and cannot be on while timing).
-NCU_METRICS_CSV = os.path.join(ROOT, "profiles", "r02_metrics.csv")
+NCU_METRICS_CSV = os.path.join(ROOT, "profiles", "r03_metrics.csv")
+
+
+def metrics_page(workload="config3", physics="config3", precision="f64", storage=0, variant=0):
+    """The committed raw ncu page of the configuration a line is printed for (profiles/r03_metrics.md names the command of each), or None:
+    FP64 default pipeline only - the pages hold FP64 op counts and the launch order velocity / stage / velocity / stage."""
+    if precision != "f64" or storage or variant:
+        return None
+    tag = workload if workload != "config3" else ("paper" if physics == "paper" else "config3")
+    if workload != "config3" and physics == "paper":
+        return None
+    return NCU_METRICS_CSV if tag == "config3" else os.path.join(ROOT, "profiles", "r03_metrics_%s.csv" % tag)
 LAUNCH_KEYS = ("velocity1", "stage1", "velocity2", "stage2")
 
 
@@ -465,7 +476,8 @@ def main():
         if variant1:
             alg_kernel = {"stage1": 0.5 * flops_cu, "stage2": 0.5 * flops_cu}
         bytes_kernel = {k: v * bscale for k, v in {"stage1": ALG_BYTES_STAGE["stage1"], "stage2": ALG_BYTES_STAGE["stage2"], "velocity1": 10 * 8.0, "velocity2": 10 * 8.0}.items()}
-        ncu = ncu_metrics() if (ncell == 128 ** 3 and default_pipeline and args.physics == "config3" and not f32 and not other) else {}
+        page = metrics_page(args.workload, args.physics, args.precision, args.storage, args.variant)
+        ncu = ncu_metrics(page) if page else {}
         ex_kernel, pipe_kernel, traffic_kernel = {}, {}, {}
         for k, m in ncu.items():
             try:
@@ -490,12 +502,14 @@ def main():
             roof = {"bound": "alu", "achieved": flops_launch / dur / 1e12, "peak": alu_gflops / 1e3, "unit": "TFLOP/s"}
         else:
             roof = {"bound": "hbm", "achieved": bytes_launch / dur / 1e9, "peak": hbm_peak, "unit": "GB/s"}
-        roof["frac"] = roof["achieved"] / roof["peak"]
+        # a fraction is printed only where the executed flops of THIS configuration's kernels are on file (min(alg, executed) numerator);
+        # without a page the minimal count alone would be the numerator, which is known to be too kind (frac_on_minimal_count keeps it, labelled)
+        roof["frac"] = roof["achieved"] / roof["peak"] if dom in ex_kernel else None
         useful_step = sum(useful.values())
         step_roof_s = max(useful_step * ncell / (alu_gflops * 1e9), ALG_BYTES_PER_CELL_UPDATE * bscale * ncell / (hbm_peak * 1e9))
         kname = ("velocity_tile_kernel" if "velocity" in dom else "stage_tile_kernel") if default_pipeline else ("stage_reduced_kernel" if args.storage else ("stage_cell_kernel" if variant1 else "stage_kernel"))
         roof.update({
-            "traffic": traffic_kernel.get(dom), "traffic_source": os.path.relpath(NCU_METRICS_CSV, ROOT) if dom in traffic_kernel else None,
+            "traffic": traffic_kernel.get(dom), "traffic_source": os.path.relpath(page, ROOT) if dom in traffic_kernel else None,
             "kernel": "%s (%s)" % (kname, dom), "launch_ms": prof[dom],
             "peak_source": ("FP32 FMA microbenchmark, same run (vh_measure_fp32_peak)" if f32 else "FP64 FMA microbenchmark, same run (vh_measure_peaks)") if roof["bound"] == "alu" else hbm_src,
             "numerator": "min(minimal algorithmic flops, executed flops) of this kernel per cell x cells per launch" if dom in ex_kernel else
@@ -512,10 +526,10 @@ def main():
             "op_mix_per_cell_update": {k: round(v, 1) for k, v in mix.items()},
             "hbm_view": {"achieved_gbs": bytes_launch / dur / 1e9, "peak_gbs": hbm_peak, "peak_source": hbm_src, "frac": bytes_launch / dur / 1e9 / hbm_peak,
                          "copy_gbs_same_run": copy_gbs},
-            "step_roofline_ms": step_roof_s * 1e3, "step_frac": step_roof_s / (ms / K * 1e-3),
+            "step_roofline_ms": step_roof_s * 1e3, "step_frac": step_roof_s / (ms / K * 1e-3) if len(ex_kernel) == len(cand) else None,
             "per_kernel_ms": prof,
             "per_kernel": {k: {"ms": prof[k], "alg_flops_per_cell": alg_kernel[k], "executed_flops_per_cell": ex_kernel.get(k),
-                               "frac": useful[k] * ncell / (prof[k] * 1e-3) / (alu_gflops * 1e9), "fp64_pipe_util": pipe_kernel.get(k),
+                               "frac": useful[k] * ncell / (prof[k] * 1e-3) / (alu_gflops * 1e9) if k in ex_kernel else None, "fp64_pipe_util": pipe_kernel.get(k),
                                "traffic": traffic_kernel.get(k), "alg_bytes": bytes_kernel[k] * ncell} for k in cand},
         })
         line = {

@@ -137,14 +137,19 @@ def test_committed_ncu_metrics_file_is_what_bench_reads():
     sys.path.insert(0, ROOT)
     import bench
 
-    m = bench.ncu_metrics()
-    assert list(m) == list(bench.LAUNCH_KEYS)
-    ncell = 128 ** 3
-    for key, row in m.items():
-        assert ("velocity" in key) == ("velocity" in row["kernel"])
-        flops = (2 * row["smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"] + row["smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"]
-                 + row["smsp__sass_thread_inst_executed_op_dmul_pred_on.sum"]) / ncell
-        assert 500 < flops < 5000, (key, flops)
-        assert 0.2 < row["sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"] / 100 < 1.0
-        traffic = row["dram__bytes_read.sum"] + row["dram__bytes_write.sum"]
-        assert 1e8 < traffic < 3e9
+    pages = {"config3": 128 ** 3, "config4": 256 * 201 * 201, "config5": 512 * 512 * 128, "paper": 128 ** 3}
+    for tag, ncell in pages.items():
+        page = bench.metrics_page(workload=tag if tag.startswith("config") else "config3", physics="paper" if tag == "paper" else "config3")
+        assert page and os.path.exists(page), tag
+        m = bench.ncu_metrics(page)
+        assert list(m) == list(bench.LAUNCH_KEYS), tag
+        for key, row in m.items():
+            assert ("velocity" in key) == ("velocity" in row["kernel"])
+            flops = (2 * row["smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"] + row["smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"]
+                     + row["smsp__sass_thread_inst_executed_op_dmul_pred_on.sum"]) / ncell
+            assert 500 < flops < 5000, (tag, key, flops)
+            assert 0.2 < row["sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"] / 100 < 1.0
+            traffic = (row["dram__bytes_read.sum"] + row["dram__bytes_write.sum"]) / ncell
+            assert 50 < traffic < 1500, (tag, key, traffic)
+    # no page, no fraction: single precision, reduced storage and the A/B kernel variants have none
+    assert bench.metrics_page(precision="f32") is None and bench.metrics_page(storage=1) is None and bench.metrics_page(variant=1) is None
