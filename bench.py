@@ -275,6 +275,51 @@ def run_reference(args):
     return 0
 
 
+def run_small(args, vh, torch, dev, rank):
+    """configs[0] (1d shock tube, 200 cells, 100 steps) and configs[1] (2+1d viscous Gubser, 201^2, 400 steps) of BASELINE.json: wall time
+    of the WHOLE run, CUDA events around vh_step(n_steps) after one untimed run, best of five; the serial oracle's
+    full run beside it.  Labelled extra lines: these grids are launch-bound (a step is four launches of a few microseconds of work), so no
+    roofline fraction is printed."""
+    if rank != 0:
+        return 0
+    if args.workload == "config1":
+        prm, init, n_steps, _ = inputs.config_shocktube()
+        what = "configs[0] (labelled extra line): 1d ideal shock tube, 200 cells, 100 steps"
+    else:
+        prm, init, n_steps, _ = inputs.config_gubser()
+        what = "configs[1] (labelled extra line): 2+1d conformal viscous Gubser flow, 201x201, 400 steps"
+    t = lambda a: None if a is None else torch.as_tensor(a, device=dev)
+    s = vh.Solver(prm, device=dev)
+    arrays = (t(init["e"]), t(init["u"]), t(init.get("pi")), t(init.get("Pi")))
+    best, launches = None, 0
+    for rep in range(6):                      # rep 0 is the warm-up run
+        s.set_initial(*arrays)
+        torch.cuda.synchronize()
+        n0 = s.launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(); s.step(n_steps); ev1.record()
+        torch.cuda.synchronize()
+        launches = s.launch_count() - n0
+        if rep > 0:
+            best = ev0.elapsed_time(ev1) if best is None else min(best, ev0.elapsed_time(ev1))
+    st = s.status()
+    s.close()
+    ncell = prm["nx"] * prm["ny"] * prm["nz"]
+    line = {"metric": METRIC.replace("at 128^3 viscous", "whole run of " + args.workload), "value": ncell * n_steps / (best * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": n_steps, "warmup": n_steps, "ms_per_step": best / n_steps, "run_ms": best, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": what}, "gpu_launches": int(launches), "roofline": None,
+            "status": {"n_inversion_failures": st["n_inversion_failures"], "n_nonfinite": st["n_nonfinite"]}}
+    if not args.no_cpu_baseline:
+        sys.path.insert(0, os.path.join(ROOT, "oracle"))
+        import vh_oracle
+        o = vh_oracle.Oracle(prm)
+        o.set_initial(init["e"], init["u"], init.get("pi"), init.get("Pi"))
+        t0 = time.perf_counter(); o.step(n_steps); dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": ncell * n_steps / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": "the full run, serial C++ oracle -O2, 1 core", "seconds": dt}
+    print(json.dumps(line))
+    return 0
+
+
 def run_slab(args, vh, torch, dist, dev, rank, world, local):
     """ONE grid split into eta-slabs, one per rank, neighbour exchange of boundary planes after every kernel (vh.SlabSolver):
     strong scaling.  A labelled extra line - the default N > 1 mode stays independent replicas (north_star: no sharding).  The same event on
@@ -333,7 +378,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-paper-physics", action="store_true", help="skip the second, labelled measurement with the lattice EOS and Eq. 17 zeta/s")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"], help="f32: the single-precision build (libvh_f32.so; SURVEY 8(f) NEXT-3), a labelled extra line")
-    ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config5"],
+    ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config5", "config1", "config2"],
                     help="config4 (256 batched 2+1d events) / config5 (512x512x128): labelled extra lines; the default is the BASELINE.json metric")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (the default: BASELINE.json north_star fixes one GPU, no sharding) or ONE grid split into eta-slabs "
@@ -365,6 +410,8 @@ def main():
 
     if args.decomposition == "slab":
         return run_slab(args, vh, torch, dist, dev, rank, world, local)
+    if args.workload in ("config1", "config2"):
+        return run_small(args, vh, torch, dev, rank)
     prm, init = workload(rank, args.physics, args.workload)
     other = (args.workload != "config3")
     f32 = (args.precision == "f32")
